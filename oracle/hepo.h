@@ -1,0 +1,117 @@
+/*
+ * hepo.h — CPU ORACLE for the columnar HEP kernels of arXiv:1906.06242.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call this library.  It shares no code with the CUDA
+ * path (paper_1906_06242_b200/, include/hepk.h) and neither includes the other.
+ *
+ * Every function is a plain per-event loop in the paper's own order (Listing 1,
+ * loop over events, skip masked rows, loop over the event's particles
+ * between offsets[iev] and offsets[iev+1], skip masked particles).  All pointers are HOST
+ * pointers.  Return value: 0 = OK, -1 = invalid argument.
+ *
+ * Two result classes:
+ *   exact class     masks, counts, indices, bin slots, max/min: float32 expression tree,
+ *                   one IEEE round-to-nearest op per node, no FMA contraction
+ *                   (build with -ffp-contract=off, no -ffast-math);
+ *   tolerance class sums, masses, weighted bins: float64 accumulation from the float32
+ *                   inputs, rounded once to float32.
+ *
+ * Pinned by tests/test_oracle_*.py (closed forms, brute force, numpy special cases,
+ * invariants).  Conventions the paper is silent on (empty-event sentinels, out-of-range lookup
+ * policy, NaN routing, electron cut, the 30 variables of config 4) are DESIGN.md readings and
+ * are marked "parity unpinned" there and below.
+ */
+#ifndef HEPO_H
+#define HEPO_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* PAPER.md:L132 "object selection based on cuts on objects: jet, lepton selection based on pT, eta".
+ * out[i] = (pt[i] > pt_min) && (|eta[i]| < abs_eta_max); eta == NULL drops the second term. */
+int32_t hepo_select_mask(const float* pt, const float* eta, int64_t n, float pt_min, float abs_eta_max,
+                         uint8_t* out_mask);
+
+/* Listing 1 and the generic kernels sum/max/min_in_offsets.
+ * Element for global index g is data[g - content_base].  mask_rows / mask_content may be NULL (all true).
+ * Outputs are overwritten for every event.  Empty values: sum 0.0f, count 0, max -inf, min +inf,
+ * argmax -1 (parity unpinned: the paper does not say). */
+int32_t hepo_segmented_reduce_sum(const float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                                  const uint8_t* mask_rows, const uint8_t* mask_content, float* out);
+int32_t hepo_segmented_reduce_max(const float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                                  const uint8_t* mask_rows, const uint8_t* mask_content, float* out);
+int32_t hepo_segmented_reduce_min(const float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                                  const uint8_t* mask_rows, const uint8_t* mask_content, float* out);
+int32_t hepo_segmented_reduce_count(const float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                                    const uint8_t* mask_rows, const uint8_t* mask_content, int32_t* out);
+int32_t hepo_segmented_reduce_argmax(const float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                                     const uint8_t* mask_rows, const uint8_t* mask_content, int32_t* out);
+
+/* mask_deltar_first: out_matched[j] = 1 iff object j of collection 1 is selected and some
+ * selected object of collection 2 in the same event has dR^2 = deta^2 + dphi^2 < dr_max^2. */
+int32_t hepo_deltar_mask(const float* eta1, const float* phi1, const int64_t* offsets1, int64_t base1, const uint8_t* sel1,
+                         const float* eta2, const float* phi2, const int64_t* offsets2, int64_t base2, const uint8_t* sel2,
+                         int64_t n_events, float dr_max, uint8_t* out_matched);
+
+/* Invariant mass of the two highest-pt selected particles per event (coordinates pT, eta, phi, M:
+ * PAPER.md:L11; candidate-mass step: PAPER.md:L136; "first two ... ordered by pT": PAPER.md:L105). */
+int32_t hepo_pair_invmass(const float* pt, const float* eta, const float* phi, const float* mass,
+                          const int64_t* offsets, int64_t n_events, int64_t content_base, const uint8_t* mask_content,
+                          float* out_mass, int32_t* out_i1, int32_t* out_i2);
+
+/* get_bin_contents: out[i] = table[bin_x(x[i]) * ny + bin_y(y[i])]; y == NULL -> 1-D. */
+int32_t hepo_lookup_binned(const float* x, const float* y, int64_t n,
+                           const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                           const float* table, float* out);
+
+/* fill_histogram.  sumw/counts have nbins+2 slots [under, bins..., over] and accumulate. */
+int32_t hepo_fill_histogram(const float* data, const float* weights, int64_t n,
+                            const float* edges, int32_t nbins, float* sumw, int64_t* counts);
+
+/* ---- fused chain (PAPER.md:L129-139 for the analysis steps) ---- */
+enum { HEPO_OBS_NJET = 0, HEPO_OBS_HT, HEPO_OBS_MAXPT, HEPO_OBS_MINPT, HEPO_OBS_MJJ, HEPO_OBS_SUBPT, HEPO_N_OBS };
+
+typedef struct {
+    const int64_t* offsets;   /* [n_events+1]; NULL = collection absent */
+    int64_t content_base;
+    int64_t n_objects;
+    const float* pt;
+    const float* eta;
+    const float* phi;
+    const float* mass;        /* only read for jets */
+} hepo_collection;
+
+typedef struct {
+    int64_t n_events;
+    hepo_collection jets, muons, electrons;
+    float jet_pt_min, jet_abs_eta_max, lep_pt_min, dr_max;
+    /* calibration; calib_table == NULL -> none and n_variants must be 1 */
+    const float* calib_pt_edges;  int32_t calib_npt;
+    const float* calib_eta_edges; int32_t calib_neta;
+    const float* calib_table;     /* [npt][neta] */
+    const float* calib_scales;    /* [n_variants] */
+    int32_t n_variants;
+    int32_t n_wvar;
+    const float* weights;         /* [n_wvar][n_events]; NULL -> weight 1 */
+    const float* axis_edges[HEPO_N_OBS];   /* NULL -> observable not histogrammed */
+    int32_t axis_nbins[HEPO_N_OBS];
+    /* per-event outputs, each [n_variants][n_events], all nullable */
+    int32_t* out_njet; int32_t* out_argmax;
+    float* out_ht; float* out_maxpt; float* out_minpt; float* out_mjj; float* out_subpt;
+    uint8_t* out_jet_mask;        /* [n_variants][jets.n_objects] clean-jet mask */
+    /* histograms (accumulate): sumw [V][active obs o][n_wvar][nbins_o+2]; counts [V][active obs o][nbins_o+2] */
+    float* hist_sumw; int64_t* hist_counts;
+} hepo_chain_desc;
+
+int32_t hepo_analysis_chain(const hepo_chain_desc* d);
+size_t  hepo_chain_desc_size(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
