@@ -1,0 +1,246 @@
+// hepk_common.cuh — shared host/device helpers of libhepk (sm_100a only).
+//
+// Nothing here is shared with the CPU oracle (oracle/): the two sides have independent sources.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/hepk.h"
+
+// ------------------------------------------------------------------------------------------ host side
+namespace hepk {
+
+void set_error(const char* fmt, ...);
+int32_t cuda_fail(cudaError_t e, const char* what);
+int sm_count();                 // SMs of the current device (cached per device)
+int max_smem_optin();           // max opt-in dynamic shared memory per CTA
+
+#define HEPK_CUDA_TRY(call)                                         \
+    do {                                                            \
+        cudaError_t _e = (call);                                    \
+        if (_e != cudaSuccess) return ::hepk::cuda_fail(_e, #call); \
+    } while (0)
+
+#define HEPK_REQUIRE(cond, msg)                              \
+    do {                                                     \
+        if (!(cond)) {                                       \
+            ::hepk::set_error("%s: %s", __func__, msg);      \
+            return HEPK_ERR_INVALID;                         \
+        }                                                    \
+    } while (0)
+
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace hepk
+
+// ------------------------------------------------------------------------------------------ device side
+namespace hepk {
+namespace dev {
+
+// float32 constants of the dphi wrap: PI_F = 0x40490FDB, TWO_PI_F = 0x40C90FDB (R6).
+#define HEPK_PI_F 3.14159274101257324f
+#define HEPK_TWO_PI_F 6.28318548202514648f
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+
+// ---- mbarrier + TMA 1-D bulk copy (cp.async.bulk, SASS UBLKCP) -------------------------------
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void fence_mbar_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+// generic-proxy accesses to shared memory before this point are ordered before later async-proxy (TMA) accesses
+__device__ __forceinline__ void fence_proxy_async_smem()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// global -> shared bulk copy; dst, src 16-byte aligned, bytes a multiple of 16
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---- staging a slice [l0, l1) of a column into shared memory -----------------------------------
+// Element l of `col` lands at dst[l - a0], a0 <= l0 chosen so that the 16-byte aligned body of the slice
+// can be moved by ONE bulk copy; the ragged head (col not 16-byte aligned near element 0) and the tail
+// beyond the last full 16-byte group of the column go through ordinary loads.  Works for any
+// sizeof(T)-aligned column pointer.  dst must be 16-byte aligned with room for (l1-l0) + 2*(16/sizeof(T)) elements.
+template <typename T>
+struct StageGeom {
+    static constexpr int A = 16 / (int)sizeof(T);
+    long long a0;      // column index mapped to dst[0] (may be negative)
+    long long bulk0;   // bulk body [bulk0, bulk1)
+    long long bulk1;
+    __device__ __forceinline__ StageGeom(const T* col, long long l0, long long l1, long long n_total)
+    {
+        const int mis = (int)((reinterpret_cast<uintptr_t>(col) / sizeof(T)) % A);
+        a0 = l0 - ((l0 + mis) % A);
+        long long first = a0 < 0 ? a0 + A : a0;
+        long long ceil1 = l1 + ((A - (int)((l1 + mis) % A)) % A);
+        long long floorn = n_total - ((n_total + mis) % A);
+        long long last = ceil1 < floorn ? ceil1 : floorn;
+        bulk0 = first;
+        bulk1 = last > first ? last : first;
+    }
+};
+
+// Issue the copies of one column.  Called by ALL threads of the CTA (uniform arguments).
+// Thread `issuer` issues the bulk copy and returns its byte count (others return 0); the scalar head/tail
+// elements are copied by the first few threads and become visible at the next __syncthreads().
+template <typename T>
+__device__ __forceinline__ uint32_t stage_column(T* dst, const T* __restrict__ col, long long l0, long long l1,
+                                                 long long n_total, uint64_t* bar, int tid, int issuer,
+                                                 long long* a0_out)
+{
+    StageGeom<T> g(col, l0, l1, n_total);
+    *a0_out = g.a0;
+    uint32_t bytes = 0;
+    if (tid == issuer && g.bulk1 > g.bulk0 && l1 > l0) {
+        bytes = (uint32_t)((g.bulk1 - g.bulk0) * (long long)sizeof(T));
+        bulk_g2s(dst + (g.bulk0 - g.a0), col + g.bulk0, bytes, bar);
+    }
+    // scalar head [l0, min(bulk0, l1)) and tail [max(bulk1, l0), l1)
+    const long long head_end = g.bulk0 < l1 ? g.bulk0 : l1;
+    const long long head_n = head_end > l0 ? head_end - l0 : 0;
+    const long long tail_beg = g.bulk1 > l0 ? g.bulk1 : l0;
+    const long long tail_n = (l1 > tail_beg && g.bulk0 <= l1) ? l1 - tail_beg : 0;
+    if (tid < head_n) dst[l0 + tid - g.a0] = col[l0 + tid];
+    else if (tid < head_n + tail_n) dst[tail_beg + (tid - head_n) - g.a0] = col[tail_beg + (tid - head_n)];
+    return bytes;
+}
+
+// ---- exact-class float32 arithmetic (one IEEE rn operation per node, never contracted) ------------
+// dR^2 = deta^2 + dphi^2 with the single-step phi wrap.  |dphi| > PI_F  <=>  the oracle's two-sided test
+// (dphi > PI_F or dphi <= -PI_F), except at dphi == -PI_F exactly, where (-PI_F + 2PI_F)^2 == PI_F^2 ==
+// (-PI_F)^2 bit for bit; and (|d| - 2PI_F)^2 == (d -/+ 2PI_F)^2 because negation is exact.
+__device__ __forceinline__ float dr2_exact(float eta_a, float phi_a, float eta_b, float phi_b)
+{
+    const float deta = __fsub_rn(eta_a, eta_b);
+    const float ad = fabsf(__fsub_rn(phi_a, phi_b));
+    const float w = ad > HEPK_PI_F ? __fsub_rn(ad, HEPK_TWO_PI_F) : ad;
+    return __fadd_rn(__fmul_rn(deta, deta), __fmul_rn(w, w));
+}
+
+// B(v): b with edges[b] <= v < edges[b+1]; clamped (v < edges[0] -> 0; v >= edges[n] or NaN -> n-1).
+__device__ __forceinline__ int find_bin_clamped(float v, const float* edges, int n)
+{
+    if (v < edges[0]) return 0;
+    if (!(v < edges[n])) return n - 1;
+    int lo = 0, hi = n;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (v >= edges[mid]) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// Histogram slot: 0 underflow, 1+b, nbins+1 overflow/NaN.  Arithmetic guess for (near-)uniform axes,
+// verified against the edges; anything the guess gets wrong falls back to the binary search, so the
+// result is exact for any ascending edges.
+__device__ __forceinline__ int hist_slot(float x, const float* edges, int nbins, float lo, float inv_w)
+{
+    if (x < lo) return 0;
+    if (!(x < edges[nbins])) return nbins + 1;
+    int g = (int)((x - lo) * inv_w);
+    g = g < 0 ? 0 : (g > nbins - 1 ? nbins - 1 : g);
+    if (edges[g] <= x) {
+        if (x < edges[g + 1]) return 1 + g;
+        if (g + 2 <= nbins && x < edges[g + 2]) return 2 + g;
+    } else if (g > 0 && edges[g - 1] <= x) {
+        return g;
+    }
+    int a = 0, b = nbins;
+    while (b - a > 1) {
+        const int mid = (a + b) >> 1;
+        if (x >= edges[mid]) a = mid; else b = mid;
+    }
+    return 1 + a;
+}
+
+// ---- tolerance-class float32 pair mass, cancellation-free form ---------------------------------
+// M^2 = m1^2 + m2^2 + 2 pt1 pt2 [ ch1 ch2 t + 2 (sinh^2(deta/2) + sin^2(dphi/2)) ],
+//   ch_i = cosh(eta_i), x_i = (m_i / (pt_i ch_i))^2, x = x1 + x2 + x1 x2, t = x / (sqrt(1+x) + 1)
+// which equals (E1+E2)^2 - |p1+p2|^2 for E = sqrt(pt^2 cosh^2 eta + m^2) with every term >= 0
+// (DESIGN.md "pair mass"): E1E2 = pt1 pt2 ch1 ch2 (1+t), cosh(deta) - cos(dphi) = 2 sinh^2 + 2 sin^2.
+// dphi is reduced to [-pi, pi] with an error-free subtraction and a two-term 2*pi so that jets
+// straddling the +-pi seam keep full relative accuracy.
+__device__ __forceinline__ float pair_mass_f32(float pt1, float eta1, float phi1, float m1,
+                                               float pt2, float eta2, float phi2, float m2)
+{
+    const float e1 = expf(eta1), e2 = expf(eta2);
+    const float ch1 = 0.5f * (e1 + 1.0f / e1);
+    const float ch2 = 0.5f * (e2 + 1.0f / e2);
+    // sinh(deta/2) through expm1 (no cancellation for small deta)
+    const float hx = 0.5f * fabsf(eta1 - eta2);
+    const float em1 = expm1f(hx);
+    const float sh = 0.5f * (em1 + em1 / (em1 + 1.0f));
+    // dphi = phi1 - phi2 as an unevaluated sum d + dl (TwoSum), wrapped by 2*pi = TWO_PI_F + TWO_PI_LO
+    float d = __fsub_rn(phi1, phi2);
+    const float bb = __fsub_rn(d, phi1);
+    float dl = __fsub_rn(__fsub_rn(phi1, __fsub_rn(d, bb)), __fadd_rn(phi2, bb));
+    const float TWO_PI_LO = -1.7484555e-07f;   // 2*pi - TWO_PI_F
+    if (d > HEPK_PI_F) { d = __fsub_rn(d, HEPK_TWO_PI_F); dl = __fsub_rn(dl, TWO_PI_LO); }
+    else if (d < -HEPK_PI_F) { d = __fadd_rn(d, HEPK_TWO_PI_F); dl = __fadd_rn(dl, TWO_PI_LO); }
+    const float sn = sinf(0.5f * (d + dl));
+    const float r1 = m1 / (pt1 * ch1), r2 = m2 / (pt2 * ch2);
+    const float x1 = r1 * r1, x2 = r2 * r2;
+    const float x = x1 + x2 + x1 * x2;
+    const float t = x / (sqrtf(1.0f + x) + 1.0f);
+    const float bracket = ch1 * ch2 * t + 2.0f * (sh * sh + sn * sn);
+    const float msq = m1 * m1 + m2 * m2 + 2.0f * pt1 * pt2 * bracket;
+    return sqrtf(fmaxf(msq, 0.0f));
+}
+
+// ---- per-event running state of the reductions (count, sum, min, top-2 with first-index ties) ------
+struct Top2 {
+    float b1, b2;
+    int i1, i2;
+    __device__ __forceinline__ void init() { b1 = b2 = -CUDART_INF_F; i1 = i2 = -1; }
+    // strict > keeps the smallest index among equal values, for both places
+    __device__ __forceinline__ void push(float p, int k)
+    {
+        if (p > b1) { b2 = b1; i2 = i1; b1 = p; i1 = k; }
+        else if (p > b2) { b2 = p; i2 = k; }
+    }
+    // general data (may hold NaN or -inf): NaN skipped, the first element always taken (oracle's argmax rule)
+    __device__ __forceinline__ void push_any(float p, int k)
+    {
+        if (p != p) return;
+        if (i1 < 0 || p > b1) { b2 = b1; i2 = i1; b1 = p; i1 = k; }
+        else if (i2 < 0 || p > b2) { b2 = p; i2 = k; }
+    }
+};
+
+}  // namespace dev
+}  // namespace hepk

@@ -1,0 +1,224 @@
+"""Parity of the fused CUDA chain (hepk_analysis_chain / hepk_analysis_chain_host, through the C ABI)
+against the CPU oracle's chain on the same seeded events.  Exact class: jet masks, njet, argmax, maxpt,
+minpt, histogram counts.  Tolerance class (1e-5 rel, 1e-6 abs): ht, mjj, subpt(exact in fact), weighted bins."""
+import numpy as np
+import pytest
+import torch
+
+import hepgen
+from oracle import hepo
+from _util import assert_exact, assert_tol, to_np
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hk():
+    from paper_1906_06242_b200 import binding
+    binding.lib()
+    return binding
+
+
+def compare(out, ref, wl, plan=None, e0=0, e1=None, check_hists=True, what=""):
+    sl = slice(e0, e1)
+    for k in ("njet", "argmax", "maxpt", "minpt", "subpt"):
+        assert_exact(to_np(out[k])[:, sl] if e1 else to_np(out[k]), ref[k], f"{what}{k}")
+    for k in ("ht", "mjj"):
+        assert_tol(to_np(out[k])[:, sl] if e1 else to_np(out[k]), ref[k], f"{what}{k}")
+    if "jet_mask" in out and "jet_mask" in ref:
+        assert_exact(to_np(out["jet_mask"]), ref["jet_mask"], f"{what}jet_mask")
+    if check_hists:
+        assert_exact(to_np(out["hist_counts"]), ref["hist_counts"], f"{what}hist_counts")
+        assert_tol(to_np(out["hist_sumw"]), ref["hist_sumw"], f"{what}hist_sumw")
+
+
+def run_gpu(hk, wl, **kw):
+    inp = hk.upload(wl)
+    out, plan = hk.analysis_chain(inp, want_mask=True, **kw)
+    torch.cuda.synchronize()
+    return out, plan
+
+
+@pytest.mark.parametrize("config,n", [(0, None), (1, 200_037), (2, 300_011), (3, 100_003), (4, 30_001)])
+def test_chain_matches_oracle(hk, config, n):
+    wl = hepgen.generate(config, n_events=n)
+    ref = hepo.analysis_chain(wl)
+    out, plan = run_gpu(hk, wl)
+    compare(out, ref, wl)
+    # invariants on the device result itself
+    for name in wl.hists:
+        sw, ct = plan.hist_view(name)
+        assert (to_np(ct).sum(axis=1) == wl.n_events).all()
+
+
+def test_chain_is_repeatable_and_accumulates(hk):
+    wl = hepgen.generate(2, n_events=50_000)
+    ref = hepo.analysis_chain(wl, want_mask=False)
+    inp = hk.upload(wl)
+    plan = hk.ChainPlan(inp)
+    plan.run(); plan.run()
+    torch.cuda.synchronize()
+    assert_exact(to_np(plan.out["hist_counts"]), 2 * ref["hist_counts"])       # histograms accumulate
+    assert_tol(to_np(plan.out["hist_sumw"]), 2.0 * ref["hist_sumw"].astype(np.float64))
+    assert_exact(to_np(plan.out["njet"]), ref["njet"])                          # per-event outputs are overwritten
+
+
+@pytest.mark.parametrize("tune", [dict(cap_jets=64, cap_leptons=32), dict(cap_jets=300, cap_leptons=16),
+                                  dict(cap_jets=4096, cap_leptons=1024, ctas_per_sm=1)])
+def test_chain_small_buffers_cut_tiles_and_giant_events(hk, tune):
+    """Staging buffers far smaller than a tile: tiles are processed in pieces, and events larger than the
+    buffers go through the per-event global-memory path.  Results must not change."""
+    for config in (2, 3):
+        wl = hepgen.generate(config, n_events=6_000)
+        ref = hepo.analysis_chain(wl)
+        out, _ = run_gpu(hk, wl, tune=tune)
+        compare(out, ref, wl, what=f"cfg{config} {tune} ")
+
+
+def _custom(n, cj, cm, ce, seed=0, config=2):
+    """Workload with prescribed multiplicities."""
+    wl = hepgen.generate(config, n_events=n, seed=seed)
+    rng = np.random.default_rng(seed + 100)
+
+    def coll(counts, mass):
+        off = np.zeros(n + 1, np.int64)
+        off[1:] = np.cumsum(counts)
+        m = int(off[-1])
+        return hepgen.Collection(off, (20 + rng.exponential(30, m)).astype(np.float32),
+                                 rng.uniform(-2.5, 2.5, m).astype(np.float32),
+                                 rng.uniform(-np.pi, np.pi, m).astype(np.float32),
+                                 (rng.exponential(10, m) if mass is None else np.full(m, mass)).astype(np.float32))
+    wl.jets, wl.muons = coll(cj, None), coll(cm, 0.1057)
+    wl.electrons = coll(ce, 0.000511) if ce is not None else None
+    return wl
+
+
+def test_chain_edge_multiplicities(hk):
+    n = 3000
+    rng = np.random.default_rng(1)
+    z = np.zeros(n, np.int64)
+    cases = {
+        "no_jets_at_all": (z, rng.poisson(1.5, n), rng.poisson(1, n)),
+        "no_leptons_at_all": (rng.poisson(8, n), z, z),
+        "everything_empty": (z, z, z),
+        "all_at_cap": (np.full(n, 40), np.full(n, 6), np.full(n, 6)),
+        "no_electron_collection": (rng.poisson(8, n), rng.poisson(1.5, n), None),
+        "single_jet_events": (np.ones(n, np.int64), rng.poisson(1.5, n), rng.poisson(1, n)),
+    }
+    g = rng.poisson(8, n)
+    g[17], g[1500], g[2999] = 3000, 700, 5000          # giant events (first tile, middle, last event)
+    gm = rng.poisson(1.5, n)
+    gm[1501] = 900                                     # giant lepton event
+    cases["giant_events"] = (g, gm, rng.poisson(1, n))
+    for name, (cj, cm, ce) in cases.items():
+        wl = _custom(n, cj, cm, ce, seed=3)
+        ref = hepo.analysis_chain(wl)
+        out, _ = run_gpu(hk, wl)
+        compare(out, ref, wl, what=name + " ")
+    for n1 in (1, 2, 127, 128, 129):
+        wl = hepgen.generate(2, n_events=n1, seed=9)
+        compare(run_gpu(hk, wl)[0], hepo.analysis_chain(wl), wl, what=f"n={n1} ")
+
+
+def test_chain_ties_and_threshold_values(hk):
+    """Hand-built ties (equal pt) and values sitting exactly on the cuts and on bin edges."""
+    n = 4000
+    rng = np.random.default_rng(2)
+    wl = _custom(n, rng.poisson(6, n) + 2, rng.poisson(1.5, n), rng.poisson(1, n), seed=5)
+    j = wl.jets
+    pt = j.pt
+    for e in range(0, n, 3):                           # equal leading pts -> first index must win, next is subleading
+        a, b = j.offsets[e], j.offsets[e + 1]
+        k = rng.integers(2, b - a + 1)
+        idx = rng.choice(np.arange(a, b), size=k, replace=False)
+        pt[idx] = np.float32(200.0)
+    pt[rng.random(pt.size) < 0.02] = np.float32(30.0)                      # exactly on the pt cut (fails: strict >)
+    j.eta[rng.random(pt.size) < 0.02] = np.float32(2.4)                    # exactly on the eta cut
+    j.eta[rng.random(pt.size) < 0.02] = np.float32(-2.4)
+    pt[rng.random(pt.size) < 0.02] = np.float32(500.0)                     # on the last edge of the maxpt axis -> overflow
+    ref = hepo.analysis_chain(wl)
+    out, _ = run_gpu(hk, wl)
+    compare(out, ref, wl)
+    assert (ref["argmax"][0] >= 0).sum() > 1000
+
+
+def test_chain_misaligned_columns_and_content_base(hk):
+    """Columns that are only 4-byte aligned, and an event range given as an offsets slice plus content_base."""
+    wl = hepgen.generate(2, n_events=20_000, seed=4)
+    e0, e1 = 4_001, 17_777
+    ref = hepo.analysis_chain(wl, e0, e1)
+    inp = hk.upload(wl)
+
+    def shifted(t, s):
+        buf = torch.empty(t.numel() + 8, dtype=t.dtype, device="cuda")
+        v = buf[s: s + t.numel()]
+        v.copy_(t)
+        return v
+
+    def cut(c, wlc, shifts):
+        g0, g1 = int(wlc.offsets[e0]), int(wlc.offsets[e1])
+        cols = [shifted(getattr(c, nm)[g0:g1].contiguous(), s) for nm, s in zip(("pt", "eta", "phi", "mass"), shifts)]
+        return hk.DeviceCollection(c.offsets[e0:e1 + 1].contiguous(), *cols, content_base=g0)
+    inp.jets = cut(inp.jets, wl.jets, (1, 2, 3, 1))
+    inp.muons = cut(inp.muons, wl.muons, (3, 0, 1, 2))
+    inp.electrons = cut(inp.electrons, wl.electrons, (2, 2, 1, 0))
+    inp.weights = inp.weights[:, e0:e1].contiguous()
+    inp.n_events = e1 - e0
+    out, plan = hk.analysis_chain(inp, want_mask=True)
+    torch.cuda.synchronize()
+    g0, g1 = int(wl.jets.offsets[e0]), int(wl.jets.offsets[e1])
+    ref["jet_mask"] = ref["jet_mask"][:, g0:g1]
+    compare(out, ref, wl)
+
+
+def test_chain_optional_outputs(hk):
+    wl = hepgen.generate(1, n_events=20_000)
+    ref = hepo.analysis_chain(wl, want_mask=False)
+    inp = hk.upload(wl)
+    out, _ = hk.analysis_chain(inp, want_event_outputs=False)              # histograms only
+    torch.cuda.synchronize()
+    assert_exact(to_np(out["hist_counts"]), ref["hist_counts"])
+    assert_tol(to_np(out["hist_sumw"]), ref["hist_sumw"])
+    out, _ = hk.analysis_chain(inp, want_hists=False)                      # per-event outputs only
+    torch.cuda.synchronize()
+    compare(out, ref, wl, check_hists=False)
+    inp.weights = None                                                      # weights NULL -> sumw == counts
+    out, plan = hk.analysis_chain(inp)
+    torch.cuda.synchronize()
+    assert_exact(to_np(out["hist_sumw"]), ref["hist_counts"].astype(np.float32))
+
+
+@pytest.mark.parametrize("overlap", [False, True])
+def test_chain_host_streaming(hk, overlap):
+    """hepk_analysis_chain_host: host buffers in, host buffers out, batches with and without copy/compute overlap."""
+    for config, n, batch in ((2, 100_003, 30_000), (4, 20_001, 7_000)):
+        wl = hepgen.generate(config, n_events=n)
+        ref = hepo.analysis_chain(wl, want_mask=False)
+        plan = hk.HostChainPlan(wl, batch_events=batch)
+        out = plan.run(overlap=overlap)
+        compare({k: v for k, v in out.items()}, ref, wl, what=f"cfg{config} ")
+        out = plan.run(overlap=overlap)                                    # histograms accumulate on the host side too
+        assert_exact(to_np(out["hist_counts"]), 2 * ref["hist_counts"])
+
+
+def test_chain_full_size_config2_sampled(hk):
+    """BASELINE.json config 2 at full size (10 M events) in the launch configuration bench.py times:
+    per-event outputs on sampled event ranges the oracle recomputes, histogram counts over ALL events."""
+    wl = hepgen.generate(2)
+    inp = hk.upload(wl)
+    plan = hk.ChainPlan(inp)
+    plan.run()
+    torch.cuda.synchronize()
+    N = wl.n_events
+    for e0 in (0, 1_234_567, 5_000_001, N - 200_000):
+        ref = hepo.analysis_chain(wl, e0, e0 + 200_000, want_mask=False)
+        out = {k: plan.out[k][:, e0:e0 + 200_000] for k in ("njet", "argmax", "maxpt", "minpt", "subpt", "ht", "mjj")}
+        compare(out, ref, wl, check_hists=False, what=f"events {e0}.. ")
+    ref = hepo.analysis_chain(wl, want_mask=False)
+    assert_exact(to_np(plan.out["hist_counts"]), ref["hist_counts"])
+    assert_tol(to_np(plan.out["hist_sumw"]), ref["hist_sumw"])
+    tot = wl.weights.astype(np.float64).sum()
+    for name in wl.hists:
+        sw, ct = plan.hist_view(name)
+        assert to_np(ct).sum() == N
+        assert abs(to_np(sw).astype(np.float64).sum() - tot) <= 1e-5 * tot
