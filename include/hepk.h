@@ -233,6 +233,16 @@ size_t  hepk_chain_host_workspace_bytes(const hepk_chain_desc* d, int64_t batch_
 int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t batch_events, int32_t overlap,
                                  void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Device-side timing of the dominant kernel (measurement hook for bench.py; no part of the method).
+ * Between hepk_profile_begin() and hepk_profile_end() every hepk_analysis_chain call records a CUDA event
+ * pair on its launch stream directly around the fused chain kernel (at most 4096 launches are kept).
+ * hepk_profile_end() waits for the recorded events, stores the summed kernel time in milliseconds in
+ * *total_ms (HOST pointer) and the number of timed launches in *n_launches (HOST pointer; either may be
+ * NULL), and switches the recording off.  Not thread-safe; one profiling session per process at a time. */
+int32_t hepk_profile_begin(void);
+int32_t hepk_profile_end(double* total_ms, int32_t* n_launches);
+
 #ifdef __cplusplus
 }
 #endif

@@ -86,7 +86,18 @@ def _ptr(t, dtype=None):
     assert isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous(), "expected a contiguous CUDA tensor"
     if dtype is not None:
         assert t.dtype == dtype, (t.dtype, dtype)
+    if t.numel() == 0:          # torch gives empty tensors a NULL data_ptr; the C ABI wants a valid (unread) pointer
+        return C.c_void_p(_empty_buffer(t.device).data_ptr())
     return C.c_void_p(t.data_ptr())
+
+
+_EMPTY = {}
+
+
+def _empty_buffer(device):
+    if device not in _EMPTY:
+        _EMPTY[device] = torch.zeros(16, dtype=torch.uint8, device=device)
+    return _EMPTY[device]
 
 
 def _stream(stream):
@@ -107,6 +118,17 @@ def version():
 
 def last_error():
     return lib().hepk_last_error().decode()
+
+
+def profile_begin():
+    _check(lib().hepk_profile_begin(), "profile_begin")
+
+
+def profile_end():
+    """(summed milliseconds of the fused chain kernel, number of timed launches) since profile_begin()."""
+    ms, n = C.c_double(0.0), C.c_int32(0)
+    _check(lib().hepk_profile_end(C.byref(ms), C.byref(n)), "profile_end")
+    return ms.value, n.value
 
 
 def select_mask(pt, eta, pt_min, abs_eta_max, out=None, stream=None):
@@ -278,8 +300,11 @@ def _fill_collection(s, c):
 class ChainPlan:
     """Pre-built descriptor, outputs and workspace for repeated hepk_analysis_chain calls on fixed buffers."""
 
+    EVENT_OUTPUTS = ("njet", "argmax", "ht", "maxpt", "minpt", "mjj", "subpt")
+
     def __init__(self, inp: ChainInputs, want_event_outputs=True, want_mask=False, want_hists=True, want_counts=True,
                  tune=None):
+        """want_event_outputs: True (all seven), False (none) or a tuple of names from EVENT_OUTPUTS."""
         self.inp = inp
         dev = inp.jets.pt.device
         N, V, W = inp.n_events, inp.n_variants, inp.n_wvar
@@ -306,12 +331,12 @@ class ChainPlan:
             d.weights = inp.weights.data_ptr()
         self.out = {}
         if want_event_outputs:
-            for k in ("njet", "argmax"):
-                self.out[k] = torch.empty((V, N), dtype=torch.int32, device=dev)
-            for k in ("ht", "maxpt", "minpt", "mjj", "subpt"):
-                self.out[k] = torch.empty((V, N), dtype=torch.float32, device=dev)
-            for k, t in self.out.items():
-                setattr(d, "out_" + k, t.data_ptr())
+            names = self.EVENT_OUTPUTS if want_event_outputs is True else tuple(want_event_outputs)
+            for k in names:
+                assert k in self.EVENT_OUTPUTS, k
+                dt = torch.int32 if k in ("njet", "argmax") else torch.float32
+                self.out[k] = torch.empty((V, N), dtype=dt, device=dev)
+                setattr(d, "out_" + k, self.out[k].data_ptr())
         if want_mask:
             self.out["jet_mask"] = torch.zeros((V, inp.jets.pt.numel()), dtype=torch.uint8, device=dev)
             d.out_jet_mask = self.out["jet_mask"].data_ptr()
@@ -410,13 +435,12 @@ class HostChainPlan:
         self.out = {}
         self.d2h_bytes = 0
         if want_event_outputs:
-            for k in ("njet", "argmax"):
-                self.out[k] = torch.empty((V, N), dtype=torch.int32).pin_memory()
-            for k in ("ht", "maxpt", "minpt", "mjj", "subpt"):
-                self.out[k] = torch.empty((V, N), dtype=torch.float32).pin_memory()
-            for k, t in self.out.items():
-                setattr(d, "out_" + k, t.data_ptr())
-                self.d2h_bytes += t.numel() * 4
+            names = ChainPlan.EVENT_OUTPUTS if want_event_outputs is True else tuple(want_event_outputs)
+            for k in names:
+                dt = torch.int32 if k in ("njet", "argmax") else torch.float32
+                self.out[k] = torch.empty((V, N), dtype=dt).pin_memory()
+                setattr(d, "out_" + k, self.out[k].data_ptr())
+                self.d2h_bytes += self.out[k].numel() * 4
         axes = {k: pin(v) for k, v in wl.axes.items()}
         self.axes = axes
         self.prefix, self.spv = hist_layout(wl.hists, axes)

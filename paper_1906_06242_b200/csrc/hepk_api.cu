@@ -39,10 +39,53 @@ static DevInfo& devinfo()
     return d;
 }
 
+// ---- optional device-side timing of the dominant kernel (hepk_profile_begin / hepk_profile_end) -------------
+static const int PROF_MAX = 4096;
+static bool g_prof_on = false;
+static int g_prof_n = 0;
+static cudaEvent_t g_prof_ev[PROF_MAX][2];
+static bool g_prof_created = false;
+
+void profile_mark(cudaStream_t st, int which)
+{
+    if (!g_prof_on || g_prof_n >= PROF_MAX) return;
+    cudaEventRecord(g_prof_ev[g_prof_n][which], st);
+    if (which == 1) g_prof_n++;
+}
+
 int sm_count() { return devinfo().sms; }
 int max_smem_optin() { return devinfo().smem_optin; }
 
 }  // namespace hepk
+
+extern "C" int32_t hepk_profile_begin(void)
+{
+    using namespace hepk;
+    if (!g_prof_created) {
+        for (int i = 0; i < PROF_MAX; ++i)
+            for (int k = 0; k < 2; ++k) HEPK_CUDA_TRY(cudaEventCreate(&g_prof_ev[i][k]));
+        g_prof_created = true;
+    }
+    g_prof_n = 0;
+    g_prof_on = true;
+    return HEPK_OK;
+}
+
+extern "C" int32_t hepk_profile_end(double* total_ms, int32_t* n_launches)
+{
+    using namespace hepk;
+    g_prof_on = false;
+    double tot = 0.0;
+    for (int i = 0; i < g_prof_n; ++i) {
+        float ms = 0.f;
+        HEPK_CUDA_TRY(cudaEventSynchronize(g_prof_ev[i][1]));
+        HEPK_CUDA_TRY(cudaEventElapsedTime(&ms, g_prof_ev[i][0], g_prof_ev[i][1]));
+        tot += ms;
+    }
+    if (total_ms) *total_ms = tot;
+    if (n_launches) *n_launches = g_prof_n;
+    return HEPK_OK;
+}
 
 extern "C" int32_t hepk_version(void) { return 100; }
 extern "C" const char* hepk_last_error(void) { return hepk::g_err; }

@@ -108,6 +108,16 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSm
     if (top.i2 >= 0) {
         subpt = top.b2;
         mjj = pair_mass_f32(top.b1, eta1, phi1, m1, top.b2, eta2, phi2, m2);
+        if (P.axis_edges[HEPK_OBS_MJJ] && (P.hist_acc || P.hist_counts)) {
+            // the bin of mjj is decided by the float64-defined value: refine when the fast value is near an edge
+            const float* ed = S.edges + P.edge_prefix[HEPK_OBS_MJJ];
+            const int nb = P.axis_nbins[HEPK_OBS_MJJ];
+            const int slot = hist_slot(mjj, ed, nb, S.axis_lo[HEPK_OBS_MJJ], S.axis_inv[HEPK_OBS_MJJ]);
+            const float band = fmaf(mjj, HEPK_MASS_GUARD_REL, HEPK_MASS_GUARD_ABS);
+            const bool near_lo = slot >= 1 && mjj - ed[slot - 1] <= band;
+            const bool near_hi = slot <= nb && ed[slot] - mjj <= band;
+            if (near_lo || near_hi) mjj = pair_mass_f64(top.b1, eta1, phi1, m1, top.b2, eta2, phi2, m2);
+        }
     }
     const long long o = (long long)v * P.n_events + ev;
     if (P.out_njet) P.out_njet[o] = cnt;
@@ -157,7 +167,8 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, const Chai
     const long long g0 = P.joff[ev], g1 = P.joff[ev + 1];
     for (int v = 0; v < P.V; ++v) {
         int cnt = 0;
-        float sum = 0.0f, mn = CUDART_INF_F;
+        double sum = 0.0;
+        float mn = CUDART_INF_F;
         Top2 top;
         top.init();
         for (long long g = g0; g < g1; ++g) {
@@ -178,7 +189,7 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, const Chai
             if (P.out_jet_mask) P.out_jet_mask[(long long)v * P.jn + j] = clean ? 1 : 0;
             if (clean) {
                 cnt++;
-                sum += p;
+                sum += (double)p;
                 mn = fminf(mn, p);
                 top.push(p, (int)(g - g0));
             }
@@ -189,7 +200,7 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, const Chai
             e1 = P.jeta[a]; p1 = P.jphi[a]; m1 = P.jmass[a];
             e2 = P.jeta[b]; p2 = P.jphi[b]; m2 = P.jmass[b];
         }
-        finish_event(P, S, ev, v, cnt, sum, mn, top, e1, p1, m1, e2, p2, m2);
+        finish_event(P, S, ev, v, cnt, (float)sum, mn, top, e1, p1, m1, e2, p2, m2);
     }
 }
 
@@ -356,7 +367,8 @@ __global__ void __launch_bounds__(TILE) chain_kernel(const __grid_constant__ Cha
                 for (int v = 0; v < P.V; ++v) {
                     const float sv = P.scales[v];
                     int cnt = 0;
-                    float sum = 0.0f, mn = CUDART_INF_F;
+                    double sum = 0.0;      // float64: exact for these inputs, so HT and its bin do not depend on the order (R15)
+                    float mn = CUDART_INF_F;
                     Top2 top;
                     top.init();
                     for (int k = k0; k < k1; ++k) {
@@ -364,7 +376,7 @@ __global__ void __launch_bounds__(TILE) chain_kernel(const __grid_constant__ Cha
                         if (CALIB) p = __fmul_rn(p, __fmul_rn(S.corr[k], sv));
                         if (p > P.jet_pt_min) {
                             cnt++;
-                            sum += p;
+                            sum += (double)p;
                             mn = fminf(mn, p);
                             top.push(p, k - k0);
                         }
@@ -375,7 +387,7 @@ __global__ void __launch_bounds__(TILE) chain_kernel(const __grid_constant__ Cha
                         e1 = S.jeta[a + sh_eta]; p1 = S.jphi[a + sh_phi]; m1 = S.jmass[a + sh_mass];
                         e2 = S.jeta[b + sh_eta]; p2 = S.jphi[b + sh_phi]; m2 = S.jmass[b + sh_mass];
                     }
-                    finish_event(P, S, e0 + ev0 + tid, v, cnt, sum, mn, top, e1, p1, m1, e2, p2, m2);
+                    finish_event(P, S, e0 + ev0 + tid, v, cnt, (float)sum, mn, top, e1, p1, m1, e2, p2, m2);
                 }
             }
             fence_proxy_async_smem();   // this thread's generic writes to the staging buffers precede the next bulk copies
@@ -510,7 +522,9 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (grid < 1) grid = 1;
 
     if (want_sumw) HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)n_sumw * sizeof(double), st));
+    profile_mark(st, 0);
     kern<<<(unsigned)grid, TILE, smem, st>>>(P);
+    profile_mark(st, 1);
     HEPK_CUDA_TRY(cudaGetLastError());
     if (want_sumw) {
         dev::chain_finalize_hist<<<(unsigned)((n_sumw + 255) / 256), 256, 0, st>>>(d->hist_sumw, (const double*)workspace, (int)n_sumw);

@@ -17,6 +17,7 @@ void set_error(const char* fmt, ...);
 int32_t cuda_fail(cudaError_t e, const char* what);
 int sm_count();                 // SMs of the current device (cached per device)
 int max_smem_optin();           // max opt-in dynamic shared memory per CTA
+void profile_mark(cudaStream_t st, int which);   // no-op unless hepk_profile_begin() is active (which: 0 before, 1 after)
 
 #define HEPK_CUDA_TRY(call)                                         \
     do {                                                            \
@@ -221,6 +222,30 @@ __device__ __forceinline__ float pair_mass_f32(float pt1, float eta1, float phi1
     const float msq = m1 * m1 + m2 * m2 + 2.0f * pt1 * pt2 * bracket;
     return sqrtf(fmaxf(msq, 0.0f));
 }
+
+// The defining form in float64 (include/hepk.h, hepk_pair_invmass).  Used only where the float32 result above
+// lands within its own error band of a histogram edge, so that the bin is decided by the float32 rounding of
+// the float64 value — the precision the result is defined in (R16).
+static __device__ __noinline__ float pair_mass_f64(float pt1, float eta1, float phi1, float m1,
+                                            float pt2, float eta2, float phi2, float m2)
+{
+    const double a1 = pt1, a2 = pt2;
+    double s1, c1, s2, c2;
+    sincos((double)phi1, &s1, &c1);
+    sincos((double)phi2, &s2, &c2);
+    const double ch1 = cosh((double)eta1), ch2 = cosh((double)eta2);
+    const double e = sqrt(a1 * a1 * ch1 * ch1 + (double)m1 * (double)m1) + sqrt(a2 * a2 * ch2 * ch2 + (double)m2 * (double)m2);
+    const double px = a1 * c1 + a2 * c2, py = a1 * s1 + a2 * s2;
+    const double pz = a1 * sinh((double)eta1) + a2 * sinh((double)eta2);
+    double msq = e * e - px * px - py * py - pz * pz;
+    if (!(msq > 0.0)) msq = 0.0;
+    return (float)sqrt(msq);
+}
+
+// relative half-width of the band around a histogram edge inside which pair_mass_f32 is not trusted to pick the
+// bin (its measured worst error is 1.1e-6 relative; R16)
+#define HEPK_MASS_GUARD_REL 8e-6f
+#define HEPK_MASS_GUARD_ABS 1e-6f
 
 // ---- per-event running state of the reductions (count, sum, min, top-2 with first-index ties) ------
 struct Top2 {
