@@ -1,17 +1,20 @@
 // hepk_chain.cu — the fused analysis chain (include/hepk.h, hepk_analysis_chain).
 //
-// One persistent kernel.  Each CTA walks tiles of TILE events; per tile it
-//   1. turns the three int64 offsets slices into tile-local int32 offsets in shared memory,
-//   2. stages the tile's contiguous column slices (jets: pt, eta, phi, mass; leptons: pt, eta, phi)
-//      into shared memory with TMA 1-D bulk copies (cp.async.bulk + mbarrier), and meanwhile expands
-//      the offsets into a per-jet event id,
-//   3. phase 1, one thread per JET (flat, every lane busy): selection, dR cleaning against the event's
-//      leptons, calibration lookup; the verdict is folded into the staged pt (NaN = not clean),
-//   4. phase 2, one thread per EVENT: count / sum / min / top-2 over the event's jets from shared
-//      memory, leading-pair mass, coalesced per-event outputs, shared-memory histograms,
-// and merges its privatised histograms into float64 accumulators (workspace) every few tiles.
-// A tile that does not fit the staging buffers is processed in pieces; a single event that does not fit
-// goes through a plain per-event loop on global memory.
+// One persistent kernel; the path is bound by instruction issue before it is bound by HBM (DESIGN.md
+// "chain kernel"), so the layout below is chosen to execute as few instructions per event as possible
+// with every lane busy.  Each CTA walks tiles of T events (T threads); per tile
+//   0. the tile's jet-column slices (pt, eta, phi, mass: 63 % of the bytes) are moved into shared memory by
+//      TMA 1-D bulk copies (cp.async.bulk + mbarrier) issued by warp 0 — no thread instructions per byte;
+//   1. prep, one thread per EVENT, while the bulk copies are in flight: the event's six offsets (coalesced
+//      LDG), its selected leptons compacted into one combined (eta, phi) list in shared memory, and a packed
+//      (list start, list length) word written for each of its jets;
+//   2. phase 1, one thread per JET (flat: every lane busy): dR test against the event's combined lepton list,
+//      eta cut, (calibration lookup), verdict folded into the staged pt (-inf / NaN = not clean);
+//   3. phase 2, one thread per EVENT: count / float64 sum / min / top-2 over the event's jets from shared
+//      memory, leading-pair mass, coalesced per-event outputs, shared-memory histograms.
+// Privatised histograms are merged into float64 global accumulators every few thousand events.
+// A tile whose jets or leptons do not fit the shared-memory buffers (a giant event, a dense run) is processed
+// by the paper's own loop shape (Listing 1): one thread per event, straight from global memory.
 #include <string.h>
 
 #include "hepk_common.cuh"
@@ -41,7 +44,8 @@ struct ChainParams {
     unsigned char* out_jet_mask;
     double* hist_acc;                    // workspace: [V][active o][W][nbins_o+2] float64, or nullptr
     unsigned long long* hist_counts;     // [V][active o][nbins_o+2], or nullptr
-    int cap_j, cap_l;
+    int cap_j, cap_l;                    // staged jets per tile / combined selected leptons per tile
+    int jk[4];                           // (misalignment of the jet column in floats - jbase) mod 4: pt, eta, phi, mass
     long long n_tiles;
     int flush_tiles;
 };
@@ -50,10 +54,10 @@ namespace dev {
 
 struct ChainSmem {
     uint64_t* bar;
-    int *loc_j, *loc_m, *loc_e;
+    long long* bnd;                      // [2][6]: joff[e0], joff[e1], moff[e0], moff[e1], eoff[e0], eoff[e1] of this / the next tile
     float *jpt, *jeta, *jphi, *jmass, *corr;
-    unsigned short* evid;
-    float *mpt, *meta, *mphi, *ept, *eeta, *ephi;
+    unsigned int* info;                  // per staged jet: combined-lepton list start | length << 16
+    float2* lep;                         // combined (eta, phi) of the tile's selected leptons, event by event
     float *edges, *axis_lo, *axis_inv;
     float *cal_pt_edges, *cal_eta_edges, *cal_table;
     float* h_sumw;
@@ -63,29 +67,21 @@ struct ChainSmem {
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // One layout function used by the host (size) and the device (pointers).
-template <int TILE>
 __host__ __device__ inline size_t chain_smem_layout(const ChainParams& P, bool calib, unsigned char* base, ChainSmem* s)
 {
     size_t o = 0;
     auto take = [&](size_t bytes, size_t al) { o = align_up(o, al); size_t r = o; o += bytes; return r; };
     size_t r;
     r = take(8, 8); if (s) s->bar = (uint64_t*)(base + r);
-    r = take((TILE + 1) * 4, 4); if (s) s->loc_j = (int*)(base + r);
-    r = take((TILE + 1) * 4, 4); if (s) s->loc_m = (int*)(base + r);
-    r = take((TILE + 1) * 4, 4); if (s) s->loc_e = (int*)(base + r);
-    const size_t cj = (size_t)P.cap_j * 4, cl = (size_t)P.cap_l * 4;
+    r = take(12 * 8, 8); if (s) s->bnd = (long long*)(base + r);
+    const size_t cj = (size_t)P.cap_j * 4;
     r = take(cj, 16); if (s) s->jpt = (float*)(base + r);
     r = take(cj, 16); if (s) s->jeta = (float*)(base + r);
     r = take(cj, 16); if (s) s->jphi = (float*)(base + r);
     r = take(cj, 16); if (s) s->jmass = (float*)(base + r);
     r = take(calib ? cj : 0, 16); if (s) s->corr = (float*)(base + r);
-    r = take((size_t)P.cap_j * 2, 4); if (s) s->evid = (unsigned short*)(base + r);
-    r = take(cl, 16); if (s) s->mpt = (float*)(base + r);
-    r = take(cl, 16); if (s) s->meta = (float*)(base + r);
-    r = take(cl, 16); if (s) s->mphi = (float*)(base + r);
-    r = take(cl, 16); if (s) s->ept = (float*)(base + r);
-    r = take(cl, 16); if (s) s->eeta = (float*)(base + r);
-    r = take(cl, 16); if (s) s->ephi = (float*)(base + r);
+    r = take(cj, 4); if (s) s->info = (unsigned int*)(base + r);
+    r = take((size_t)P.cap_l * 8, 8); if (s) s->lep = (float2*)(base + r);
     r = take((size_t)P.edge_prefix[HEPK_N_OBS] * 4, 4); if (s) s->edges = (float*)(base + r);
     r = take(HEPK_N_OBS * 4, 4); if (s) s->axis_lo = (float*)(base + r);
     r = take(HEPK_N_OBS * 4, 4); if (s) s->axis_inv = (float*)(base + r);
@@ -98,17 +94,36 @@ __host__ __device__ inline size_t chain_smem_layout(const ChainParams& P, bool c
     return align_up(o, 16);
 }
 
-// Per event and variant: leading-pair mass, outputs, histograms.  Shared by the tile path and the
-// per-event fallback.  `k1`/`k2` leading jets' (eta, phi, mass) are passed in by value.
+// One observable of one event and variant into the privatised histograms.
+template <int OB>
+__device__ __forceinline__ void fill_obs(const ChainParams& P, const ChainSmem& S, long long ev, int v, float x)
+{
+    if (!P.axis_edges[OB]) return;
+    const int nb = P.axis_nbins[OB];
+    const int slot = hist_slot(x, S.edges + P.edge_prefix[OB], nb, S.axis_lo[OB], S.axis_inv[OB]);
+    const int spv = P.obs_prefix[HEPK_N_OBS];
+    if (P.hist_counts) atomicAdd(&S.h_cnt[v * spv + P.obs_prefix[OB] + slot], 1u);
+    if (P.hist_acc) {
+        float* h = S.h_sumw + (size_t)(v * spv + P.obs_prefix[OB]) * P.W + slot;
+        for (int w = 0; w < P.W; ++w) {
+            const float wt = P.weights ? __ldg(P.weights + (long long)w * P.n_events + ev) : 1.0f;
+            atomicAdd(h + w * (nb + 2), wt);
+        }
+    }
+}
+
+// Per event and variant: leading-pair mass, outputs, histograms.  Shared by the tile path and the per-event
+// path.  The leading jets' (eta, phi, mass) are passed in by value; i2 < 0 means fewer than two clean jets.
 __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSmem& S, long long ev, int v,
-                                             int cnt, float sum, float mn, const Top2& top,
+                                             int cnt, float sum, float mn, float b1, float b2, int i1, int i2,
                                              float eta1, float phi1, float m1, float eta2, float phi2, float m2)
 {
     float mjj = 0.0f, subpt = 0.0f;
-    if (top.i2 >= 0) {
-        subpt = top.b2;
-        mjj = pair_mass_f32(top.b1, eta1, phi1, m1, top.b2, eta2, phi2, m2);
-        if (P.axis_edges[HEPK_OBS_MJJ] && (P.hist_acc || P.hist_counts)) {
+    const bool hists = P.hist_acc || P.hist_counts;
+    if (i2 >= 0) {
+        subpt = b2;
+        mjj = pair_mass_fast(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
+        if (hists && P.axis_edges[HEPK_OBS_MJJ]) {
             // the bin of mjj is decided by the float64-defined value: refine when the fast value is near an edge
             const float* ed = S.edges + P.edge_prefix[HEPK_OBS_MJJ];
             const int nb = P.axis_nbins[HEPK_OBS_MJJ];
@@ -116,36 +131,45 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSm
             const float band = fmaf(mjj, HEPK_MASS_GUARD_REL, HEPK_MASS_GUARD_ABS);
             const bool near_lo = slot >= 1 && mjj - ed[slot - 1] <= band;
             const bool near_hi = slot <= nb && ed[slot] - mjj <= band;
-            if (near_lo || near_hi) mjj = pair_mass_f64(top.b1, eta1, phi1, m1, top.b2, eta2, phi2, m2);
+            if (near_lo || near_hi) mjj = pair_mass_f64(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
         }
     }
     const long long o = (long long)v * P.n_events + ev;
     if (P.out_njet) P.out_njet[o] = cnt;
-    if (P.out_argmax) P.out_argmax[o] = top.i1;
+    if (P.out_argmax) P.out_argmax[o] = i1;
     if (P.out_ht) P.out_ht[o] = sum;
-    if (P.out_maxpt) P.out_maxpt[o] = top.b1;
+    if (P.out_maxpt) P.out_maxpt[o] = b1;
     if (P.out_minpt) P.out_minpt[o] = mn;
     if (P.out_mjj) P.out_mjj[o] = mjj;
     if (P.out_subpt) P.out_subpt[o] = subpt;
-
-    if (!P.hist_acc && !P.hist_counts) return;
-    const float obs[HEPK_N_OBS] = {(float)cnt, sum, top.b1, mn, mjj, subpt};
-    const int spv = P.obs_prefix[HEPK_N_OBS];
-#pragma unroll
-    for (int ob = 0; ob < HEPK_N_OBS; ++ob) {
-        if (!P.axis_edges[ob]) continue;
-        const int nb = P.axis_nbins[ob];
-        const int slot = hist_slot(obs[ob], S.edges + P.edge_prefix[ob], nb, S.axis_lo[ob], S.axis_inv[ob]);
-        if (P.hist_counts) atomicAdd(&S.h_cnt[v * spv + P.obs_prefix[ob] + slot], 1u);
-        if (P.hist_acc) {
-            float* h = S.h_sumw + (size_t)(v * spv + P.obs_prefix[ob]) * P.W + slot;
-            for (int w = 0; w < P.W; ++w) {
-                const float wt = P.weights ? __ldg(P.weights + (long long)w * P.n_events + ev) : 1.0f;
-                atomicAdd(h + w * (nb + 2), wt);
-            }
-        }
-    }
+    if (!hists) return;
+    fill_obs<HEPK_OBS_NJET>(P, S, ev, v, (float)cnt);
+    fill_obs<HEPK_OBS_HT>(P, S, ev, v, sum);
+    fill_obs<HEPK_OBS_MAXPT>(P, S, ev, v, b1);
+    fill_obs<HEPK_OBS_MINPT>(P, S, ev, v, mn);
+    fill_obs<HEPK_OBS_MJJ>(P, S, ev, v, mjj);
+    fill_obs<HEPK_OBS_SUBPT>(P, S, ev, v, subpt);
 }
+
+// Running per-event state of phase 2.  `p` is the jet's pt if it is clean in this variant, else -inf.
+struct EventAcc {
+    int cnt, i1, i2;
+    double sum;      // float64: exact for float32 terms of like magnitude, so HT and its bin do not depend on the order (R15)
+    float mn, b1, b2;
+    __device__ __forceinline__ void init() { cnt = 0; i1 = i2 = -1; sum = 0.0; mn = CUDART_INF_F; b1 = b2 = -CUDART_INF_F; }
+    __device__ __forceinline__ void push(float p, bool ok, int k)
+    {
+        cnt += ok ? 1 : 0;
+        if (ok) sum += (double)p;
+        mn = fminf(mn, ok ? p : CUDART_INF_F);
+        // top-2 with the first-index tie rule: strict > keeps the smallest index among equal values, for both places
+        const bool gt1 = p > b1, gt2 = p > b2;
+        i2 = gt1 ? i1 : (gt2 ? k : i2);
+        i1 = gt1 ? k : i1;
+        b2 = fmaxf(b2, fminf(b1, p));
+        b1 = fmaxf(b1, p);
+    }
+};
 
 // dR match of one jet against one lepton collection of event `ev`, straight from global memory.
 __device__ inline bool match_global(const ChainParams& P, float eta, float phi, const long long* off, long long base,
@@ -159,18 +183,15 @@ __device__ inline bool match_global(const ChainParams& P, float eta, float phi, 
     return false;
 }
 
-// Fallback for an event too large for the staging buffers: the paper's own loop shape (Listing 1),
-// one thread, everything from global memory.  Slow; only pathological inputs get here.
+// Path for the events of a tile that does not fit the shared-memory buffers: the paper's own loop shape
+// (Listing 1), one thread per event, everything from global memory.  Slow; only unusual tiles get here.
 template <bool CALIB>
 __device__ __noinline__ void chain_event_global(const ChainParams& P, const ChainSmem& S, long long ev)
 {
     const long long g0 = P.joff[ev], g1 = P.joff[ev + 1];
     for (int v = 0; v < P.V; ++v) {
-        int cnt = 0;
-        double sum = 0.0;
-        float mn = CUDART_INF_F;
-        Top2 top;
-        top.init();
+        EventAcc a;
+        a.init();
         for (long long g = g0; g < g1; ++g) {
             const long long j = g - P.jbase;
             const float eta = P.jeta[j], phi = P.jphi[j];
@@ -187,58 +208,73 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, const Chai
                 clean = !matched;
             }
             if (P.out_jet_mask) P.out_jet_mask[(long long)v * P.jn + j] = clean ? 1 : 0;
-            if (clean) {
-                cnt++;
-                sum += (double)p;
-                mn = fminf(mn, p);
-                top.push(p, (int)(g - g0));
-            }
+            a.push(clean ? p : -CUDART_INF_F, clean, (int)(g - g0));
         }
         float e1 = 0, p1 = 0, m1 = 0, e2 = 0, p2 = 0, m2 = 0;
-        if (top.i2 >= 0) {
-            const long long a = g0 - P.jbase + top.i1, b = g0 - P.jbase + top.i2;
-            e1 = P.jeta[a]; p1 = P.jphi[a]; m1 = P.jmass[a];
-            e2 = P.jeta[b]; p2 = P.jphi[b]; m2 = P.jmass[b];
+        if (a.i2 >= 0) {
+            const long long x = g0 - P.jbase + a.i1, y = g0 - P.jbase + a.i2;
+            e1 = P.jeta[x]; p1 = P.jphi[x]; m1 = P.jmass[x];
+            e2 = P.jeta[y]; p2 = P.jphi[y]; m2 = P.jmass[y];
         }
-        finish_event(P, S, ev, v, cnt, (float)sum, mn, top, e1, p1, m1, e2, p2, m2);
+        finish_event(P, S, ev, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
     }
 }
 
-template <int TILE>
+template <int T>
 __device__ __forceinline__ void flush_hist(const ChainParams& P, const ChainSmem& S, int tid)
 {
     const int spv = P.obs_prefix[HEPK_N_OBS];
     if (P.hist_acc) {
         const int n = spv * P.V * P.W;
-        for (int i = tid; i < n; i += TILE) {
+        for (int i = tid; i < n; i += T) {
             const float x = S.h_sumw[i];
             if (x != 0.0f) { atomicAdd(P.hist_acc + i, (double)x); S.h_sumw[i] = 0.0f; }
         }
     }
     if (P.hist_counts) {
         const int n = spv * P.V;
-        for (int i = tid; i < n; i += TILE) {
+        for (int i = tid; i < n; i += T) {
             const unsigned int c = S.h_cnt[i];
             if (c) { atomicAdd(P.hist_counts + i, (unsigned long long)c); S.h_cnt[i] = 0u; }
         }
     }
 }
 
-template <int TILE, bool CALIB>
-__global__ void __launch_bounds__(TILE) chain_kernel(const __grid_constant__ ChainParams P)
+// The six boundary offsets of tile `tile` (first and one-past-last event of each collection).
+template <int T, bool HAS_EL>
+__device__ __forceinline__ void load_bounds(const ChainParams& P, long long tile, long long* b)
+{
+    const long long e0 = tile * T;
+    const long long e1 = e0 + T < P.n_events ? e0 + T : P.n_events;
+    b[0] = __ldg(P.joff + e0); b[1] = __ldg(P.joff + e1);
+    b[2] = __ldg(P.moff + e0); b[3] = __ldg(P.moff + e1);
+    if (HAS_EL) { b[4] = __ldg(P.eoff + e0); b[5] = __ldg(P.eoff + e1); }
+    else { b[4] = 0; b[5] = 0; }
+}
+
+template <int T, bool CALIB, bool HAS_EL>
+__global__ void __launch_bounds__(T) chain_kernel(const __grid_constant__ ChainParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     ChainSmem S;
-    chain_smem_layout<TILE>(P, CALIB, smem_raw, &S);
+    chain_smem_layout(P, CALIB, smem_raw, &S);
     const int tid = threadIdx.x;
-    const bool has_el = P.eoff != nullptr;
+    const int warp = tid >> 5, lane = tid & 31;
 
-    // ---- one-time setup: barrier, axis edges, calibration tables, zeroed histograms
-    if (tid == 0) { mbar_init(S.bar, 1); fence_mbar_init(); }
+    // ---- one-time setup: barrier, axis edges, calibration tables, zeroed histograms, first tile's bounds
+    if (tid == 0) {
+        mbar_init(S.bar, 1);
+        fence_mbar_init();
+        long long b[6];
+        load_bounds<T, HAS_EL>(P, blockIdx.x, b);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) S.bnd[i] = b[i];
+    }
+#pragma unroll
     for (int ob = 0; ob < HEPK_N_OBS; ++ob) {
         if (!P.axis_edges[ob]) continue;
         const int nb = P.axis_nbins[ob];
-        for (int i = tid; i <= nb; i += TILE) S.edges[P.edge_prefix[ob] + i] = P.axis_edges[ob][i];
+        for (int i = tid; i <= nb; i += T) S.edges[P.edge_prefix[ob] + i] = P.axis_edges[ob][i];
         if (tid == 0) {
             const float lo = P.axis_edges[ob][0], hi = P.axis_edges[ob][nb];
             S.axis_lo[ob] = lo;
@@ -246,162 +282,174 @@ __global__ void __launch_bounds__(TILE) chain_kernel(const __grid_constant__ Cha
         }
     }
     if (CALIB) {
-        for (int i = tid; i <= P.cal_npt; i += TILE) S.cal_pt_edges[i] = P.cal_pt_edges[i];
-        for (int i = tid; i <= P.cal_neta; i += TILE) S.cal_eta_edges[i] = P.cal_eta_edges[i];
-        for (int i = tid; i < P.cal_npt * P.cal_neta; i += TILE) S.cal_table[i] = P.cal_table[i];
+        for (int i = tid; i <= P.cal_npt; i += T) S.cal_pt_edges[i] = P.cal_pt_edges[i];
+        for (int i = tid; i <= P.cal_neta; i += T) S.cal_eta_edges[i] = P.cal_eta_edges[i];
+        for (int i = tid; i < P.cal_npt * P.cal_neta; i += T) S.cal_table[i] = P.cal_table[i];
     }
     {
         const int spv = P.obs_prefix[HEPK_N_OBS];
-        if (P.hist_acc) for (int i = tid; i < spv * P.V * P.W; i += TILE) S.h_sumw[i] = 0.0f;
-        if (P.hist_counts) for (int i = tid; i < spv * P.V; i += TILE) S.h_cnt[i] = 0u;
+        if (P.hist_acc) for (int i = tid; i < spv * P.V * P.W; i += T) S.h_sumw[i] = 0.0f;
+        if (P.hist_counts) for (int i = tid; i < spv * P.V; i += T) S.h_cnt[i] = 0u;
     }
     __syncthreads();
 
     uint32_t parity = 0;
-    int tiles_since_flush = 0;
-    const int cap_j = P.cap_j - 8, cap_l = P.cap_l - 8;     // room for the alignment shift and padding
+    int tiles_since_flush = 0, it = 0;
+    const int V = CALIB ? P.V : 1;
 
-    for (long long tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
-        const long long e0 = tile * TILE;
-        const int ne = (int)((P.n_events - e0) < TILE ? (P.n_events - e0) : TILE);
-        // ---- 1. tile-local offsets
-        const long long jb = P.joff[e0], mb = P.moff[e0], eb = has_el ? P.eoff[e0] : 0;
-        for (int i = tid; i <= ne; i += TILE) {
-            S.loc_j[i] = (int)(P.joff[e0 + i] - jb);
-            S.loc_m[i] = (int)(P.moff[e0 + i] - mb);
-            S.loc_e[i] = has_el ? (int)(P.eoff[e0 + i] - eb) : 0;
-        }
-        __syncthreads();
+    for (long long tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x, ++it) {
+        const long long* B = S.bnd + (it & 1) * 6;
+        const long long e0 = tile * T;
+        const int ne = (int)((P.n_events - e0) < T ? (P.n_events - e0) : T);
+        const long long jb = B[0], je = B[1], mb = B[2], me = B[3], qb = B[4], qe = B[5];
+        const bool fit = (je - jb) <= (long long)(P.cap_j - 8) && (me - mb) + (qe - qb) <= (long long)P.cap_l;
 
-        int ev0 = 0;
-        while (ev0 < ne) {
-            // ---- how many events from ev0 fit the staging buffers
-            const int bj = S.loc_j[ev0], bm = S.loc_m[ev0], be = S.loc_e[ev0];
-            int n_fit;
-            if (S.loc_j[ne] - bj <= cap_j && S.loc_m[ne] - bm <= cap_l && S.loc_e[ne] - be <= cap_l) {
-                n_fit = ne - ev0;
-            } else {
-                const bool f = tid >= ev0 && tid < ne && S.loc_j[tid + 1] - bj <= cap_j &&
-                               S.loc_m[tid + 1] - bm <= cap_l && S.loc_e[tid + 1] - be <= cap_l;
-                n_fit = __syncthreads_count(f);
+        // bounds of this CTA's next tile: loaded now, stored at the end of this one (latency hidden)
+        const long long tile_next = tile + gridDim.x;
+        long long nb[6];
+        if (tid == 0 && tile_next < P.n_tiles) load_bounds<T, HAS_EL>(P, tile_next, nb);
+
+        if (fit) {
+            const int njt = (int)(je - jb);
+            const long long lj0 = jb - P.jbase;
+            // ---- 0. warp 0 starts the bulk copies of the four jet columns
+            if (warp == 0) {
+                long long a0;
+                uint32_t bytes = 0;
+                bytes += stage_column(S.jpt, P.jpt, lj0, lj0 + njt, P.jn, S.bar, lane, 0, &a0);
+                bytes += stage_column(S.jeta, P.jeta, lj0, lj0 + njt, P.jn, S.bar, lane, 0, &a0);
+                bytes += stage_column(S.jphi, P.jphi, lj0, lj0 + njt, P.jn, S.bar, lane, 0, &a0);
+                bytes += stage_column(S.jmass, P.jmass, lj0, lj0 + njt, P.jn, S.bar, lane, 0, &a0);
+                __syncwarp();                       // the lanes' scalar head/tail stores precede lane 0's release
+                if (lane == 0) mbar_arrive_expect_tx(S.bar, bytes);
             }
-            if (n_fit == 0) {   // a single event larger than the buffers
-                if (tid == 0) chain_event_global<CALIB>(P, S, e0 + ev0);
-                ev0 += 1;
-                __syncthreads();
-                continue;
-            }
-            const int ev1 = ev0 + n_fit;
-            const int nj = S.loc_j[ev1] - bj, nm = S.loc_m[ev1] - bm, nel = S.loc_e[ev1] - be;
-
-            // ---- 2. stage the column slices with bulk copies
-            long long a0;
-            int sh_pt, sh_eta, sh_phi, sh_mass, sh_mpt, sh_meta, sh_mphi, sh_ept = 0, sh_eeta = 0, sh_ephi = 0;
-            const long long lj0 = jb + bj - P.jbase, lm0 = mb + bm - P.mbase, le0 = eb + be - P.ebase;
-            if (tid == 0) fence_proxy_async_smem();
-            uint32_t bytes = 0;
-            bytes += stage_column(S.jpt, P.jpt, lj0, lj0 + nj, P.jn, S.bar, tid, 0, &a0);   sh_pt = (int)(lj0 - a0);
-            bytes += stage_column(S.jeta, P.jeta, lj0, lj0 + nj, P.jn, S.bar, tid, 0, &a0); sh_eta = (int)(lj0 - a0);
-            bytes += stage_column(S.jphi, P.jphi, lj0, lj0 + nj, P.jn, S.bar, tid, 0, &a0); sh_phi = (int)(lj0 - a0);
-            bytes += stage_column(S.jmass, P.jmass, lj0, lj0 + nj, P.jn, S.bar, tid, 0, &a0); sh_mass = (int)(lj0 - a0);
-            bytes += stage_column(S.mpt, P.mpt, lm0, lm0 + nm, P.mn, S.bar, tid, 0, &a0);   sh_mpt = (int)(lm0 - a0);
-            bytes += stage_column(S.meta, P.meta, lm0, lm0 + nm, P.mn, S.bar, tid, 0, &a0); sh_meta = (int)(lm0 - a0);
-            bytes += stage_column(S.mphi, P.mphi, lm0, lm0 + nm, P.mn, S.bar, tid, 0, &a0); sh_mphi = (int)(lm0 - a0);
-            if (has_el) {
-                bytes += stage_column(S.ept, P.ept, le0, le0 + nel, P.en, S.bar, tid, 0, &a0);   sh_ept = (int)(le0 - a0);
-                bytes += stage_column(S.eeta, P.eeta, le0, le0 + nel, P.en, S.bar, tid, 0, &a0); sh_eeta = (int)(le0 - a0);
-                bytes += stage_column(S.ephi, P.ephi, le0, le0 + nel, P.en, S.bar, tid, 0, &a0); sh_ephi = (int)(le0 - a0);
-            }
-            if (tid == 0) mbar_arrive_expect_tx(S.bar, bytes);
-
-            // ---- meanwhile: expand offsets into a per-jet event id (needs only the offsets)
-            if (tid < n_fit) {
-                const int k0 = S.loc_j[ev0 + tid] - bj, k1 = S.loc_j[ev0 + tid + 1] - bj;
-                for (int k = k0; k < k1; ++k) S.evid[k] = (unsigned short)tid;
+            // ---- 1. prep, one thread per event (overlaps the copies)
+            int kj0 = 0, nj = 0;
+            if (tid < ne) {
+                const long long ev = e0 + tid;
+                const long long j0 = __ldg(P.joff + ev), j1 = __ldg(P.joff + ev + 1);
+                const long long m0 = __ldg(P.moff + ev), m1 = __ldg(P.moff + ev + 1);
+                long long q0 = 0, q1 = 0;
+                if (HAS_EL) { q0 = __ldg(P.eoff + ev); q1 = __ldg(P.eoff + ev + 1); }
+                kj0 = (int)(j0 - jb);
+                nj = (int)(j1 - j0);
+                const int l0 = (int)(m0 - mb) + (int)(q0 - qb);
+                int c = 0;
+                {
+                    const int nm = (int)(m1 - m0);
+                    const float* lp = P.mpt + (m0 - P.mbase);
+                    const float* le = P.meta + (m0 - P.mbase);
+                    const float* lf = P.mphi + (m0 - P.mbase);
+                    for (int i = 0; i < nm; ++i) {
+                        const float pt = lp[i], eta = le[i], phi = lf[i];
+                        if (pt > P.lep_pt_min) S.lep[l0 + c++] = make_float2(eta, phi);
+                    }
+                }
+                if (HAS_EL) {
+                    const int nq = (int)(q1 - q0);
+                    const float* lp = P.ept + (q0 - P.ebase);
+                    const float* le = P.eeta + (q0 - P.ebase);
+                    const float* lf = P.ephi + (q0 - P.ebase);
+                    for (int i = 0; i < nq; ++i) {
+                        const float pt = lp[i], eta = le[i], phi = lf[i];
+                        if (pt > P.lep_pt_min) S.lep[l0 + c++] = make_float2(eta, phi);
+                    }
+                }
+                const unsigned int info = (unsigned int)l0 | ((unsigned int)c << 16);
+                unsigned int* ip = S.info + kj0;
+                for (int k = 0; k < nj; ++k) ip[k] = info;
             }
             mbar_wait(S.bar, parity);
             parity ^= 1u;
             __syncthreads();
 
-            // ---- lepton selection folded into the staged eta (NaN never matches)
-            for (int m = tid; m < nm; m += TILE)
-                if (!(S.mpt[m + sh_mpt] > P.lep_pt_min)) S.meta[m + sh_meta] = CUDART_NAN_F;
-            for (int m = tid; m < nel; m += TILE)
-                if (!(S.ept[m + sh_ept] > P.lep_pt_min)) S.eeta[m + sh_eeta] = CUDART_NAN_F;
-            __syncthreads();
-
-            // ---- 3. phase 1: one thread per jet
-            for (int j = tid; j < nj; j += TILE) {
-                const float pt = S.jpt[j + sh_pt], eta = S.jeta[j + sh_eta], phi = S.jphi[j + sh_phi];
-                const int a = ev0 + (int)S.evid[j];
-                bool matched = false;
-                {
-                    const int m0 = S.loc_m[a] - bm, m1 = S.loc_m[a + 1] - bm;
-                    for (int m = m0; m < m1; ++m)
-                        matched |= dr2_exact(eta, phi, S.meta[m + sh_meta], S.mphi[m + sh_mphi]) < P.dr2_max;
-                    const int q0 = S.loc_e[a] - be, q1 = S.loc_e[a + 1] - be;
-                    for (int m = q0; m < q1; ++m)
-                        matched |= dr2_exact(eta, phi, S.eeta[m + sh_eeta], S.ephi[m + sh_ephi]) < P.dr2_max;
-                }
-                const bool base = (fabsf(eta) < P.jet_abs_eta_max) && !matched;
-                if (!CALIB) {
-                    const bool clean = base && (pt > P.jet_pt_min);
-                    if (P.out_jet_mask) P.out_jet_mask[lj0 + j] = clean ? 1 : 0;
-                    if (!clean) S.jpt[j + sh_pt] = CUDART_NAN_F;
-                } else {
-                    const int bx = find_bin_clamped(pt, S.cal_pt_edges, P.cal_npt);
-                    const int by = find_bin_clamped(eta, S.cal_eta_edges, P.cal_neta);
-                    const float c = S.cal_table[bx * P.cal_neta + by];
-                    S.corr[j] = base ? c : CUDART_NAN_F;
-                    if (P.out_jet_mask)
-                        for (int v = 0; v < P.V; ++v)
-                            P.out_jet_mask[(long long)v * P.jn + lj0 + j] =
-                                (base && (__fmul_rn(pt, __fmul_rn(c, P.scales[v])) > P.jet_pt_min)) ? 1 : 0;
+            // ---- 2. phase 1: one thread per jet
+            const int sh_pt = ((int)jb + P.jk[0]) & 3, sh_eta = ((int)jb + P.jk[1]) & 3;
+            const int sh_phi = ((int)jb + P.jk[2]) & 3, sh_mass = ((int)jb + P.jk[3]) & 3;
+            {
+                float* ppt = S.jpt + sh_pt;
+                const float* peta = S.jeta + sh_eta;
+                const float* pphi = S.jphi + sh_phi;
+                for (int j = tid; j < njt; j += T) {
+                    const unsigned int info = S.info[j];
+                    const float eta = peta[j], phi = pphi[j];
+                    const float2* L = S.lep + (info & 0xffffu);
+                    const int n = (int)(info >> 16);
+                    bool matched = false;
+                    for (int t = 0; t < n; ++t) {
+                        const float2 l = L[t];
+                        matched |= dr2_exact(eta, phi, l.x, l.y) < P.dr2_max;
+                    }
+                    const float pt = ppt[j];
+                    const bool base = (fabsf(eta) < P.jet_abs_eta_max) && !matched;
+                    if (!CALIB) {
+                        const bool clean = base && (pt > P.jet_pt_min);
+                        if (P.out_jet_mask) P.out_jet_mask[lj0 + j] = clean ? 1 : 0;
+                        ppt[j] = clean ? pt : -CUDART_INF_F;
+                    } else {
+                        const int bx = find_bin_clamped(pt, S.cal_pt_edges, P.cal_npt);
+                        const int by = find_bin_clamped(eta, S.cal_eta_edges, P.cal_neta);
+                        const float c = S.cal_table[bx * P.cal_neta + by];
+                        S.corr[j] = c;
+                        if (!base) ppt[j] = CUDART_NAN_F;
+                        if (P.out_jet_mask)
+                            for (int v = 0; v < V; ++v)
+                                P.out_jet_mask[(long long)v * P.jn + lj0 + j] =
+                                    (base && (__fmul_rn(pt, __fmul_rn(c, P.scales[v])) > P.jet_pt_min)) ? 1 : 0;
+                    }
                 }
             }
             __syncthreads();
 
-            // ---- 4. phase 2: one thread per event
-            if (tid < n_fit) {
-                const int k0 = S.loc_j[ev0 + tid] - bj, k1 = S.loc_j[ev0 + tid + 1] - bj;
-                for (int v = 0; v < P.V; ++v) {
+            // ---- 3. phase 2: one thread per event
+            if (tid < ne) {
+                const float* pp = S.jpt + sh_pt + kj0;
+                const float* cc = S.corr + kj0;
+                for (int v = 0; v < V; ++v) {
                     const float sv = P.scales[v];
-                    int cnt = 0;
-                    double sum = 0.0;      // float64: exact for these inputs, so HT and its bin do not depend on the order (R15)
-                    float mn = CUDART_INF_F;
-                    Top2 top;
-                    top.init();
-                    for (int k = k0; k < k1; ++k) {
-                        float p = S.jpt[k + sh_pt];
-                        if (CALIB) p = __fmul_rn(p, __fmul_rn(S.corr[k], sv));
-                        if (p > P.jet_pt_min) {
-                            cnt++;
-                            sum += (double)p;
-                            mn = fminf(mn, p);
-                            top.push(p, k - k0);
+                    EventAcc a;
+                    a.init();
+#pragma unroll 2
+                    for (int k = 0; k < nj; ++k) {
+                        float p = pp[k];
+                        bool ok;
+                        if (CALIB) {
+                            p = __fmul_rn(p, __fmul_rn(cc[k], sv));     // NaN when the jet failed eta / dR
+                            ok = p > P.jet_pt_min;
+                            p = ok ? p : -CUDART_INF_F;
+                        } else {
+                            ok = p > P.jet_pt_min;                      // -inf when not clean
                         }
+                        a.push(p, ok, k);
                     }
                     float e1 = 0, p1 = 0, m1 = 0, e2 = 0, p2 = 0, m2 = 0;
-                    if (top.i2 >= 0) {
-                        const int a = k0 + top.i1, b = k0 + top.i2;
-                        e1 = S.jeta[a + sh_eta]; p1 = S.jphi[a + sh_phi]; m1 = S.jmass[a + sh_mass];
-                        e2 = S.jeta[b + sh_eta]; p2 = S.jphi[b + sh_phi]; m2 = S.jmass[b + sh_mass];
+                    if (a.i2 >= 0) {
+                        const int x = kj0 + a.i1, y = kj0 + a.i2;
+                        e1 = S.jeta[x + sh_eta]; p1 = S.jphi[x + sh_phi]; m1 = S.jmass[x + sh_mass];
+                        e2 = S.jeta[y + sh_eta]; p2 = S.jphi[y + sh_phi]; m2 = S.jmass[y + sh_mass];
                     }
-                    finish_event(P, S, e0 + ev0 + tid, v, cnt, (float)sum, mn, top, e1, p1, m1, e2, p2, m2);
+                    finish_event(P, S, e0 + tid, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
                 }
             }
-            fence_proxy_async_smem();   // this thread's generic writes to the staging buffers precede the next bulk copies
-            __syncthreads();
-            ev0 = ev1;
+        } else {
+            if (tid < ne) chain_event_global<CALIB>(P, S, e0 + tid);
         }
+
+        if (tid == 0 && tile_next < P.n_tiles) {
+            long long* Bn = S.bnd + ((it + 1) & 1) * 6;
+#pragma unroll
+            for (int i = 0; i < 6; ++i) Bn[i] = nb[i];
+        }
+        fence_proxy_async_smem();   // this thread's generic accesses to the staging buffers precede the next bulk copies
+        __syncthreads();
         if (++tiles_since_flush >= P.flush_tiles) {
-            flush_hist<TILE>(P, S, tid);
+            flush_hist<T>(P, S, tid);
             tiles_since_flush = 0;
             __syncthreads();
         }
     }
     __syncthreads();
-    flush_hist<TILE>(P, S, tid);
+    flush_hist<T>(P, S, tid);
 }
 
 // sumw[i] = float32(float64(sumw[i]) + acc[i])
@@ -449,7 +497,7 @@ static long long hist_slots_per_variant(const hepk_chain_desc* d)
 
 static int round_up4(long long x) { return (int)((x + 3) / 4 * 4); }
 
-template <int TILE>
+template <int T>
 static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStream_t st)
 {
     ChainParams P;
@@ -464,6 +512,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     P.jet_pt_min = d->jet_pt_min; P.jet_abs_eta_max = d->jet_abs_eta_max; P.lep_pt_min = d->lep_pt_min;
     P.dr2_max = d->dr_max * d->dr_max;      // float32 product (exact class)
     const bool calib = d->calib_table != nullptr;
+    const bool has_el = d->electrons.offsets != nullptr;
     P.cal_pt_edges = d->calib_pt_edges; P.cal_eta_edges = d->calib_eta_edges; P.cal_table = d->calib_table;
     P.cal_npt = d->calib_npt; P.cal_neta = d->calib_neta;
     for (int v = 0; v < HEPK_MAX_VARIANTS; ++v) P.scales[v] = calib ? d->calib_scales[v] : 1.0f;
@@ -483,38 +532,50 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     const bool want_sumw = d->hist_sumw && sp > 0, want_cnt = d->hist_counts && sp > 0;
     P.hist_acc = want_sumw ? (double*)workspace : nullptr;
     P.hist_counts = want_cnt ? (unsigned long long*)d->hist_counts : nullptr;
-    P.n_tiles = (d->n_events + TILE - 1) / TILE;
-    P.flush_tiles = 4096 / TILE > 0 ? 4096 / TILE : 1;
+    P.n_tiles = (d->n_events + T - 1) / T;
+    P.flush_tiles = 4096 / T > 0 ? 4096 / T : 1;
+    const float* jc[4] = {d->jets.pt, d->jets.eta, d->jets.phi, d->jets.mass};
+    for (int c = 0; c < 4; ++c) {
+        const long long mis = (long long)((reinterpret_cast<uintptr_t>(jc[c]) / sizeof(float)) % 4);
+        P.jk[c] = (int)((((mis - d->jets.content_base) % 4) + 4) % 4);
+    }
 
-    // staging capacities from the mean multiplicities (a tile that overflows is processed in pieces)
+    // staging capacities from the mean multiplicities: mean + ~5 sigma of a Poisson-like tile total
+    // (a tile that does not fit takes the per-event path)
     const double nev = (double)(d->n_events > 0 ? d->n_events : 1);
     auto cap_for = [&](double mean, int floor_) {
-        const double t = TILE * mean;
-        long long c = (long long)(t * 1.12 + 6.0 * sqrt(2.0 * t + 1.0)) + 24;
+        const double t = T * mean;
+        long long c = (long long)(t + 5.0 * sqrt(2.0 * t + 1.0)) + 16;
         return c < floor_ ? floor_ : (int)c;
     };
     double mean_l = (double)d->muons.n_objects / nev;
-    if (d->electrons.offsets && (double)d->electrons.n_objects / nev > mean_l) mean_l = (double)d->electrons.n_objects / nev;
+    if (has_el) mean_l += (double)d->electrons.n_objects / nev;
     P.cap_j = round_up4(d->tune_cap_jets > 0 ? d->tune_cap_jets : cap_for((double)d->jets.n_objects / nev, 256));
     P.cap_l = round_up4(d->tune_cap_leptons > 0 ? d->tune_cap_leptons : cap_for(mean_l, 128));
-    if (P.cap_j > 65536 - 8) P.cap_j = 65536 - 8;        // event ids are 16-bit, jet indices must stay small
     if (P.cap_j < 16) P.cap_j = 16;
-    if (P.cap_l < 16) P.cap_l = 16;
+    if (P.cap_l < 4) P.cap_l = 4;
+    if (P.cap_l > 65532) P.cap_l = 65532;      // list start and length are packed in 16 bits each
 
     const int smem_max = max_smem_optin();
-    size_t smem = dev::chain_smem_layout<TILE>(P, calib, nullptr, nullptr);
+    size_t smem = dev::chain_smem_layout(P, calib, nullptr, nullptr);
     while (smem > (size_t)smem_max && P.cap_j > 64) {   // shrink the jet buffers before giving up
         P.cap_j = round_up4(P.cap_j / 2);
-        smem = dev::chain_smem_layout<TILE>(P, calib, nullptr, nullptr);
+        smem = dev::chain_smem_layout(P, calib, nullptr, nullptr);
+    }
+    while (smem > (size_t)smem_max && P.cap_l > 64) {
+        P.cap_l = round_up4(P.cap_l / 2);
+        smem = dev::chain_smem_layout(P, calib, nullptr, nullptr);
     }
     if (smem > (size_t)smem_max) {
         set_error("hepk_analysis_chain: histograms need %zu bytes of shared memory (max %d)", smem, smem_max);
         return HEPK_ERR_UNSUPPORTED;
     }
-    auto kern = calib ? dev::chain_kernel<TILE, true> : dev::chain_kernel<TILE, false>;
+    void (*kern)(ChainParams);
+    if (calib) kern = has_el ? dev::chain_kernel<T, true, true> : dev::chain_kernel<T, true, false>;
+    else kern = has_el ? dev::chain_kernel<T, false, true> : dev::chain_kernel<T, false, false>;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    HEPK_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, TILE, smem));
+    HEPK_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, T, smem));
     if (occ < 1) occ = 1;
     if (d->tune_ctas_per_sm > 0 && d->tune_ctas_per_sm < occ) occ = d->tune_ctas_per_sm;
     long long grid = (long long)sm_count() * occ;
@@ -523,7 +584,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
 
     if (want_sumw) HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)n_sumw * sizeof(double), st));
     profile_mark(st, 0);
-    kern<<<(unsigned)grid, TILE, smem, st>>>(P);
+    kern<<<(unsigned)grid, T, smem, st>>>(P);
     profile_mark(st, 1);
     HEPK_CUDA_TRY(cudaGetLastError());
     if (want_sumw) {
