@@ -209,7 +209,7 @@ typedef struct hepk_chain_desc {
     int32_t tune_cap_jets;       /* shared-memory capacity (jets per staged tile) */
     int32_t tune_cap_leptons;    /* capacity per lepton collection */
     int32_t tune_ctas_per_sm;    /* persistent CTAs per SM */
-    int32_t tune_reserved;
+    int32_t tune_tile_events;    /* events per tile: 32, 64, 128 or 256 */
 } hepk_chain_desc;
 
 /* `d` is a HOST pointer to a descriptor whose array pointers are DEVICE pointers.  `workspace` is a

@@ -613,5 +613,10 @@ extern "C" int32_t hepk_analysis_chain(const hepk_chain_desc* d, void* workspace
         HEPK_REQUIRE(workspace != nullptr, "workspace is NULL");
         HEPK_REQUIRE(workspace_bytes >= hepk_chain_workspace_bytes(d), "workspace too small");
     }
-    return chain_launch<128>(d, workspace, (cudaStream_t)stream);
+    switch (d->tune_tile_events) {
+        case 32: return chain_launch<32>(d, workspace, (cudaStream_t)stream);
+        case 64: return chain_launch<64>(d, workspace, (cudaStream_t)stream);
+        case 256: return chain_launch<256>(d, workspace, (cudaStream_t)stream);
+        default: return chain_launch<128>(d, workspace, (cudaStream_t)stream);
+    }
 }
