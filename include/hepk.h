@@ -206,10 +206,10 @@ typedef struct hepk_chain_desc {
      *   hist_counts int64   [n_variants][active o][nbins_o+2] */
     float* hist_sumw; int64_t* hist_counts;
     /* tuning / test hooks; 0 = automatic */
-    int32_t tune_cap_jets;       /* shared-memory capacity (jets per staged tile) */
+    int32_t tune_cap_jets;       /* shared-memory capacity (jets per staged 32-event tile) */
     int32_t tune_cap_leptons;    /* capacity per lepton collection */
     int32_t tune_ctas_per_sm;    /* persistent CTAs per SM */
-    int32_t tune_tile_events;    /* events per tile: 32, 64, 128 or 256 */
+    int32_t tune_warps_per_cta;  /* warps (each owning its own tiles and staging region) per CTA, at most 16 */
 } hepk_chain_desc;
 
 /* `d` is a HOST pointer to a descriptor whose array pointers are DEVICE pointers.  `workspace` is a

@@ -92,6 +92,13 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
                  : "memory");
 }
 
+__device__ __forceinline__ void bulk_g2s_addr(uint32_t dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
 // ---- staging a slice [l0, l1) of a column into shared memory -----------------------------------
 // Element l of `col` lands at dst[l - a0], a0 <= l0 chosen so that the 16-byte aligned body of the slice
 // can be moved by ONE bulk copy; the ragged head (col not 16-byte aligned near element 0) and the tail
