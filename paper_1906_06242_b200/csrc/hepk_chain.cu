@@ -1,19 +1,21 @@
 // hepk_chain.cu — the fused analysis chain (include/hepk.h, hepk_analysis_chain).
 //
-// The path is bound by instruction issue before it is bound by HBM, so the layout is
-// chosen to execute few instructions per event, keep lanes busy and never stall a whole CTA:
+// The path is bound by instruction issue before it is bound by HBM: at 60 % of the
+// HBM peak an SM may spend ~40 warp instructions per event.  The layout is chosen to execute few instructions
+// per event, keep lanes busy and never stall a whole CTA:
 //
 //   * WARP-AUTONOMOUS tiles.  A tile is 32 consecutive events and belongs to ONE warp, which owns a private
 //     staging region of shared memory and a private mbarrier.  There is no CTA-wide barrier in the steady state;
 //     warps drift apart and hide each other's latencies.
-//   * TMA staging of everything.  For a tile the warp's lanes 0..12 each issue one 1-D bulk copy
-//     (cp.async.bulk + mbarrier complete_tx): the four jet columns, three muon and three electron columns, and
-//     the three offsets slices.  No thread instruction is spent per byte and every byte is read from HBM once.
-//     The bounds (offsets[e0], offsets[e1]) a copy needs are loaded one tile ahead.
-//   * phase 0, one lane per EVENT: offsets from shared memory, selected leptons compacted into one combined
-//     (eta, phi) list, a 16-bit (list start, length) word written for each of the event's jets;
-//   * phase 1, one lane per JET (flat, all lanes busy): dR against the event's lepton list, eta cut,
-//     (calibration lookup), verdict folded into the staged pt;
+//   * TMA staging of the content columns.  Lanes 0..9 of the warp each issue one 1-D bulk copy
+//     (cp.async.bulk + mbarrier complete_tx): four jet columns, three muon and three electron columns.  No thread
+//     instruction is spent per byte and every byte is read from HBM once.  The offsets of the tile's events are
+//     read one tile ahead with coalesced loads and live in registers (one event per lane).
+//   * phase 0, one lane per EVENT: selected leptons compacted into one combined (eta, phi) list; the event's
+//     jets are appended to one of eight buckets keyed by the number of selected leptons, which yields a
+//     permutation of the tile's jets in which neighbouring jets have the same dR trip count;
+//   * phase 1, one lane per JET in that order (flat, all lanes busy, uniform trip counts): dR against the
+//     event's lepton list, eta cut, (calibration lookup), verdict folded into the staged pt;
 //   * phase 2, one lane per EVENT: count / float64 sum / min / top-2 over the event's jets, the leading pair's
 //     (eta, phi, mass) into registers — after which the staging region is released and the next tile's copies are
 //     issued — then the pair mass, coalesced per-event outputs and the CTA's shared-memory histograms.
@@ -27,23 +29,25 @@
 namespace hepk {
 
 constexpr int TILE_EVENTS = 32;     // events per warp tile
-constexpr int NCOL = 13;            // staged columns: 0-3 jets pt,eta,phi,mass; 4-6 muons; 7-9 electrons; 10-12 offsets j,m,e
+constexpr int NCOL = 10;            // staged columns: 0-3 jets pt,eta,phi,mass; 4-6 muons pt,eta,phi; 7-9 electrons
+constexpr int MAX_JETS_TILE = 1024; // jet index inside a tile fits 10 bits
 constexpr int MAX_LIST = 2047;      // combined lepton list start fits 11 bits
 constexpr int MAX_LEP_EVENT = 31;   // selected leptons of one event fit 5 bits
+constexpr int N_BUCKETS = 8;        // jets are ordered by min(selected leptons of their event, 7)
 
 struct ChainParams {
     long long n_events;
     long long n_tiles;
     // staged columns (see NCOL)
     const char* col_ptr[NCOL];      // element 0 of the column
-    long long col_base[NCOL];       // content_base of the collection (0 for offsets)
+    long long col_base[NCOL];       // content_base of the collection
     long long col_n[NCOL];          // valid elements
-    int col_mis[NCOL];              // (address / element size) mod (16 / element size)
+    int col_mis[NCOL];              // (address / 4) mod 4
     int col_dst[NCOL];              // byte offset of the staging buffer inside a warp's region
     int col_cap[NCOL];              // slice capacity in elements (the buffer has 8 more)
     int col_coll[NCOL];             // collection 0 jets, 1 muons, 2 electrons
-    int n_col;                      // 13, or 0 when the staged path is disabled
-    int sh_add[10];                 // (col_mis - content_base) mod 4 per float column: shift = (lo32(offsets[e0]) + sh_add) & 3
+    int n_col;                      // NCOL, or 0 when the staged path is disabled
+    int sh_add[NCOL];               // (col_mis - content_base) mod 4: shift = (lo32(offsets[e0]) + sh_add) & 3
     const long long* off[3];        // offsets arrays: jets, muons, electrons (electrons nullptr if absent)
     long long jn;
     const float *jpt, *jeta, *jphi, *jmass; long long jbase;
@@ -64,7 +68,7 @@ struct ChainParams {
     unsigned char* out_jet_mask;
     double* hist_acc;                    // workspace: [V][active o][W][nbins_o+2] float64, or nullptr
     unsigned long long* hist_counts;     // [V][active o][nbins_o+2], or nullptr
-    int info_off, lep_off, corr_off;     // byte offsets inside a warp's region
+    int order_off, lep_off, corr_off, bucket_off;   // byte offsets inside a warp's region
     int region_bytes, shared_bytes;      // per-warp region; CTA-shared part in front of the regions
     int flush_tiles;                     // warp 0 of a CTA flushes the histograms every this many of its tiles
 };
@@ -73,7 +77,7 @@ namespace dev {
 
 // CTA-shared part of shared memory (in front of the warps' staging regions).
 struct ChainShared {
-    float *edges, *axis_lo, *axis_inv;
+    float *edges, *axis_lo, *axis_inv;   // axis_inv == 0: the axis is not uniform enough for the arithmetic bin guess
     float *cal_pt_edges, *cal_eta_edges, *cal_table;
     float* h_sumw;
     unsigned int* h_cnt;
@@ -99,17 +103,67 @@ __host__ __device__ inline size_t chain_shared_layout(const ChainParams& P, bool
     return align_up(o, 128);
 }
 
-// Histogram slot of one observable (uniform branch on whether the observable is histogrammed).
-template <int OB>
-__device__ __forceinline__ int obs_slot(const ChainParams& P, const ChainShared& S, float x)
+// ---- shared-memory atomics in the shared state space (no generic-address dispatch) ----------------------
+__device__ __forceinline__ unsigned int atom_add_shared_u32(uint32_t addr, unsigned int v)
 {
-    if (!P.axis_edges[OB]) return -1;
-    return P.obs_prefix[OB] + hist_slot(x, S.edges + P.edge_prefix[OB], P.axis_nbins[OB], S.axis_lo[OB], S.axis_inv[OB]);
+    unsigned int r;
+    asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(r) : "r"(addr), "r"(v) : "memory");
+    return r;
+}
+__device__ __forceinline__ void red_add_shared_u32(uint32_t addr, unsigned int v)
+{
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_add_shared_f32(uint32_t addr, float v)
+{
+    asm volatile("red.shared.add.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float sqrt_approx(float x)
+{
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
 }
 
-// dR^2 < thr, exact class.  Same value as dr2_exact: with a = |dphi| and t = a - 2PI_F, the wrapped magnitude
-// is min(a, |t|): a > PI_F  =>  |t| <= PI_F < a (rn is monotone), a < PI_F  =>  |t| >= PI_F > a, and at
-// a == PI_F both are PI_F.  Three instructions for the wrap instead of four (|.| is a free operand modifier).
+// Histogram slot (0 underflow, 1+b, nbins+1 overflow/NaN).  inv != 0 means the kernel has verified at start-up
+// that |(edges[i] - lo) * inv - i| <= 0.5 for every edge; the same monotone float32 expression applied to x then
+// lands within one bin of the right one, and a single +-1 step against the edges makes the result exact.
+__device__ __forceinline__ int slot_lean(float x, const float* edges, int nb, float lo, float inv)
+{
+    if (inv == 0.0f) {       // irregular axis: binary search on the edges
+        if (x < edges[0]) return 0;
+        if (!(x < edges[nb])) return nb + 1;
+        int a = 0, b = nb;
+        while (b - a > 1) {
+            const int mid = (a + b) >> 1;
+            if (x >= edges[mid]) a = mid; else b = mid;
+        }
+        return 1 + a;
+    }
+    int g = (int)((x - lo) * inv);                 // NaN -> 0, +-inf saturate
+    g = max(0, min(g, nb - 1));
+    const float a = edges[g], b = edges[g + 1];
+    int s = g + 1;
+    s += (x >= b) ? 1 : 0;
+    s -= (x < a) ? 1 : 0;
+    return (x != x) ? nb + 1 : s;
+}
+
+// dR^2, exact class.  Same value as dr2_exact: with a = |dphi| and t = a - 2PI_F, the wrapped magnitude is
+// min(a, |t|): a > PI_F  =>  |t| <= PI_F < a (rn is monotone), a < PI_F  =>  |t| >= PI_F > a, and at a == PI_F
+// both are PI_F.  Three instructions for the wrap instead of four (|.| is a free operand modifier).
 __device__ __forceinline__ float dr2_min(float eta_a, float phi_a, float eta_b, float phi_b)
 {
     const float deta = __fsub_rn(eta_a, eta_b);
@@ -117,6 +171,73 @@ __device__ __forceinline__ float dr2_min(float eta_a, float phi_a, float eta_b, 
     const float t = __fsub_rn(fabsf(d), HEPK_TWO_PI_F);
     const float w = fminf(fabsf(d), fabsf(t));
     return __fadd_rn(__fmul_rn(deta, deta), __fmul_rn(w, w));
+}
+
+// pair_mass_fast (hepk_common.cuh) with the hardware approximations (ex2, rcp, sqrt: 1-2 ulp each) in place of
+// the library calls; tolerance class, every term of M^2 >= 0, ~60 instructions.
+__device__ __forceinline__ float pair_mass_lean(float pt1, float eta1, float phi1, float m1,
+                                                float pt2, float eta2, float phi2, float m2)
+{
+    const float LOG2E = 1.44269504088896341f;
+    const float e1 = ex2_approx(eta1 * LOG2E), e2 = ex2_approx(eta2 * LOG2E);
+    const float ch1 = 0.5f * (e1 + rcp_approx(e1));
+    const float ch2 = 0.5f * (e2 + rcp_approx(e2));
+    const float h = 0.5f * fabsf(eta1 - eta2);
+    const float h2 = h * h;
+    float sh_small = fmaf(h2, 1.0f / 39916800.0f, 1.0f / 362880.0f);
+    sh_small = fmaf(sh_small, h2, 1.0f / 5040.0f);
+    sh_small = fmaf(sh_small, h2, 1.0f / 120.0f);
+    sh_small = fmaf(sh_small, h2, 1.0f / 6.0f);
+    sh_small = fmaf(sh_small * h2, h, h);
+    const float eh = ex2_approx(h * LOG2E);
+    const float sh_big = 0.5f * (eh - rcp_approx(eh));
+    const float sh = h <= 1.0f ? sh_small : sh_big;
+    float d = __fsub_rn(phi1, phi2);
+    const float bb = __fsub_rn(d, phi1);
+    float dl = __fsub_rn(__fsub_rn(phi1, __fsub_rn(d, bb)), __fadd_rn(phi2, bb));
+    const float TWO_PI_LO = -1.7484555e-07f;   // 2*pi - TWO_PI_F
+    if (d > HEPK_PI_F) { d = __fsub_rn(d, HEPK_TWO_PI_F); dl = __fsub_rn(dl, TWO_PI_LO); }
+    else if (d < -HEPK_PI_F) { d = __fadd_rn(d, HEPK_TWO_PI_F); dl = __fadd_rn(dl, TWO_PI_LO); }
+    const float x_ = 0.5f * (d + dl), z = x_ * x_;
+    float sn = fmaf(z, 1.0f / 6227020800.0f, -1.0f / 39916800.0f);
+    sn = fmaf(sn, z, 1.0f / 362880.0f);
+    sn = fmaf(sn, z, -1.0f / 5040.0f);
+    sn = fmaf(sn, z, 1.0f / 120.0f);
+    sn = fmaf(sn, z, -1.0f / 6.0f);
+    sn = fmaf(sn * z, x_, x_);
+    const float r1 = m1 * rcp_approx(pt1 * ch1), r2 = m2 * rcp_approx(pt2 * ch2);
+    const float x1 = r1 * r1, x2 = r2 * r2;
+    const float x = x1 + x2 + x1 * x2;
+    const float t = x * rcp_approx(sqrt_approx(1.0f + x) + 1.0f);
+    const float bracket = ch1 * ch2 * t + 2.0f * (sh * sh + sn * sn);
+    const float msq = m1 * m1 + m2 * m2 + 2.0f * pt1 * pt2 * bracket;
+    return sqrt_approx(fmaxf(msq, 0.0f));
+}
+
+// One observable of one event and variant into the privatised histograms (`wt0` = weight column 0).
+template <int OB>
+__device__ __forceinline__ void fill_obs(const ChainParams& P, const ChainShared& S, long long ev, int v, int slot, float wt0)
+{
+    if (!P.axis_edges[OB]) return;
+    const int spv = P.obs_prefix[HEPK_N_OBS], pre = P.obs_prefix[OB];
+    if (P.hist_counts) red_add_shared_u32(smem_u32(S.h_cnt) + 4u * (unsigned)(v * spv + pre + slot), 1u);
+    if (P.hist_acc) {
+        // sumw layout [v][o][w][nbins_o + 2]
+        uint32_t a = smem_u32(S.h_sumw) + 4u * (unsigned)((v * spv + pre) * P.W + slot);
+        red_add_shared_f32(a, wt0);
+        const unsigned stride = 4u * (unsigned)(P.axis_nbins[OB] + 2);
+        for (int w = 1; w < P.W; ++w) {
+            a += stride;
+            red_add_shared_f32(a, __ldg(P.weights + (long long)w * P.n_events + ev));
+        }
+    }
+}
+
+template <int OB>
+__device__ __forceinline__ int obs_slot(const ChainParams& P, const ChainShared& S, float x)
+{
+    if (!P.axis_edges[OB]) return 0;
+    return slot_lean(x, S.edges + P.edge_prefix[OB], P.axis_nbins[OB], S.axis_lo[OB], S.axis_inv[OB]);
 }
 
 // Per event and variant: leading-pair mass, outputs, histograms.  Shared by the staged path and the per-event
@@ -129,16 +250,22 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     const bool hists = P.hist_acc || P.hist_counts;
     if (i2 >= 0) {
         subpt = b2;
-        mjj = pair_mass_fast(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
-        if (hists && P.axis_edges[HEPK_OBS_MJJ]) {
+        mjj = pair_mass_lean(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
+    }
+    int s_mjj = 0;
+    if (hists && P.axis_edges[HEPK_OBS_MJJ]) {
+        s_mjj = obs_slot<HEPK_OBS_MJJ>(P, S, mjj);
+        if (i2 >= 0) {
             // the bin of mjj is decided by the float64-defined value: refine when the fast value is near an edge
             const float* ed = S.edges + P.edge_prefix[HEPK_OBS_MJJ];
             const int nb = P.axis_nbins[HEPK_OBS_MJJ];
-            const int slot = hist_slot(mjj, ed, nb, S.axis_lo[HEPK_OBS_MJJ], S.axis_inv[HEPK_OBS_MJJ]);
             const float band = fmaf(mjj, HEPK_MASS_GUARD_REL, HEPK_MASS_GUARD_ABS);
-            const bool near_lo = slot >= 1 && mjj - ed[slot - 1] <= band;
-            const bool near_hi = slot <= nb && ed[slot] - mjj <= band;
-            if (near_lo || near_hi) mjj = pair_mass_f64(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
+            const bool near_lo = s_mjj >= 1 && mjj - ed[s_mjj - 1] <= band;
+            const bool near_hi = s_mjj <= nb && ed[s_mjj] - mjj <= band;
+            if (near_lo || near_hi) {
+                mjj = pair_mass_f64(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
+                s_mjj = obs_slot<HEPK_OBS_MJJ>(P, S, mjj);
+            }
         }
     }
     const long long o = (long long)v * P.n_events + ev;
@@ -150,33 +277,13 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     if (P.out_mjj) P.out_mjj[o] = mjj;
     if (P.out_subpt) P.out_subpt[o] = subpt;
     if (!hists) return;
-    int slot[HEPK_N_OBS];
-    slot[HEPK_OBS_NJET] = obs_slot<HEPK_OBS_NJET>(P, S, (float)cnt);
-    slot[HEPK_OBS_HT] = obs_slot<HEPK_OBS_HT>(P, S, sum);
-    slot[HEPK_OBS_MAXPT] = obs_slot<HEPK_OBS_MAXPT>(P, S, b1);
-    slot[HEPK_OBS_MINPT] = obs_slot<HEPK_OBS_MINPT>(P, S, mn);
-    slot[HEPK_OBS_MJJ] = obs_slot<HEPK_OBS_MJJ>(P, S, mjj);
-    slot[HEPK_OBS_SUBPT] = obs_slot<HEPK_OBS_SUBPT>(P, S, subpt);
-    const int spv = P.obs_prefix[HEPK_N_OBS];
-    if (P.hist_counts) {
-        unsigned int* hc = S.h_cnt + v * spv;
-#pragma unroll
-        for (int ob = 0; ob < HEPK_N_OBS; ++ob)
-            if (slot[ob] >= 0) atomicAdd(hc + slot[ob], 1u);
-    }
-    if (P.hist_acc) {
-        // sumw layout [v][o][w][nbins_o + 2]: slot index inside observable o's block moves with w
-        for (int w = 0; w < P.W; ++w) {
-            const float wt = P.weights ? __ldg(P.weights + (long long)w * P.n_events + ev) : 1.0f;
-            float* h = S.h_sumw + (size_t)v * spv * P.W;
-#pragma unroll
-            for (int ob = 0; ob < HEPK_N_OBS; ++ob) {
-                if (slot[ob] < 0) continue;
-                const int pre = P.obs_prefix[ob];
-                atomicAdd(h + (size_t)pre * P.W + (size_t)w * (P.axis_nbins[ob] + 2) + (slot[ob] - pre), wt);
-            }
-        }
-    }
+    const float wt0 = (P.hist_acc && P.weights) ? __ldg(P.weights + ev) : 1.0f;
+    fill_obs<HEPK_OBS_NJET>(P, S, ev, v, obs_slot<HEPK_OBS_NJET>(P, S, (float)cnt), wt0);
+    fill_obs<HEPK_OBS_HT>(P, S, ev, v, obs_slot<HEPK_OBS_HT>(P, S, sum), wt0);
+    fill_obs<HEPK_OBS_MAXPT>(P, S, ev, v, obs_slot<HEPK_OBS_MAXPT>(P, S, b1), wt0);
+    fill_obs<HEPK_OBS_MINPT>(P, S, ev, v, obs_slot<HEPK_OBS_MINPT>(P, S, mn), wt0);
+    fill_obs<HEPK_OBS_MJJ>(P, S, ev, v, s_mjj, wt0);
+    fill_obs<HEPK_OBS_SUBPT>(P, S, ev, v, obs_slot<HEPK_OBS_SUBPT>(P, S, subpt), wt0);
 }
 
 // Running per-event state of phase 2.
@@ -293,32 +400,48 @@ __device__ __forceinline__ void load_bounds(const ChainParams& P, const LaneCol&
     }
 }
 
-// Start the bulk copies of tile `tile` into the warp's staging region; all 32 lanes call it, converged.
-// Returns false (nothing issued) when some slice does not fit: capacity, 16-byte alignment at the array ends.
-// Element l of a column lands at buffer index l - a0, a0 = l0 - ((l0 + mis) mod A), so the copy is 16-byte
-// aligned on both sides; the consumer recomputes the same shift.
-__device__ __forceinline__ bool issue_tile(const ChainParams& P, const LaneCol& c, long long tile, int lane,
-                                           long long lo, long long hi, uint64_t* bar)
+// Low words of offsets[e] and offsets[e+1] of the lane's event (lane = event of the tile), three collections.
+struct EventOffsets { int j0, j1, m0, m1, q0, q1; };
+
+template <bool HAS_EL>
+__device__ __forceinline__ void load_event_offsets(const ChainParams& P, long long tile, int lane, EventOffsets& o)
 {
-    const long long e0 = tile * TILE_EVENTS;
-    const long long rest = P.n_events - e0;
-    const int ne = rest < TILE_EVENTS ? (int)rest : TILE_EVENTS;
-    const bool is_off = lane >= 10;
-    const int A = is_off ? 2 : 4, esh = is_off ? 3 : 2;
-    const long long l0 = is_off ? e0 : lo - c.base;
-    const long long l1 = is_off ? e0 + ne + 1 : hi - c.base;
+    const long long e = tile * TILE_EVENTS + lane;
+    const long long i0 = e < P.n_events ? e : P.n_events;
+    const long long i1 = e + 1 < P.n_events ? e + 1 : P.n_events;
+    o.j0 = (int)__ldg(P.off[0] + i0); o.j1 = (int)__ldg(P.off[0] + i1);
+    o.m0 = (int)__ldg(P.off[1] + i0); o.m1 = (int)__ldg(P.off[1] + i1);
+    if (HAS_EL) { o.q0 = (int)__ldg(P.off[2] + i0); o.q1 = (int)__ldg(P.off[2] + i1); }
+    else { o.q0 = 0; o.q1 = 0; }
+}
+
+// offsets[e0] of the jets (64-bit): lane 0 stages a jet column, so its `lo` bound is exactly that value
+__device__ __forceinline__ long long cur_lo_jets(const ChainParams&, long long cur_lo, int)
+{
+    const unsigned int a = __shfl_sync(0xffffffffu, (unsigned int)cur_lo, 0);
+    const unsigned int b = __shfl_sync(0xffffffffu, (unsigned int)((unsigned long long)cur_lo >> 32), 0);
+    return (long long)(((unsigned long long)b << 32) | a);
+}
+
+// Start the bulk copies of a tile into the warp's staging region; all 32 lanes call it, converged.
+// Returns false (nothing issued) when some slice does not fit: capacity, 16-byte alignment at the array ends.
+// Element l of a column lands at buffer index l - a0, a0 = l0 - ((l0 + mis) mod 4), so the copy is 16-byte
+// aligned on both sides; the consumer recomputes the same shift.
+__device__ __forceinline__ bool issue_tile(const LaneCol& c, int lane, long long lo, long long hi, uint64_t* bar)
+{
+    const long long l0 = lo - c.base, l1 = hi - c.base;
     const long long n = l1 - l0;
-    const int sh = ((int)l0 + c.mis) & (A - 1);
+    const int sh = ((int)l0 + c.mis) & 3;
     const long long a0 = l0 - sh;
-    const long long len = (n + sh + A - 1) & ~(long long)(A - 1);
+    const long long len = (n + sh + 3) & ~3ll;
     const bool active = c.ptr != nullptr && n != 0;
     const bool ok = !active || (n > 0 && n <= c.cap && a0 >= 0 && a0 + len <= c.n);
     if (!__all_sync(0xffffffffu, ok)) return false;
-    const uint32_t bytes = active ? ((uint32_t)len << esh) : 0u;
+    const uint32_t bytes = active ? ((uint32_t)len << 2) : 0u;
     const uint32_t total = __reduce_add_sync(0xffffffffu, bytes);
     if (lane == 0) mbar_arrive_expect_tx(bar, total);
     __syncwarp();
-    if (active) bulk_g2s_addr(c.dst, c.ptr + (a0 << esh), bytes, bar);
+    if (active) bulk_g2s_addr(c.dst, c.ptr + (a0 << 2), bytes, bar);
     return true;
 }
 
@@ -338,16 +461,12 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
         mbar_init(bar, 1);
         fence_mbar_init();
     }
+    if (lane < 2 * N_BUCKETS) ((int*)(R + P.bucket_off))[lane] = 0;
 #pragma unroll
     for (int ob = 0; ob < HEPK_N_OBS; ++ob) {
         if (!P.axis_edges[ob]) continue;
         const int nb = P.axis_nbins[ob];
         for (int i = tid; i <= nb; i += nthr) S.edges[P.edge_prefix[ob] + i] = P.axis_edges[ob][i];
-        if (tid == 0) {
-            const float lo = P.axis_edges[ob][0], hi = P.axis_edges[ob][nb];
-            S.axis_lo[ob] = lo;
-            S.axis_inv[ob] = (float)nb / (hi - lo);
-        }
     }
     if (CALIB) {
         for (int i = tid; i <= P.cal_npt; i += nthr) S.cal_pt_edges[i] = P.cal_pt_edges[i];
@@ -358,6 +477,23 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
         const int spv = P.obs_prefix[HEPK_N_OBS];
         if (P.hist_acc) for (int i = tid; i < spv * P.V * P.W; i += nthr) S.h_sumw[i] = 0.0f;
         if (P.hist_counts) for (int i = tid; i < spv * P.V; i += nthr) S.h_cnt[i] = 0u;
+    }
+    __syncthreads();
+    // per axis: is the arithmetic bin guess of slot_lean safe?  (|(edges[i] - lo) * inv - i| <= 0.5 for every edge)
+#pragma unroll
+    for (int ob = 0; ob < HEPK_N_OBS; ++ob) {
+        if (!P.axis_edges[ob]) continue;
+        const int nb = P.axis_nbins[ob];
+        const float* ed = S.edges + P.edge_prefix[ob];
+        const float lo = ed[0], hi = ed[nb];
+        const float inv = (float)nb / (hi - lo);
+        bool ok = (hi > lo) && (inv > 0.0f) && (inv < CUDART_INF_F);
+        for (int i = tid; i <= nb; i += nthr) ok = ok && (fabsf((ed[i] - lo) * inv - (float)i) <= 0.5f);
+        ok = __syncthreads_and(ok);
+        if (tid == 0) {
+            S.axis_lo[ob] = lo;
+            S.axis_inv[ob] = ok ? inv : 0.0f;
+        }
     }
     LaneCol col;
     col.ptr = nullptr; col.off = nullptr; col.base = 0; col.n = 0; col.mis = 0; col.cap = 0; col.dst = 0;
@@ -371,24 +507,27 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
     }
     __syncthreads();
 
-    // staging buffers of this warp
-    const int* const so_j = (const int*)(R + P.col_dst[10]) + 2 * P.col_mis[10];   // low words of the offsets slices
-    const int* const so_m = (const int*)(R + P.col_dst[11]) + 2 * P.col_mis[11];
-    const int* const so_e = (const int*)(R + P.col_dst[12]) + 2 * P.col_mis[12];
-    unsigned short* const sinfo = (unsigned short*)(R + P.info_off);
+    // this warp's buffers
+    unsigned int* const sorder = (unsigned int*)(R + P.order_off);
     float2* const slep = (float2*)(R + P.lep_off);
     float* const scorr = (float*)(R + P.corr_off);
+    const uint32_t bucket_a = smem_u32(R + P.bucket_off);
     const int V = CALIB ? P.V : 1;
 
     const long long GW = (long long)gridDim.x * nwarp;
     long long tile = (long long)warp * gridDim.x + blockIdx.x;
     uint32_t parity = 0;
-    int since_flush = 0;
+    int since_flush = 0, bsel = 0;
     bool fit = false;
+    long long cur_lo = 0;
+    EventOffsets eo;
+    eo.j0 = eo.j1 = eo.m0 = eo.m1 = eo.q0 = eo.q1 = 0;
     if (tile < P.n_tiles) {
         long long lo, hi;
         load_bounds(P, col, tile, lo, hi);
-        fit = issue_tile(P, col, tile, lane, lo, hi, bar);
+        load_event_offsets<HAS_EL>(P, tile, lane, eo);
+        fit = issue_tile(col, lane, lo, hi, bar);
+        cur_lo = lo;
     }
 
     for (; tile < P.n_tiles; tile += GW) {
@@ -398,83 +537,101 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
         const long long tile_next = tile + GW;
         const bool has_next = tile_next < P.n_tiles;
         long long nlo = 0, nhi = 0;
-        if (has_next) load_bounds(P, col, tile_next, nlo, nhi);
+        EventOffsets neo;
+        neo.j0 = neo.j1 = neo.m0 = neo.m1 = neo.q0 = neo.q1 = 0;
+        if (has_next) {
+            load_bounds(P, col, tile_next, nlo, nhi);
+            load_event_offsets<HAS_EL>(P, tile_next, lane, neo);
+        }
         bool staged = fit;
         bool released = false;
         fit = false;
 
         if (staged) {
-            mbar_wait(bar, parity);
-            parity ^= 1u;
-            // ---- phase 0: one lane per event
-            const int jb = so_j[0], mb = so_m[0], qb = HAS_EL ? so_e[0] : 0;
-            const int njt = so_j[2 * ne] - jb;
-            const float* spt = (const float*)(R + P.col_dst[0]) + ((jb + P.sh_add[0]) & 3);
+            // ---- phase 0: one lane per event.  Offsets are in registers; the lepton columns are needed first.
+            const int jb = __shfl_sync(0xffffffffu, eo.j0, 0);
+            const int mb = __shfl_sync(0xffffffffu, eo.m0, 0);
+            const int qb = __shfl_sync(0xffffffffu, eo.q0, 0);
+            const int njt = __shfl_sync(0xffffffffu, eo.j1, ne - 1) - jb;
+            float* spt = (float*)(R + P.col_dst[0]) + ((jb + P.sh_add[0]) & 3);
             const float* seta = (const float*)(R + P.col_dst[1]) + ((jb + P.sh_add[1]) & 3);
             const float* sphi = (const float*)(R + P.col_dst[2]) + ((jb + P.sh_add[2]) & 3);
             const float* smass = (const float*)(R + P.col_dst[3]) + ((jb + P.sh_add[3]) & 3);
-            int kj0 = 0, nj = 0, c = 0;
-            if (lane < ne) {
-                kj0 = so_j[2 * lane] - jb;
-                nj = so_j[2 * lane + 2] - so_j[2 * lane];
-                const int m0 = so_m[2 * lane] - mb, nm = so_m[2 * lane + 2] - so_m[2 * lane];
-                int q0 = 0, nq = 0;
-                if (HAS_EL) { q0 = so_e[2 * lane] - qb; nq = so_e[2 * lane + 2] - so_e[2 * lane]; }
-                const int l0 = m0 + q0;
-                {
-                    const float* lp = (const float*)(R + P.col_dst[4]) + ((mb + P.sh_add[4]) & 3) + m0;
-                    const float* le = (const float*)(R + P.col_dst[5]) + ((mb + P.sh_add[5]) & 3) + m0;
-                    const float* lf = (const float*)(R + P.col_dst[6]) + ((mb + P.sh_add[6]) & 3) + m0;
-                    for (int i = 0; i < nm; ++i)
-                        if (lp[i] > P.lep_pt_min) {
-                            if (c < MAX_LEP_EVENT) slep[l0 + c] = make_float2(le[i], lf[i]);
-                            ++c;
-                        }
-                }
-                if (HAS_EL) {
-                    const float* lp = (const float*)(R + P.col_dst[7]) + ((qb + P.sh_add[7]) & 3) + q0;
-                    const float* le = (const float*)(R + P.col_dst[8]) + ((qb + P.sh_add[8]) & 3) + q0;
-                    const float* lf = (const float*)(R + P.col_dst[9]) + ((qb + P.sh_add[9]) & 3) + q0;
-                    for (int i = 0; i < nq; ++i)
-                        if (lp[i] > P.lep_pt_min) {
-                            if (c < MAX_LEP_EVENT) slep[l0 + c] = make_float2(le[i], lf[i]);
-                            ++c;
-                        }
-                }
-                const unsigned short info = (unsigned short)(l0 | (c << 11));
-                unsigned short* ip = sinfo + kj0;
-                for (int k = 0; k < nj; ++k) ip[k] = info;
+            const bool live = lane < ne;
+            const int kj0 = live ? eo.j0 - jb : 0, nj = live ? eo.j1 - eo.j0 : 0;
+            const int km0 = eo.m0 - mb, nm = live ? eo.m1 - eo.m0 : 0;
+            const int kq0 = eo.q0 - qb, nq = (HAS_EL && live) ? eo.q1 - eo.q0 : 0;
+            const int l0 = live ? km0 + kq0 : 0;
+            mbar_wait(bar, parity);
+            parity ^= 1u;
+            int c = 0;
+            {
+                const float* lp = (const float*)(R + P.col_dst[4]) + ((mb + P.sh_add[4]) & 3) + km0;
+                const float* le = (const float*)(R + P.col_dst[5]) + ((mb + P.sh_add[5]) & 3) + km0;
+                const float* lf = (const float*)(R + P.col_dst[6]) + ((mb + P.sh_add[6]) & 3) + km0;
+                float2* out = slep + l0;
+#pragma unroll 1
+                for (int i = 0; i < nm; ++i)
+                    if (lp[i] > P.lep_pt_min) out[c++] = make_float2(le[i], lf[i]);
             }
+            if (HAS_EL) {
+                const float* lp = (const float*)(R + P.col_dst[7]) + ((qb + P.sh_add[7]) & 3) + kq0;
+                const float* le = (const float*)(R + P.col_dst[8]) + ((qb + P.sh_add[8]) & 3) + kq0;
+                const float* lf = (const float*)(R + P.col_dst[9]) + ((qb + P.sh_add[9]) & 3) + kq0;
+                float2* out = slep + l0;
+#pragma unroll 1
+                for (int i = 0; i < nq; ++i)
+                    if (lp[i] > P.lep_pt_min) out[c++] = make_float2(le[i], lf[i]);
+            }
+            // bucket the event's jets by its number of selected leptons: position inside the bucket from a
+            // shared-memory counter (any order inside a bucket will do), bucket bases from the eight totals
+            const int key = c < N_BUCKETS - 1 ? c : N_BUCKETS - 1;
+            const uint32_t bk = bucket_a + (uint32_t)bsel * (4u * N_BUCKETS);
+            int pos = 0;
+            if (nj > 0) pos = (int)atom_add_shared_u32(bk + 4u * (unsigned)key, (unsigned)nj);
+            if (lane < N_BUCKETS) ((int*)(R + P.bucket_off))[(bsel ^ 1) * N_BUCKETS + lane] = 0;   // the other set, for the next tile
             // an event with more selected leptons than the packed word can count: the whole tile goes the slow way
             staged = !__any_sync(0xffffffffu, c > MAX_LEP_EVENT);
             __syncwarp();
-
             if (staged) {
-                // ---- phase 1: one lane per jet
-                const long long lj0 = ((const long long*)(R + P.col_dst[10]) + P.col_mis[10])[0] - P.jbase;
-                float* wpt = const_cast<float*>(spt);
-                for (int j = lane; j < njt; j += 32) {
-                    const unsigned int info = sinfo[j];
-                    const float eta = seta[j], phi = sphi[j];
-                    const float2* L = slep + (info & 2047u);
-                    const int n = (int)(info >> 11);
-                    bool matched = false;
-                    for (int t = 0; t < n; ++t) {
-                        const float2 l = L[t];
-                        matched |= dr2_min(eta, phi, l.x, l.y) < P.dr2_max;
+                const int4 t0 = ((const int4*)(R + P.bucket_off))[bsel * 2], t1 = ((const int4*)(R + P.bucket_off))[bsel * 2 + 1];
+                int base = 0;
+                base += key > 0 ? t0.x : 0; base += key > 1 ? t0.y : 0; base += key > 2 ? t0.z : 0; base += key > 3 ? t0.w : 0;
+                base += key > 4 ? t1.x : 0; base += key > 5 ? t1.y : 0; base += key > 6 ? t1.z : 0;
+                {
+                    unsigned int word = (unsigned)kj0 | ((unsigned)l0 << 10) | ((unsigned)c << 21);
+                    unsigned int* op = sorder + base + pos;
+#pragma unroll 1
+                    for (int k = 0; k < nj; ++k) op[k] = word + (unsigned)k;
+                }
+                __syncwarp();
+
+                // ---- phase 1: one lane per jet, in bucket order (neighbouring lanes: same lepton count)
+                const long long lj0 = cur_lo_jets(P, cur_lo, lane) - P.jbase;
+#pragma unroll 1
+                for (int t = lane; t < njt; t += 32) {
+                    const unsigned int word = sorder[t];
+                    const int j = (int)(word & 1023u);
+                    const float2* L = slep + ((word >> 10) & 2047u);
+                    const int n = (int)(word >> 21);
+                    const float eta = seta[j], phi = sphi[j], pt = spt[j];
+                    float dmin = CUDART_INF_F;
+#pragma unroll 1
+                    for (int i = 0; i < n; ++i) {
+                        const float2 l = L[i];
+                        dmin = fminf(dmin, dr2_min(eta, phi, l.x, l.y));
                     }
-                    const float pt = spt[j];
-                    const bool base = (fabsf(eta) < P.jet_abs_eta_max) && !matched;
+                    const bool base = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
                     if (!CALIB) {
                         const bool clean = base && (pt > P.jet_pt_min);
                         if (P.out_jet_mask) P.out_jet_mask[lj0 + j] = clean ? 1 : 0;
-                        wpt[j] = clean ? pt : -CUDART_INF_F;
+                        spt[j] = clean ? pt : -CUDART_INF_F;
                     } else {
                         const int bx = find_bin_clamped(pt, S.cal_pt_edges, P.cal_npt);
                         const int by = find_bin_clamped(eta, S.cal_eta_edges, P.cal_neta);
                         const float cf = S.cal_table[bx * P.cal_neta + by];
                         scorr[j] = cf;
-                        if (!base) wpt[j] = CUDART_NAN_F;
+                        if (!base) spt[j] = CUDART_NAN_F;
                         if (P.out_jet_mask)
                             for (int v = 0; v < V; ++v)
                                 P.out_jet_mask[(long long)v * P.jn + lj0 + j] =
@@ -490,6 +647,7 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
                     const float sv = P.scales[v];
                     EventAcc a;
                     a.init();
+#pragma unroll 1
                     for (int k = 0; k < nj; ++k) {
                         float p = pp[k];
                         bool ok;
@@ -512,21 +670,24 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
                         // the staging region is dead from here: start the next tile's copies under the finishing math
                         fence_proxy_async_smem();
                         __syncwarp();
-                        if (has_next) fit = issue_tile(P, col, tile_next, lane, nlo, nhi, bar);
+                        if (has_next) fit = issue_tile(col, lane, nlo, nhi, bar);
                         released = true;
                     }
-                    if (lane < ne)
+                    if (live)
                         finish_event(P, S, e0 + lane, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
                 }
             }
+            bsel ^= 1;
         }
         if (!released) {
             fence_proxy_async_smem();
             __syncwarp();
-            if (has_next) fit = issue_tile(P, col, tile_next, lane, nlo, nhi, bar);
+            if (has_next) fit = issue_tile(col, lane, nlo, nhi, bar);
         }
         if (!staged && lane < ne) chain_event_global<CALIB>(P, S, e0 + lane);
         __syncwarp();
+        eo = neo;
+        cur_lo = nlo;
 
         if (warp == 0 && ++since_flush >= P.flush_tiles) {
             flush_hist(P, S, lane, 32);
@@ -604,19 +765,10 @@ static int chain_region_layout(ChainParams& P, const hepk_chain_desc* d, bool ca
         const long long b = coll[k]->content_base % 4;
         P.sh_add[c] = (int)(((P.col_mis[c] - b) % 4 + 4) % 4);
     }
-    for (int k = 0; k < 3; ++k) {
-        const int c = 10 + k;
-        P.col_ptr[c] = (const char*)coll[k]->offsets;
-        P.col_base[c] = 0;
-        P.col_n[c] = d->n_events + 1;
-        P.col_mis[c] = (int)((reinterpret_cast<uintptr_t>(coll[k]->offsets) / 8) % 2);
-        P.col_cap[c] = TILE_EVENTS + 1;
-        P.col_coll[c] = k;
-        P.col_dst[c] = take((size_t)(TILE_EVENTS + 1 + 3) * 8);
-    }
-    P.info_off = take((size_t)cap_j * 2);
+    P.order_off = take((size_t)cap_j * 4);
     P.lep_off = take((size_t)(cap_m + cap_e) * 8);
     P.corr_off = take(calib ? (size_t)cap_j * 4 : 0);
+    P.bucket_off = take(2 * N_BUCKETS * 4);
     return (int)dev::align_up(o, 128);
 }
 
@@ -670,6 +822,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     int cap_e = has_el ? round_up4(d->tune_cap_leptons > 0 ? d->tune_cap_leptons
                                                               : cap_for((double)d->electrons.n_objects / nev, 32)) : 0;
     if (cap_j < 16) cap_j = 16;
+    if (cap_j > MAX_JETS_TILE) cap_j = MAX_JETS_TILE;      // the jet index is packed in 10 bits
     if (cap_m < 4) cap_m = 4;
     if (has_el && cap_e < 4) cap_e = 4;
     if (cap_m > MAX_LIST / 2 - 4) cap_m = MAX_LIST / 2 - 4;      // the list start is packed in 11 bits
