@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--impl", default="hepk", choices=["hepk", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tune", default="", help="chain tuning knobs, e.g. warps_per_sm=20,ctas_per_sm=1 (testing only)")
     ap.add_argument("--ref-sample", type=int, default=1_000_000, help="events per step of the reference arm")
     return ap.parse_args()
 
@@ -195,7 +196,8 @@ def run_hepk(args):
     V = 1 if wl.calib is None else len(wl.calib["scales"])
     inp = hk.upload(wl)
     hists_only = args.config == 4          # config 4 writes histograms only
-    plan = hk.ChainPlan(inp, want_event_outputs=False if hists_only else BENCH_OUTPUTS)
+    tune = {k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(",") if kv)}
+    plan = hk.ChainPlan(inp, want_event_outputs=False if hists_only else BENCH_OUTPUTS, tune=tune or None)
     alg_bytes = algorithmic_bytes(wl, event_outputs=not hists_only)
     hist_t = [plan.out["hist_sumw"], plan.out["hist_counts"]]
 

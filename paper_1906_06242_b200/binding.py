@@ -50,7 +50,7 @@ class ChainDesc(C.Structure):
         ("out_jet_mask", C.c_void_p),
         ("hist_sumw", C.c_void_p), ("hist_counts", C.c_void_p),
         ("tune_cap_jets", C.c_int32), ("tune_cap_leptons", C.c_int32),
-        ("tune_ctas_per_sm", C.c_int32), ("tune_warps_per_cta", C.c_int32),
+        ("tune_ctas_per_sm", C.c_int32), ("tune_warps_per_cta", C.c_int32), ("tune_warps_per_sm", C.c_int32),
     ]
 
 

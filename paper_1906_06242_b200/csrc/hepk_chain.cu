@@ -30,9 +30,9 @@ namespace hepk {
 
 constexpr int TILE_EVENTS = 32;     // events per warp tile
 constexpr int NCOL = 10;            // staged columns: 0-3 jets pt,eta,phi,mass; 4-6 muons pt,eta,phi; 7-9 electrons
-constexpr int MAX_JETS_TILE = 1024; // jet index inside a tile fits 10 bits
-constexpr int MAX_LIST = 2047;      // combined lepton list start fits 11 bits
-constexpr int MAX_LEP_EVENT = 31;   // selected leptons of one event fit 5 bits
+constexpr int MAX_JETS_TILE = 512;  // byte offset of a jet inside a tile column (4 * index) fits 11 bits
+constexpr int MAX_LIST = 1023;      // byte offset of an event's lepton list (8 * start) fits 13 bits
+constexpr int MAX_LEP_EVENT = 31;   // byte length of an event's lepton list (8 * count) fits 8 bits
 constexpr int N_BUCKETS = 8;        // jets are ordered by min(selected leptons of their event, 7)
 
 struct ChainParams {
@@ -48,6 +48,7 @@ struct ChainParams {
     int col_coll[NCOL];             // collection 0 jets, 1 muons, 2 electrons
     int n_col;                      // NCOL, or 0 when the staged path is disabled
     int sh_add[NCOL];               // (col_mis - content_base) mod 4: shift = (lo32(offsets[e0]) + sh_add) & 3
+    int col_stride[3];              // bytes between the staging buffers of consecutive columns of a collection
     const long long* off[3];        // offsets arrays: jets, muons, electrons (electrons nullptr if absent)
     long long jn;
     const float *jpt, *jeta, *jphi, *jmass; long long jbase;
@@ -117,6 +118,37 @@ __device__ __forceinline__ void red_add_shared_u32(uint32_t addr, unsigned int v
 __device__ __forceinline__ void red_add_shared_f32(uint32_t addr, float v)
 {
     asm volatile("red.shared.add.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+// ---- shared-memory loads / stores by 32-bit shared address (keeps address arithmetic to one add) ----------
+__device__ __forceinline__ float lds_f32(uint32_t a)
+{
+    float r;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(a) : "memory");
+    return r;
+}
+__device__ __forceinline__ unsigned int lds_u32(uint32_t a)
+{
+    unsigned int r;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(a) : "memory");
+    return r;
+}
+__device__ __forceinline__ float2 lds_v2(uint32_t a)
+{
+    float2 r;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(a) : "memory");
+    return r;
+}
+__device__ __forceinline__ int4 lds_v4i(uint32_t a)
+{
+    int4 r;
+    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(a) : "memory");
+    return r;
+}
+__device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void sts_u32(uint32_t a, unsigned int v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts_v2(uint32_t a, float x, float y)
+{
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(x), "f"(y) : "memory");
 }
 __device__ __forceinline__ float ex2_approx(float x)
 {
@@ -214,18 +246,44 @@ __device__ __forceinline__ float pair_mass_lean(float pt1, float eta1, float phi
     return sqrt_approx(fmaxf(msq, 0.0f));
 }
 
+// What the launch asked for, as one register of flags (tested with one instruction instead of a pointer compare).
+enum : unsigned {
+    F_NJET = 1u << 0, F_ARGMAX = 1u << 1, F_HT = 1u << 2, F_MAXPT = 1u << 3, F_MINPT = 1u << 4, F_MJJ = 1u << 5,
+    F_SUBPT = 1u << 6, F_OBS0 = 1u << 8 /* .. << 13 */, F_COUNTS = 1u << 16, F_SUMW = 1u << 17, F_WEIGHTS = 1u << 18
+};
+__device__ __forceinline__ unsigned chain_features(const ChainParams& P)
+{
+    unsigned f = 0;
+    if (P.out_njet) f |= F_NJET;
+    if (P.out_argmax) f |= F_ARGMAX;
+    if (P.out_ht) f |= F_HT;
+    if (P.out_maxpt) f |= F_MAXPT;
+    if (P.out_minpt) f |= F_MINPT;
+    if (P.out_mjj) f |= F_MJJ;
+    if (P.out_subpt) f |= F_SUBPT;
+#pragma unroll
+    for (int ob = 0; ob < HEPK_N_OBS; ++ob)
+        if (P.axis_edges[ob]) f |= F_OBS0 << ob;
+    if (P.hist_counts) f |= F_COUNTS;
+    if (P.hist_acc) f |= F_SUMW;
+    if (P.weights) f |= F_WEIGHTS;
+    return f;
+}
+
 // One observable of one event and variant into the privatised histograms (`wt0` = weight column 0).
 template <int OB>
-__device__ __forceinline__ void fill_obs(const ChainParams& P, const ChainShared& S, long long ev, int v, int slot, float wt0)
+__device__ __forceinline__ void fill_obs(const ChainParams& P, const ChainShared& S, unsigned feat, long long ev, int v, float x, float wt0)
 {
-    if (!P.axis_edges[OB]) return;
+    if (!(feat & (F_OBS0 << OB))) return;
+    const int nb = P.axis_nbins[OB];
+    const int slot = slot_lean(x, S.edges + P.edge_prefix[OB], nb, S.axis_lo[OB], S.axis_inv[OB]);
     const int spv = P.obs_prefix[HEPK_N_OBS], pre = P.obs_prefix[OB];
-    if (P.hist_counts) red_add_shared_u32(smem_u32(S.h_cnt) + 4u * (unsigned)(v * spv + pre + slot), 1u);
-    if (P.hist_acc) {
+    if (feat & F_COUNTS) red_add_shared_u32(smem_u32(S.h_cnt) + 4u * (unsigned)(v * spv + pre + slot), 1u);
+    if (feat & F_SUMW) {
         // sumw layout [v][o][w][nbins_o + 2]
         uint32_t a = smem_u32(S.h_sumw) + 4u * (unsigned)((v * spv + pre) * P.W + slot);
         red_add_shared_f32(a, wt0);
-        const unsigned stride = 4u * (unsigned)(P.axis_nbins[OB] + 2);
+        const unsigned stride = 4u * (unsigned)(nb + 2);
         for (int w = 1; w < P.W; ++w) {
             a += stride;
             red_add_shared_f32(a, __ldg(P.weights + (long long)w * P.n_events + ev));
@@ -233,57 +291,44 @@ __device__ __forceinline__ void fill_obs(const ChainParams& P, const ChainShared
     }
 }
 
-template <int OB>
-__device__ __forceinline__ int obs_slot(const ChainParams& P, const ChainShared& S, float x)
-{
-    if (!P.axis_edges[OB]) return 0;
-    return slot_lean(x, S.edges + P.edge_prefix[OB], P.axis_nbins[OB], S.axis_lo[OB], S.axis_inv[OB]);
-}
-
 // Per event and variant: leading-pair mass, outputs, histograms.  Shared by the staged path and the per-event
 // path.  The leading jets' (eta, phi, mass) are passed in by value; i2 < 0 means fewer than two clean jets.
-__device__ __forceinline__ void finish_event(const ChainParams& P, const ChainShared& S, long long ev, int v,
+__device__ __forceinline__ void finish_event(const ChainParams& P, const ChainShared& S, unsigned feat, long long ev, int v,
                                              int cnt, float sum, float mn, float b1, float b2, int i1, int i2,
                                              float eta1, float phi1, float m1, float eta2, float phi2, float m2)
 {
     float mjj = 0.0f, subpt = 0.0f;
-    const bool hists = P.hist_acc || P.hist_counts;
+    const bool hists = (feat & (F_COUNTS | F_SUMW)) != 0;
     if (i2 >= 0) {
         subpt = b2;
         mjj = pair_mass_lean(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
-    }
-    int s_mjj = 0;
-    if (hists && P.axis_edges[HEPK_OBS_MJJ]) {
-        s_mjj = obs_slot<HEPK_OBS_MJJ>(P, S, mjj);
-        if (i2 >= 0) {
+        if (hists && (feat & (F_OBS0 << HEPK_OBS_MJJ))) {
             // the bin of mjj is decided by the float64-defined value: refine when the fast value is near an edge
             const float* ed = S.edges + P.edge_prefix[HEPK_OBS_MJJ];
             const int nb = P.axis_nbins[HEPK_OBS_MJJ];
+            const int s = slot_lean(mjj, ed, nb, S.axis_lo[HEPK_OBS_MJJ], S.axis_inv[HEPK_OBS_MJJ]);
             const float band = fmaf(mjj, HEPK_MASS_GUARD_REL, HEPK_MASS_GUARD_ABS);
-            const bool near_lo = s_mjj >= 1 && mjj - ed[s_mjj - 1] <= band;
-            const bool near_hi = s_mjj <= nb && ed[s_mjj] - mjj <= band;
-            if (near_lo || near_hi) {
-                mjj = pair_mass_f64(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
-                s_mjj = obs_slot<HEPK_OBS_MJJ>(P, S, mjj);
-            }
+            const bool near_lo = s >= 1 && mjj - ed[s - 1] <= band;
+            const bool near_hi = s <= nb && ed[s] - mjj <= band;
+            if (near_lo || near_hi) mjj = pair_mass_f64(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
         }
     }
     const long long o = (long long)v * P.n_events + ev;
-    if (P.out_njet) P.out_njet[o] = cnt;
-    if (P.out_argmax) P.out_argmax[o] = i1;
-    if (P.out_ht) P.out_ht[o] = sum;
-    if (P.out_maxpt) P.out_maxpt[o] = b1;
-    if (P.out_minpt) P.out_minpt[o] = mn;
-    if (P.out_mjj) P.out_mjj[o] = mjj;
-    if (P.out_subpt) P.out_subpt[o] = subpt;
+    if (feat & F_NJET) P.out_njet[o] = cnt;
+    if (feat & F_ARGMAX) P.out_argmax[o] = i1;
+    if (feat & F_HT) P.out_ht[o] = sum;
+    if (feat & F_MAXPT) P.out_maxpt[o] = b1;
+    if (feat & F_MINPT) P.out_minpt[o] = mn;
+    if (feat & F_MJJ) P.out_mjj[o] = mjj;
+    if (feat & F_SUBPT) P.out_subpt[o] = subpt;
     if (!hists) return;
-    const float wt0 = (P.hist_acc && P.weights) ? __ldg(P.weights + ev) : 1.0f;
-    fill_obs<HEPK_OBS_NJET>(P, S, ev, v, obs_slot<HEPK_OBS_NJET>(P, S, (float)cnt), wt0);
-    fill_obs<HEPK_OBS_HT>(P, S, ev, v, obs_slot<HEPK_OBS_HT>(P, S, sum), wt0);
-    fill_obs<HEPK_OBS_MAXPT>(P, S, ev, v, obs_slot<HEPK_OBS_MAXPT>(P, S, b1), wt0);
-    fill_obs<HEPK_OBS_MINPT>(P, S, ev, v, obs_slot<HEPK_OBS_MINPT>(P, S, mn), wt0);
-    fill_obs<HEPK_OBS_MJJ>(P, S, ev, v, s_mjj, wt0);
-    fill_obs<HEPK_OBS_SUBPT>(P, S, ev, v, obs_slot<HEPK_OBS_SUBPT>(P, S, subpt), wt0);
+    const float wt0 = ((feat & (F_SUMW | F_WEIGHTS)) == (F_SUMW | F_WEIGHTS)) ? __ldg(P.weights + ev) : 1.0f;
+    fill_obs<HEPK_OBS_NJET>(P, S, feat, ev, v, (float)cnt, wt0);
+    fill_obs<HEPK_OBS_HT>(P, S, feat, ev, v, sum, wt0);
+    fill_obs<HEPK_OBS_MAXPT>(P, S, feat, ev, v, b1, wt0);
+    fill_obs<HEPK_OBS_MINPT>(P, S, feat, ev, v, mn, wt0);
+    fill_obs<HEPK_OBS_MJJ>(P, S, feat, ev, v, mjj, wt0);
+    fill_obs<HEPK_OBS_SUBPT>(P, S, feat, ev, v, subpt, wt0);
 }
 
 // Running per-event state of phase 2.
@@ -304,6 +349,32 @@ struct EventAcc {
         i1 = gt1 ? k : i1;
         b2 = gt1 ? b1 : (gt2 ? p : b2);
         b1 = gt1 ? p : b1;
+    }
+    // The same update for a jet that counts iff p > pt_min (p may be anything, NaN included, otherwise), written
+    // with predicated instructions: 3 compares, 1 convert and 9 predicated operations.
+    __device__ __forceinline__ void push_lean(float p, float pt_min, int k)
+    {
+        asm("{\n\t"
+            ".reg .pred ok, g1, g2;\n\t"
+            ".reg .f64 pd;\n\t"
+            ".reg .f32 pz;\n\t"
+            "setp.gt.f32 ok, %7, %8;\n\t"
+            "setp.gt.and.f32 g1, %7, %4, ok;\n\t"
+            "setp.gt.and.f32 g2, %7, %5, ok;\n\t"
+            "selp.f32 pz, %7, 0f00000000, ok;\n\t"
+            "cvt.f64.f32 pd, pz;\n\t"
+            "@ok add.s32 %0, %0, 1;\n\t"
+            "add.f64 %1, %1, pd;\n\t"
+            "@ok min.f32 %2, %2, %7;\n\t"
+            "@g2 mov.b32 %6, %9;\n\t"
+            "@g1 mov.b32 %6, %3;\n\t"
+            "@g1 mov.b32 %3, %9;\n\t"
+            "@g2 mov.f32 %5, %7;\n\t"
+            "@g1 mov.f32 %5, %4;\n\t"
+            "@g1 mov.f32 %4, %7;\n\t"
+            "}"
+            : "+r"(cnt), "+d"(sum), "+f"(mn), "+r"(i1), "+f"(b1), "+f"(b2), "+r"(i2)
+            : "f"(p), "f"(pt_min), "r"(k));
     }
 };
 
@@ -352,7 +423,7 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, const Chai
             e1 = P.jeta[x]; p1 = P.jphi[x]; m1 = P.jmass[x];
             e2 = P.jeta[y]; p2 = P.jphi[y]; m2 = P.jmass[y];
         }
-        finish_event(P, S, ev, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
+        finish_event(P, S, chain_features(P), ev, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
     }
 }
 
@@ -445,8 +516,8 @@ __device__ __forceinline__ bool issue_tile(const LaneCol& c, int lane, long long
     return true;
 }
 
-template <bool CALIB, bool HAS_EL>
-__global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ ChainParams P)
+template <bool CALIB, bool HAS_EL, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ ChainParams P)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     ChainShared S;
@@ -507,12 +578,14 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
     }
     __syncthreads();
 
-    // this warp's buffers
-    unsigned int* const sorder = (unsigned int*)(R + P.order_off);
-    float2* const slep = (float2*)(R + P.lep_off);
-    float* const scorr = (float*)(R + P.corr_off);
-    const uint32_t bucket_a = smem_u32(R + P.bucket_off);
+    // this warp's buffers (shared-memory byte addresses)
+    const uint32_t region_a = smem_u32(R);
+    const uint32_t order_a = region_a + (uint32_t)P.order_off;
+    const uint32_t lep_a = region_a + (uint32_t)P.lep_off;
+    const uint32_t corr_a = region_a + (uint32_t)P.corr_off;
+    const uint32_t bucket_a = region_a + (uint32_t)P.bucket_off;
     const int V = CALIB ? P.V : 1;
+    const unsigned feat = chain_features(P);
 
     const long long GW = (long long)gridDim.x * nwarp;
     long long tile = (long long)warp * gridDim.x + blockIdx.x;
@@ -526,7 +599,7 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
         long long lo, hi;
         load_bounds(P, col, tile, lo, hi);
         load_event_offsets<HAS_EL>(P, tile, lane, eo);
-        fit = issue_tile(col, lane, lo, hi, bar);
+        fit = P.n_col > 0 && issue_tile(col, lane, lo, hi, bar);
         cur_lo = lo;
     }
 
@@ -548,133 +621,149 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
         fit = false;
 
         if (staged) {
-            // ---- phase 0: one lane per event.  Offsets are in registers; the lepton columns are needed first.
+            // ---- phase 0: one lane per event.  Offsets are in registers.
             const int jb = __shfl_sync(0xffffffffu, eo.j0, 0);
             const int mb = __shfl_sync(0xffffffffu, eo.m0, 0);
             const int qb = __shfl_sync(0xffffffffu, eo.q0, 0);
             const int njt = __shfl_sync(0xffffffffu, eo.j1, ne - 1) - jb;
-            float* spt = (float*)(R + P.col_dst[0]) + ((jb + P.sh_add[0]) & 3);
-            const float* seta = (const float*)(R + P.col_dst[1]) + ((jb + P.sh_add[1]) & 3);
-            const float* sphi = (const float*)(R + P.col_dst[2]) + ((jb + P.sh_add[2]) & 3);
-            const float* smass = (const float*)(R + P.col_dst[3]) + ((jb + P.sh_add[3]) & 3);
+            // shared-memory byte addresses; the columns of one collection share alignment and sit STRIDE apart
+            const uint32_t a_jpt = region_a + (uint32_t)P.col_dst[0] + 4u * (unsigned)((jb + P.sh_add[0]) & 3);
+            const uint32_t a_mpt = region_a + (uint32_t)P.col_dst[4] + 4u * (unsigned)((mb + P.sh_add[4]) & 3);
+            const uint32_t a_ept = region_a + (uint32_t)P.col_dst[7] + 4u * (unsigned)((qb + P.sh_add[7]) & 3);
+            const uint32_t js = (uint32_t)P.col_stride[0], ms = (uint32_t)P.col_stride[1], es = (uint32_t)P.col_stride[2];
+            const uint32_t d_corr0 = corr_a - a_jpt;     // calibration factor of the jet whose pt sits at address x: x + d_corr0
             const bool live = lane < ne;
             const int kj0 = live ? eo.j0 - jb : 0, nj = live ? eo.j1 - eo.j0 : 0;
             const int km0 = eo.m0 - mb, nm = live ? eo.m1 - eo.m0 : 0;
             const int kq0 = eo.q0 - qb, nq = (HAS_EL && live) ? eo.q1 - eo.q0 : 0;
             const int l0 = live ? km0 + kq0 : 0;
-            mbar_wait(bar, parity);
-            parity ^= 1u;
-            int c = 0;
-            {
-                const float* lp = (const float*)(R + P.col_dst[4]) + ((mb + P.sh_add[4]) & 3) + km0;
-                const float* le = (const float*)(R + P.col_dst[5]) + ((mb + P.sh_add[5]) & 3) + km0;
-                const float* lf = (const float*)(R + P.col_dst[6]) + ((mb + P.sh_add[6]) & 3) + km0;
-                float2* out = slep + l0;
-#pragma unroll 1
-                for (int i = 0; i < nm; ++i)
-                    if (lp[i] > P.lep_pt_min) out[c++] = make_float2(le[i], lf[i]);
-            }
-            if (HAS_EL) {
-                const float* lp = (const float*)(R + P.col_dst[7]) + ((qb + P.sh_add[7]) & 3) + kq0;
-                const float* le = (const float*)(R + P.col_dst[8]) + ((qb + P.sh_add[8]) & 3) + kq0;
-                const float* lf = (const float*)(R + P.col_dst[9]) + ((qb + P.sh_add[9]) & 3) + kq0;
-                float2* out = slep + l0;
-#pragma unroll 1
-                for (int i = 0; i < nq; ++i)
-                    if (lp[i] > P.lep_pt_min) out[c++] = make_float2(le[i], lf[i]);
-            }
-            // bucket the event's jets by its number of selected leptons: position inside the bucket from a
-            // shared-memory counter (any order inside a bucket will do), bucket bases from the eight totals
+            const int c = nm + nq;          // every lepton gets a list entry; unselected ones can never match
+            // bucket the event's jets by its lepton count: position inside the bucket from a shared-memory
+            // counter (any order inside a bucket will do), bucket bases from the eight totals
             const int key = c < N_BUCKETS - 1 ? c : N_BUCKETS - 1;
             const uint32_t bk = bucket_a + (uint32_t)bsel * (4u * N_BUCKETS);
             int pos = 0;
             if (nj > 0) pos = (int)atom_add_shared_u32(bk + 4u * (unsigned)key, (unsigned)nj);
-            if (lane < N_BUCKETS) ((int*)(R + P.bucket_off))[(bsel ^ 1) * N_BUCKETS + lane] = 0;   // the other set, for the next tile
-            // an event with more selected leptons than the packed word can count: the whole tile goes the slow way
+            if (lane < N_BUCKETS) sts_u32(bucket_a + (uint32_t)(bsel ^ 1) * (4u * N_BUCKETS) + 4u * lane, 0u);   // other set, for the next tile
+            // an event with more leptons than the packed word can count: the whole tile goes the slow way
             staged = !__any_sync(0xffffffffu, c > MAX_LEP_EVENT);
-            __syncwarp();
+            mbar_wait(bar, parity);
+            parity ^= 1u;
             if (staged) {
-                const int4 t0 = ((const int4*)(R + P.bucket_off))[bsel * 2], t1 = ((const int4*)(R + P.bucket_off))[bsel * 2 + 1];
+                // combined (eta, phi) list of the event: muons then electrons; eta = +inf marks "not selected"
+                // (deta^2 = inf, so dR^2 = inf or NaN and the minimum below ignores it)
+                uint32_t out = lep_a + 8u * (unsigned)l0;      // (l0 <= MAX_LIST by the capacities)
+                {
+                    uint32_t a = a_mpt + 4u * (unsigned)km0;
+                    const uint32_t aend = a + 4u * (unsigned)nm;
+#pragma unroll 1
+                    for (; a != aend; a += 4, out += 8) {
+                        const float pt = lds_f32(a), eta = lds_f32(a + ms), phi = lds_f32(a + 2 * ms);
+                        sts_v2(out, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                    }
+                }
+                if (HAS_EL) {
+                    uint32_t a = a_ept + 4u * (unsigned)kq0;
+                    const uint32_t aend = a + 4u * (unsigned)nq;
+#pragma unroll 1
+                    for (; a != aend; a += 4, out += 8) {
+                        const float pt = lds_f32(a), eta = lds_f32(a + es), phi = lds_f32(a + 2 * es);
+                        sts_v2(out, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                    }
+                }
+                __syncwarp();       // bucket totals complete
+                const int4 t0 = lds_v4i(bk), t1 = lds_v4i(bk + 16);
                 int base = 0;
                 base += key > 0 ? t0.x : 0; base += key > 1 ? t0.y : 0; base += key > 2 ? t0.z : 0; base += key > 3 ? t0.w : 0;
                 base += key > 4 ? t1.x : 0; base += key > 5 ? t1.y : 0; base += key > 6 ? t1.z : 0;
                 {
-                    unsigned int word = (unsigned)kj0 | ((unsigned)l0 << 10) | ((unsigned)c << 21);
-                    unsigned int* op = sorder + base + pos;
+                    // per jet: byte offset in its column [10:0], byte offset [23:11] and byte length [31:24] of the list
+                    unsigned int word = (unsigned)(kj0 << 2) | ((unsigned)l0 << 14) | ((unsigned)c << 27);
+                    uint32_t a = order_a + 4u * (unsigned)(base + pos);
+                    const uint32_t aend = a + 4u * (unsigned)nj;
 #pragma unroll 1
-                    for (int k = 0; k < nj; ++k) op[k] = word + (unsigned)k;
+                    for (; a != aend; a += 4, word += 4) sts_u32(a, word);
                 }
                 __syncwarp();
 
                 // ---- phase 1: one lane per jet, in bucket order (neighbouring lanes: same lepton count)
-                const long long lj0 = cur_lo_jets(P, cur_lo, lane) - P.jbase;
+                const uint32_t aend1 = order_a + 4u * (unsigned)njt;
 #pragma unroll 1
-                for (int t = lane; t < njt; t += 32) {
-                    const unsigned int word = sorder[t];
-                    const int j = (int)(word & 1023u);
-                    const float2* L = slep + ((word >> 10) & 2047u);
-                    const int n = (int)(word >> 21);
-                    const float eta = seta[j], phi = sphi[j], pt = spt[j];
+                for (uint32_t ao = order_a + 4u * lane; ao < aend1; ao += 128) {
+                    const unsigned int word = lds_u32(ao);
+                    const uint32_t aj = a_jpt + (word & 0x7ffu);
+                    const float pt = lds_f32(aj), eta = lds_f32(aj + js), phi = lds_f32(aj + 2 * js);
+                    uint32_t al = lep_a + ((word >> 11) & 0x1fffu);
+                    const uint32_t alend = al + (word >> 24);
                     float dmin = CUDART_INF_F;
-#pragma unroll 1
-                    for (int i = 0; i < n; ++i) {
-                        const float2 l = L[i];
-                        dmin = fminf(dmin, dr2_min(eta, phi, l.x, l.y));
+                    if (word & (8u << 24)) {            // odd count: one lepton first, then pairs
+                        const float2 l = lds_v2(al);
+                        dmin = dr2_min(eta, phi, l.x, l.y);
+                        al += 8;
                     }
-                    const bool base = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
+#pragma unroll 1
+                    for (; al != alend; al += 16) {
+                        const float2 l = lds_v2(al), m = lds_v2(al + 8);
+                        dmin = fminf(dmin, fminf(dr2_min(eta, phi, l.x, l.y), dr2_min(eta, phi, m.x, m.y)));
+                    }
+                    const bool base_ok = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
                     if (!CALIB) {
-                        const bool clean = base && (pt > P.jet_pt_min);
-                        if (P.out_jet_mask) P.out_jet_mask[lj0 + j] = clean ? 1 : 0;
-                        spt[j] = clean ? pt : -CUDART_INF_F;
+                        sts_f32(aj, (base_ok && (pt > P.jet_pt_min)) ? pt : -CUDART_INF_F);
                     } else {
                         const int bx = find_bin_clamped(pt, S.cal_pt_edges, P.cal_npt);
                         const int by = find_bin_clamped(eta, S.cal_eta_edges, P.cal_neta);
-                        const float cf = S.cal_table[bx * P.cal_neta + by];
-                        scorr[j] = cf;
-                        if (!base) spt[j] = CUDART_NAN_F;
-                        if (P.out_jet_mask)
-                            for (int v = 0; v < V; ++v)
-                                P.out_jet_mask[(long long)v * P.jn + lj0 + j] =
-                                    (base && (__fmul_rn(pt, __fmul_rn(cf, P.scales[v])) > P.jet_pt_min)) ? 1 : 0;
+                        sts_f32(aj + d_corr0, S.cal_table[bx * P.cal_neta + by]);
+                        if (!base_ok) sts_f32(aj, CUDART_NAN_F);
                     }
                 }
                 __syncwarp();
+                if (P.out_jet_mask) {
+                    // clean-jet mask, jets in their original order (coalesced bytes), from the verdicts just stored
+                    const long long lj0 = cur_lo_jets(P, cur_lo, lane) - P.jbase;
+                    for (int j = lane; j < njt; j += 32) {
+                        const float p = lds_f32(a_jpt + 4u * (unsigned)j);
+                        if (!CALIB) {
+                            P.out_jet_mask[lj0 + j] = (p > -CUDART_INF_F) ? 1 : 0;
+                        } else {
+                            const float cf = lds_f32(a_jpt + d_corr0 + 4u * (unsigned)j);
+                            for (int v = 0; v < V; ++v)      // p is NaN when the jet failed eta / dR
+                                P.out_jet_mask[(long long)v * P.jn + lj0 + j] =
+                                    (__fmul_rn(p, __fmul_rn(cf, P.scales[v])) > P.jet_pt_min) ? 1 : 0;
+                        }
+                    }
+                }
 
                 // ---- phase 2: one lane per event (lanes past the last event run with nj = 0)
-                const float* pp = spt + kj0;
-                const float* cc = scorr + kj0;
+                const uint32_t a_ev = a_jpt + 4u * (unsigned)kj0;
+                const uint32_t d_corr = d_corr0;
                 for (int v = 0; v < V; ++v) {
                     const float sv = P.scales[v];
                     EventAcc a;
                     a.init();
+                    {
+                        uint32_t ap = a_ev;
 #pragma unroll 1
-                    for (int k = 0; k < nj; ++k) {
-                        float p = pp[k];
-                        bool ok;
-                        if (CALIB) {
-                            p = __fmul_rn(p, __fmul_rn(cc[k], sv));     // NaN when the jet failed eta / dR
-                            ok = p > P.jet_pt_min;
-                            p = ok ? p : -CUDART_INF_F;
-                        } else {
-                            ok = p > P.jet_pt_min;                      // -inf when not clean
+                        for (int k = 0; k != nj; ++k, ap += 4) {
+                            float p = lds_f32(ap);
+                            if (CALIB) p = __fmul_rn(p, __fmul_rn(lds_f32(ap + d_corr), sv));     // NaN when the jet failed eta / dR
+                            a.push_lean(p, P.jet_pt_min, k);
                         }
-                        a.push(p, ok, k);
                     }
                     float e1 = 0, p1 = 0, m1 = 0, e2 = 0, p2 = 0, m2 = 0;
                     if (a.i2 >= 0) {
-                        const int x = kj0 + a.i1, y = kj0 + a.i2;
-                        e1 = seta[x]; p1 = sphi[x]; m1 = smass[x];
-                        e2 = seta[y]; p2 = sphi[y]; m2 = smass[y];
+                        const uint32_t x = a_ev + 4u * (unsigned)a.i1, y = a_ev + 4u * (unsigned)a.i2;
+                        e1 = lds_f32(x + js); p1 = lds_f32(x + 2 * js); m1 = lds_f32(x + 3 * js);
+                        e2 = lds_f32(y + js); p2 = lds_f32(y + 2 * js); m2 = lds_f32(y + 3 * js);
                     }
                     if (v == V - 1) {
                         // the staging region is dead from here: start the next tile's copies under the finishing math
                         fence_proxy_async_smem();
                         __syncwarp();
-                        if (has_next) fit = issue_tile(col, lane, nlo, nhi, bar);
+                        if (has_next && P.n_col > 0) fit = issue_tile(col, lane, nlo, nhi, bar);
                         released = true;
                     }
                     if (live)
-                        finish_event(P, S, e0 + lane, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
+                        finish_event(P, S, feat, e0 + lane, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
                 }
             }
             bsel ^= 1;
@@ -682,7 +771,7 @@ __global__ void __launch_bounds__(512, 1) chain_kernel(const __grid_constant__ C
         if (!released) {
             fence_proxy_async_smem();
             __syncwarp();
-            if (has_next) fit = issue_tile(col, lane, nlo, nhi, bar);
+            if (has_next && P.n_col > 0) fit = issue_tile(col, lane, nlo, nhi, bar);
         }
         if (!staged && lane < ne) chain_event_global<CALIB>(P, S, e0 + lane);
         __syncwarp();
@@ -765,7 +854,11 @@ static int chain_region_layout(ChainParams& P, const hepk_chain_desc* d, bool ca
         const long long b = coll[k]->content_base % 4;
         P.sh_add[c] = (int)(((P.col_mis[c] - b) % 4 + 4) % 4);
     }
-    P.order_off = take((size_t)cap_j * 4);
+    P.col_stride[0] = (cap_j + 8) * 4; P.col_stride[1] = (cap_m + 8) * 4; P.col_stride[2] = (cap_e + 8) * 4;
+    // the jet permutation overlays the lepton column buffers: they are dead once the lepton list is built, and
+    // the permutation is written after that and read until the region is released
+    P.order_off = P.col_dst[4];
+    if (o < (size_t)P.order_off + (size_t)cap_j * 4) o = (size_t)P.order_off + (size_t)cap_j * 4;
     P.lep_off = take((size_t)(cap_m + cap_e) * 8);
     P.corr_off = take(calib ? (size_t)cap_j * 4 : 0);
     P.bucket_off = take(2 * N_BUCKETS * 4);
@@ -809,12 +902,12 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     P.hist_acc = want_sumw ? (double*)workspace : nullptr;
     P.hist_counts = want_cnt ? (unsigned long long*)d->hist_counts : nullptr;
 
-    // staging capacities per 32-event tile from the mean multiplicities: mean + ~5 sigma of a Poisson-like
+    // staging capacities per 32-event tile from the mean multiplicities: mean + ~4 sigma of a Poisson-like
     // tile total (a tile that does not fit takes the per-event path)
     const double nev = (double)(d->n_events > 0 ? d->n_events : 1);
     auto cap_for = [&](double mean, int floor_) {
         const double t = TILE_EVENTS * mean;
-        long long c = (long long)(t + 5.0 * sqrt(2.0 * t + 1.0)) + 16;
+        long long c = (long long)(t + 4.0 * sqrt(2.0 * t + 1.0)) + 8;
         return c < floor_ ? floor_ : (int)c;
     };
     int cap_j = round_up4(d->tune_cap_jets > 0 ? d->tune_cap_jets : cap_for((double)d->jets.n_objects / nev, 64));
@@ -822,11 +915,11 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     int cap_e = has_el ? round_up4(d->tune_cap_leptons > 0 ? d->tune_cap_leptons
                                                               : cap_for((double)d->electrons.n_objects / nev, 32)) : 0;
     if (cap_j < 16) cap_j = 16;
-    if (cap_j > MAX_JETS_TILE) cap_j = MAX_JETS_TILE;      // the jet index is packed in 10 bits
+    if (cap_j > MAX_JETS_TILE) cap_j = MAX_JETS_TILE;      // the jet's byte offset is packed in 11 bits
     if (cap_m < 4) cap_m = 4;
     if (has_el && cap_e < 4) cap_e = 4;
-    if (cap_m > MAX_LIST / 2 - 4) cap_m = MAX_LIST / 2 - 4;      // the list start is packed in 11 bits
-    if (cap_e > MAX_LIST / 2 - 4) cap_e = MAX_LIST / 2 - 4;
+    if (cap_m > 508) cap_m = 508;        // the list start (in bytes) is packed in 13 bits
+    if (cap_e > 508) cap_e = 508;        // 2 * 508 <= MAX_LIST, multiple of 4
 
     const int smem_max = max_smem_optin();
     const int shared_bytes = (int)dev::chain_shared_layout(P, calib, nullptr, nullptr);
@@ -850,19 +943,25 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     }
     P.shared_bytes = shared_bytes;
     P.region_bytes = region;
+    // the kernel addresses the columns of a collection at a fixed stride from the first one, which needs them to
+    // share their alignment modulo 16 bytes; otherwise every tile takes the per-event path
     P.n_col = NCOL;
+    for (int c = 0; c < NCOL; ++c) {
+        const int first = P.col_coll[c] == 0 ? 0 : (P.col_coll[c] == 1 ? 4 : 7);
+        if (P.col_ptr[c] && P.col_ptr[first] && P.col_mis[c] != P.col_mis[first]) P.n_col = 0;
+    }
 
     // CTA shape: as many warps per SM as shared memory allows (up to 16), in as few CTAs as possible so that
     // the privatised histograms are shared by many warps
     const int sm_total = smem_max + 1024;              // per SM; each CTA also pays 1 KB of system shared memory
     int best_ctas = 1, best_wpc = 1, best_total = 0;
-    const int max_warps_sm = 16;
+    const int max_warps_sm = d->tune_warps_per_sm > 0 ? d->tune_warps_per_sm : 16;
     for (int ctas = 1; ctas <= 4; ++ctas) {
         if (d->tune_ctas_per_sm > 0 && ctas != d->tune_ctas_per_sm && !(ctas == 1 && d->tune_ctas_per_sm > 4)) continue;
         int budget = sm_total / ctas - 1024;
         if (budget > smem_max) budget = smem_max;
         int wpc = (budget - shared_bytes) / region;
-        if (wpc > 16) wpc = 16;
+        if (wpc > 24) wpc = 24;
         if (wpc * ctas > max_warps_sm) wpc = max_warps_sm / ctas;
         if (d->tune_warps_per_cta > 0 && wpc > d->tune_warps_per_cta) wpc = d->tune_warps_per_cta;
         if (wpc < 1) continue;
@@ -872,9 +971,15 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     const size_t smem = (size_t)shared_bytes + (size_t)wpc * region;
     P.flush_tiles = 4096 / (TILE_EVENTS * wpc) > 0 ? 4096 / (TILE_EVENTS * wpc) : 1;
 
+    // two register budgets: up to 16 warps per CTA (128 registers per thread) or up to 24 (85)
     void (*kern)(ChainParams);
-    if (calib) kern = has_el ? dev::chain_kernel<true, true> : dev::chain_kernel<true, false>;
-    else kern = has_el ? dev::chain_kernel<false, true> : dev::chain_kernel<false, false>;
+    if (wpc <= 16) {
+        if (calib) kern = has_el ? dev::chain_kernel<true, true, 512> : dev::chain_kernel<true, false, 512>;
+        else kern = has_el ? dev::chain_kernel<false, true, 512> : dev::chain_kernel<false, false, 512>;
+    } else {
+        if (calib) kern = has_el ? dev::chain_kernel<true, true, 768> : dev::chain_kernel<true, false, 768>;
+        else kern = has_el ? dev::chain_kernel<false, true, 768> : dev::chain_kernel<false, false, 768>;
+    }
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
     HEPK_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, wpc * 32, smem));
