@@ -701,10 +701,16 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         dmin = dr2_min(eta, phi, l.x, l.y);
                         al += 8;
                     }
+                    {
+                        // pairs, the next pair loaded ahead (over-read at the end stays inside the list buffer's slack)
+                        float2 l = lds_v2(al), m = lds_v2(al + 8);
 #pragma unroll 1
-                    for (; al != alend; al += 16) {
-                        const float2 l = lds_v2(al), m = lds_v2(al + 8);
-                        dmin = fminf(dmin, fminf(dr2_min(eta, phi, l.x, l.y), dr2_min(eta, phi, m.x, m.y)));
+                        for (; al != alend;) {
+                            const float2 l0_ = l, m0_ = m;
+                            al += 16;
+                            l = lds_v2(al); m = lds_v2(al + 8);
+                            dmin = fminf(dmin, fminf(dr2_min(eta, phi, l0_.x, l0_.y), dr2_min(eta, phi, m0_.x, m0_.y)));
+                        }
                     }
                     const bool base_ok = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
                     if (!CALIB) {
@@ -741,11 +747,17 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     EventAcc a;
                     a.init();
                     {
+                        // the next jet is loaded before the current one is folded in (one element of over-read
+                        // at the end stays inside the staging buffer's slack)
                         uint32_t ap = a_ev;
+                        float pn = lds_f32(ap), cn = CALIB ? lds_f32(ap + d_corr) : 1.0f;
 #pragma unroll 1
-                        for (int k = 0; k != nj; ++k, ap += 4) {
-                            float p = lds_f32(ap);
-                            if (CALIB) p = __fmul_rn(p, __fmul_rn(lds_f32(ap + d_corr), sv));     // NaN when the jet failed eta / dR
+                        for (int k = 0; k != nj; ++k) {
+                            float p = pn;
+                            if (CALIB) p = __fmul_rn(p, __fmul_rn(cn, sv));     // NaN when the jet failed eta / dR
+                            ap += 4;
+                            pn = lds_f32(ap);
+                            if (CALIB) cn = lds_f32(ap + d_corr);
                             a.push_lean(p, P.jet_pt_min, k);
                         }
                     }
@@ -859,8 +871,8 @@ static int chain_region_layout(ChainParams& P, const hepk_chain_desc* d, bool ca
     // the permutation is written after that and read until the region is released
     P.order_off = P.col_dst[4];
     if (o < (size_t)P.order_off + (size_t)cap_j * 4) o = (size_t)P.order_off + (size_t)cap_j * 4;
-    P.lep_off = take((size_t)(cap_m + cap_e) * 8);
-    P.corr_off = take(calib ? (size_t)cap_j * 4 : 0);
+    P.lep_off = take((size_t)(cap_m + cap_e + 4) * 8);
+    P.corr_off = take(calib ? (size_t)(cap_j + 8) * 4 : 0);
     P.bucket_off = take(2 * N_BUCKETS * 4);
     return (int)dev::align_up(o, 128);
 }
@@ -971,15 +983,15 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     const size_t smem = (size_t)shared_bytes + (size_t)wpc * region;
     P.flush_tiles = 4096 / (TILE_EVENTS * wpc) > 0 ? 4096 / (TILE_EVENTS * wpc) : 1;
 
-    // two register budgets: up to 16 warps per CTA (128 registers per thread) or up to 24 (85)
+    // three register budgets: up to 16 warps per CTA (128 registers per thread), 20 (102) or 24 (85)
     void (*kern)(ChainParams);
-    if (wpc <= 16) {
-        if (calib) kern = has_el ? dev::chain_kernel<true, true, 512> : dev::chain_kernel<true, false, 512>;
-        else kern = has_el ? dev::chain_kernel<false, true, 512> : dev::chain_kernel<false, false, 512>;
-    } else {
-        if (calib) kern = has_el ? dev::chain_kernel<true, true, 768> : dev::chain_kernel<true, false, 768>;
-        else kern = has_el ? dev::chain_kernel<false, true, 768> : dev::chain_kernel<false, false, 768>;
-    }
+#define HEPK_PICK(MAXT)                                                                                              \
+    (calib ? (has_el ? dev::chain_kernel<true, true, MAXT> : dev::chain_kernel<true, false, MAXT>)                 \
+           : (has_el ? dev::chain_kernel<false, true, MAXT> : dev::chain_kernel<false, false, MAXT>))
+    if (wpc <= 16) kern = HEPK_PICK(512);
+    else if (wpc <= 20) kern = HEPK_PICK(640);
+    else kern = HEPK_PICK(768);
+#undef HEPK_PICK
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
     HEPK_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, wpc * 32, smem));
