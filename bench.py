@@ -249,10 +249,13 @@ def run_hepk(args):
     per_launch_ms = kern_ms / max(kern_n, 1)
     achieved = alg_bytes / (per_launch_ms * 1e-3) / 1e9
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")      # written by hand from the ncu --set full capture
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")       # copied by hand from the ncu --set full capture
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(f"config{args.config}")
+            import csv
+            for row in csv.DictReader(open(tp)):
+                if int(row["config"]) == args.config:
+                    traffic = int(row["dram_bytes_per_launch"])
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
