@@ -178,7 +178,7 @@ def run_hepk(args):
     import torch.distributed as dist
 
     import hepgen
-    from paper_1906_06242_b200 import binding as hk
+    from paper_1906_06242_b200 import binding as hk, sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -206,8 +206,7 @@ def run_hepk(args):
             plan.zero_hists()
         plan.run()
         if world > 1:                      # the one exchange step of the path: histogram merge
-            for t in hist_t:
-                dist.all_reduce(t)
+            sharding.merge_histograms(hist_t)
 
     def barrier():
         if world > 1:
