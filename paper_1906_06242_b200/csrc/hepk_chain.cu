@@ -71,7 +71,8 @@ struct ChainParams {
     unsigned long long* hist_counts;     // [V][active o][nbins_o+2], or nullptr
     int order_off, lep_off, corr_off, bucket_off;   // byte offsets inside a warp's region
     int region_bytes, shared_bytes;      // per-warp region; CTA-shared part in front of the regions
-    int flush_tiles;                     // warp 0 of a CTA flushes the histograms every this many of its tiles
+    int flush_events;                    // a CTA flushes its histograms to the global accumulators every this many events
+    const unsigned int* wmax_bits;       // [0] bits of max |weight| over the launch, [1] != 0: a weight is not finite
 };
 
 namespace dev {
@@ -80,8 +81,10 @@ namespace dev {
 struct ChainShared {
     float *edges, *axis_lo, *axis_inv;   // axis_inv == 0: the axis is not uniform enough for the arithmetic bin guess
     float *cal_pt_edges, *cal_eta_edges, *cal_table;
-    float* h_sumw;
+    float* h_sumw;                       // int32 fixed point (w * 2^k) when wscale[0] != 0, else float
     unsigned int* h_cnt;
+    float* wscale;                       // [0] 2^k or 0, [1] 2^-k
+    unsigned int* since;                 // events filled since the last flush
 };
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -101,6 +104,8 @@ __host__ __device__ inline size_t chain_shared_layout(const ChainParams& P, bool
     const size_t spv = (size_t)P.obs_prefix[HEPK_N_OBS];
     r = take(P.hist_acc ? spv * P.V * P.W * 4 : 0, 4); if (s) s->h_sumw = (float*)(base + r);
     r = take(P.hist_counts ? spv * P.V * 4 : 0, 4); if (s) s->h_cnt = (unsigned int*)(base + r);
+    r = take(8, 4); if (s) s->wscale = (float*)(base + r);
+    r = take(4, 4); if (s) s->since = (unsigned int*)(base + r);
     return align_up(o, 128);
 }
 
@@ -114,6 +119,10 @@ __device__ __forceinline__ unsigned int atom_add_shared_u32(uint32_t addr, unsig
 __device__ __forceinline__ void red_add_shared_u32(uint32_t addr, unsigned int v)
 {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_add_shared_s32(uint32_t addr, int v)
+{
+    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 __device__ __forceinline__ void red_add_shared_f32(uint32_t addr, float v)
 {
@@ -270,24 +279,31 @@ __device__ __forceinline__ unsigned chain_features(const ChainParams& P)
     return f;
 }
 
-// One observable of one event and variant into the privatised histograms (`wt0` = weight column 0).
+// Slot of one observable: bumps its count and returns the shared-memory address of its bin in weight column 0
+// (0 when the observable is not histogrammed).  sumw layout [v][o][w][nbins_o + 2].
 template <int OB>
-__device__ __forceinline__ void fill_obs(const ChainParams& P, const ChainShared& S, unsigned feat, long long ev, int v, float x, float wt0)
+__device__ __forceinline__ uint32_t obs_bin(const ChainParams& P, const ChainShared& S, unsigned feat, int v, float x)
 {
-    if (!(feat & (F_OBS0 << OB))) return;
+    if (!(feat & (F_OBS0 << OB))) return 0u;
     const int nb = P.axis_nbins[OB];
     const int slot = slot_lean(x, S.edges + P.edge_prefix[OB], nb, S.axis_lo[OB], S.axis_inv[OB]);
     const int spv = P.obs_prefix[HEPK_N_OBS], pre = P.obs_prefix[OB];
     if (feat & F_COUNTS) red_add_shared_u32(smem_u32(S.h_cnt) + 4u * (unsigned)(v * spv + pre + slot), 1u);
-    if (feat & F_SUMW) {
-        // sumw layout [v][o][w][nbins_o + 2]
-        uint32_t a = smem_u32(S.h_sumw) + 4u * (unsigned)((v * spv + pre) * P.W + slot);
-        red_add_shared_f32(a, wt0);
-        const unsigned stride = 4u * (unsigned)(nb + 2);
-        for (int w = 1; w < P.W; ++w) {
-            a += stride;
-            red_add_shared_f32(a, __ldg(P.weights + (long long)w * P.n_events + ev));
-        }
+    return smem_u32(S.h_sumw) + 4u * (unsigned)((v * spv + pre) * P.W + slot);
+}
+
+// One weight into the bins of the active observables.  Fixed point (wscale != 0): the weight is rounded once to
+// a multiple of 2^-k and added with the native integer shared-memory atomic; else float (a compare-and-swap loop).
+__device__ __forceinline__ void add_weight(const ChainParams& P, unsigned feat, const uint32_t (&bin)[HEPK_N_OBS], int w,
+                                           float wt, float wscale)
+{
+    const int q = __float2int_rn(wt * wscale);
+#pragma unroll
+    for (int ob = 0; ob < HEPK_N_OBS; ++ob) {
+        if (!(feat & (F_OBS0 << ob))) continue;
+        const uint32_t a = bin[ob] + 4u * (unsigned)(w * (P.axis_nbins[ob] + 2));
+        if (wscale != 0.0f) red_add_shared_s32(a, q);
+        else red_add_shared_f32(a, wt);
     }
 }
 
@@ -322,13 +338,18 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     if (feat & F_MJJ) P.out_mjj[o] = mjj;
     if (feat & F_SUBPT) P.out_subpt[o] = subpt;
     if (!hists) return;
-    const float wt0 = ((feat & (F_SUMW | F_WEIGHTS)) == (F_SUMW | F_WEIGHTS)) ? __ldg(P.weights + ev) : 1.0f;
-    fill_obs<HEPK_OBS_NJET>(P, S, feat, ev, v, (float)cnt, wt0);
-    fill_obs<HEPK_OBS_HT>(P, S, feat, ev, v, sum, wt0);
-    fill_obs<HEPK_OBS_MAXPT>(P, S, feat, ev, v, b1, wt0);
-    fill_obs<HEPK_OBS_MINPT>(P, S, feat, ev, v, mn, wt0);
-    fill_obs<HEPK_OBS_MJJ>(P, S, feat, ev, v, mjj, wt0);
-    fill_obs<HEPK_OBS_SUBPT>(P, S, feat, ev, v, subpt, wt0);
+    uint32_t bin[HEPK_N_OBS];
+    bin[HEPK_OBS_NJET] = obs_bin<HEPK_OBS_NJET>(P, S, feat, v, (float)cnt);
+    bin[HEPK_OBS_HT] = obs_bin<HEPK_OBS_HT>(P, S, feat, v, sum);
+    bin[HEPK_OBS_MAXPT] = obs_bin<HEPK_OBS_MAXPT>(P, S, feat, v, b1);
+    bin[HEPK_OBS_MINPT] = obs_bin<HEPK_OBS_MINPT>(P, S, feat, v, mn);
+    bin[HEPK_OBS_MJJ] = obs_bin<HEPK_OBS_MJJ>(P, S, feat, v, mjj);
+    bin[HEPK_OBS_SUBPT] = obs_bin<HEPK_OBS_SUBPT>(P, S, feat, v, subpt);
+    if (!(feat & F_SUMW)) return;
+    const float wscale = S.wscale[0];
+    if (!(feat & F_WEIGHTS)) { add_weight(P, feat, bin, 0, 1.0f, wscale); return; }
+    add_weight(P, feat, bin, 0, __ldg(P.weights + ev), wscale);
+    for (int w = 1; w < P.W; ++w) add_weight(P, feat, bin, w, __ldg(P.weights + (long long)w * P.n_events + ev), wscale);
 }
 
 // Running per-event state of phase 2.
@@ -434,10 +455,18 @@ __device__ __forceinline__ void flush_hist(const ChainParams& P, const ChainShar
     const int spv = P.obs_prefix[HEPK_N_OBS];
     if (P.hist_acc) {
         const int n = spv * P.V * P.W;
+        const bool fixed = S.wscale[0] != 0.0f;
+        const double inv = (double)S.wscale[1];
+        int* hi = (int*)S.h_sumw;
         for (int i = t; i < n; i += nt) {
-            if (S.h_sumw[i] == 0.0f) continue;
-            const float x = atomicExch(S.h_sumw + i, 0.0f);
-            if (x != 0.0f) atomicAdd(P.hist_acc + i, (double)x);
+            if (hi[i] == 0) continue;          // +0.0f and integer 0 share the bit pattern
+            if (fixed) {
+                const int x = atomicExch(hi + i, 0);
+                if (x) atomicAdd(P.hist_acc + i, (double)x * inv);
+            } else {
+                const float x = atomicExch(S.h_sumw + i, 0.0f);
+                if (x != 0.0f) atomicAdd(P.hist_acc + i, (double)x);
+            }
         }
     }
     if (P.hist_counts) {
@@ -548,6 +577,21 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         const int spv = P.obs_prefix[HEPK_N_OBS];
         if (P.hist_acc) for (int i = tid; i < spv * P.V * P.W; i += nthr) S.h_sumw[i] = 0.0f;
         if (P.hist_counts) for (int i = tid; i < spv * P.V; i += nthr) S.h_cnt[i] = 0u;
+        if (tid == 0) {
+            // fixed-point scale of the weighted bins: 4 * flush_events entries of max |w| * 2^k stay below 2^31
+            float sc = 0.0f, inv = 0.0f;
+            if (P.wmax_bits && P.wmax_bits[1] == 0u) {
+                const float wm = __uint_as_float(P.wmax_bits[0]);
+                if (wm > 0.0f && wm < CUDART_INF_F) {
+                    int e;
+                    frexpf(wm, &e);                                    // wm < 2^e
+                    const int k = 29 - (31 - __clz(P.flush_events)) - e;   // flush_events is a power of two
+                    if (k > -100 && k < 100) { sc = ldexpf(1.0f, k); inv = ldexpf(1.0f, -k); }
+                }
+            }
+            S.wscale[0] = sc; S.wscale[1] = inv;
+            *S.since = 0u;
+        }
     }
     __syncthreads();
     // per axis: is the arithmetic bin guess of slot_lean safe?  (|(edges[i] - lo) * inv - i| <= 0.5 for every edge)
@@ -590,7 +634,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     const long long GW = (long long)gridDim.x * nwarp;
     long long tile = (long long)warp * gridDim.x + blockIdx.x;
     uint32_t parity = 0;
-    int since_flush = 0, bsel = 0;
+    int bsel = 0;
     bool fit = false;
     long long cur_lo = 0;
     EventOffsets eo;
@@ -790,13 +834,35 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         eo = neo;
         cur_lo = nlo;
 
-        if (warp == 0 && ++since_flush >= P.flush_tiles) {
-            flush_hist(P, S, lane, 32);
-            since_flush = 0;
+        {   // the warp whose tile takes the CTA's event count across a multiple of flush_events flushes the histograms
+            unsigned int c = 0;
+            if (lane == 0) c = atomicAdd(S.since, (unsigned)ne);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if ((c & ~(unsigned)(P.flush_events - 1)) != ((c + (unsigned)ne) & ~(unsigned)(P.flush_events - 1))) flush_hist(P, S, lane, 32);
         }
     }
     __syncthreads();
     flush_hist(P, S, tid, nthr);
+}
+
+// max |w| over the launch's weights (bits of a non-negative float order like unsigned integers) and a flag for
+// non-finite weights; out[0..1] zeroed by the caller.  w == nullptr: every weight is 1.
+__global__ void chain_wmax_kernel(const float* __restrict__ w, long long n, unsigned int* __restrict__ out)
+{
+    if (!w) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) out[0] = __float_as_uint(1.0f);
+        return;
+    }
+    float m = 0.0f;
+    bool bad = false;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float a = fabsf(w[i]);
+        bad = bad || !(a < CUDART_INF_F);
+        m = fmaxf(m, a);
+    }
+    const unsigned int b = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(out + 1, 1u);
+    if ((threadIdx.x & 31) == 0 && b) atomicMax(out, b);
 }
 
 // sumw[i] = float32(float64(sumw[i]) + acc[i])
@@ -981,7 +1047,8 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     }
     const int wpc = best_wpc;
     const size_t smem = (size_t)shared_bytes + (size_t)wpc * region;
-    P.flush_tiles = 4096 / (TILE_EVENTS * wpc) > 0 ? 4096 / (TILE_EVENTS * wpc) : 1;
+    P.flush_events = 1024;
+    P.wmax_bits = want_sumw ? (const unsigned int*)((const double*)workspace + n_sumw) : nullptr;
 
     // three register budgets: up to 16 warps per CTA (128 registers per thread), 20 (102) or 24 (85)
     void (*kern)(ChainParams);
@@ -1002,7 +1069,15 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (grid > need) grid = need;
     if (grid < 1) grid = 1;
 
-    if (want_sumw) HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)n_sumw * sizeof(double), st));
+    if (want_sumw) {
+        HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)n_sumw * sizeof(double) + 16, st));
+        const long long nw = (long long)P.W * P.n_events;
+        long long blocks = (nw + 256 * 8 - 1) / (256 * 8);
+        if (blocks > 4 * sm_count()) blocks = 4 * sm_count();
+        if (blocks < 1) blocks = 1;
+        dev::chain_wmax_kernel<<<(unsigned)blocks, 256, 0, st>>>(d->weights, nw, (unsigned int*)((double*)workspace + n_sumw));
+        HEPK_CUDA_TRY(cudaGetLastError());
+    }
     profile_mark(st, 0);
     kern<<<(unsigned)grid, wpc * 32, smem, st>>>(P);
     profile_mark(st, 1);
@@ -1020,7 +1095,7 @@ extern "C" size_t hepk_chain_workspace_bytes(const hepk_chain_desc* d)
 {
     if (!d || d->n_variants < 1 || d->n_wvar < 1) return 0;
     const long long n = hepk::hist_slots_per_variant(d) * d->n_variants * d->n_wvar;
-    return (size_t)(n > 0 ? n : 1) * sizeof(double);
+    return (size_t)(n > 0 ? n : 1) * sizeof(double) + 16;      // float64 accumulators + max |weight| slot
 }
 
 extern "C" int32_t hepk_analysis_chain(const hepk_chain_desc* d, void* workspace, size_t workspace_bytes, void* stream)

@@ -81,7 +81,7 @@ static bool make_plan(const hepk_chain_desc* d, long long B, HostPlan* p)
     s.out_mask = take(d->out_jet_mask ? (size_t)V * p->maxJ : 0);
     s.hist_sumw = take((size_t)p->n_sumw * 4);
     s.hist_counts = take((size_t)p->n_cnt * 8);
-    s.chain_ws = take((size_t)(p->n_sumw > 0 ? p->n_sumw : 1) * 8);
+    s.chain_ws = take((size_t)(p->n_sumw > 0 ? p->n_sumw : 1) * 8 + 16);
     s.bytes = o;
     return true;
 }
@@ -205,7 +205,7 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
         bd.hist_sumw = p.n_sumw ? (float*)(sb + p.slot.hist_sumw) : nullptr;
         bd.hist_counts = p.n_cnt ? (int64_t*)(sb + p.slot.hist_counts) : nullptr;
 
-        const int32_t rc = hepk_analysis_chain(&bd, sb + p.slot.chain_ws, (size_t)(p.n_sumw > 0 ? p.n_sumw : 1) * 8, q);
+        const int32_t rc = hepk_analysis_chain(&bd, sb + p.slot.chain_ws, (size_t)(p.n_sumw > 0 ? p.n_sumw : 1) * 8 + 16, q);
         if (rc != HEPK_OK) return rc;
 
         for (int v = 0; v < V; ++v) {
