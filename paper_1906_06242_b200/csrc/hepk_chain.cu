@@ -33,6 +33,7 @@ constexpr int NCOL = 10;            // staged columns: 0-3 jets pt,eta,phi,mass;
 constexpr int MAX_JETS_TILE = 512;  // byte offset of a jet inside a tile column (4 * index) fits 11 bits
 constexpr int MAX_LIST = 1023;      // byte offset of an event's lepton list (8 * start) fits 13 bits
 constexpr int MAX_LEP_EVENT = 31;   // byte length of an event's lepton list (8 * count) fits 8 bits
+constexpr int TAIL_CUT = 16;        // jets of an event beyond this many are handled by the whole warp, not by the event's lane
 constexpr int N_BUCKETS = 8;        // jets are ordered by min(selected leptons of their event, 7)
 
 struct ChainParams {
@@ -352,6 +353,17 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     for (int w = 1; w < P.W; ++w) add_weight(P, feat, bin, w, __ldg(P.weights + (long long)w * P.n_events + ev), wscale);
 }
 
+// Order-preserving map float -> unsigned (and back): a < b  <=>  ord_key(a) < ord_key(b); no finite value maps to 0.
+__device__ __forceinline__ unsigned int ord_key(float f)
+{
+    const unsigned int b = __float_as_uint(f);
+    return b ^ ((unsigned int)((int)b >> 31) | 0x80000000u);
+}
+__device__ __forceinline__ float ord_value(unsigned int u)
+{
+    return __uint_as_float(u ^ ((u & 0x80000000u) ? 0x80000000u : 0xffffffffu));
+}
+
 // Running per-event state of phase 2.
 struct EventAcc {
     int cnt, i1, i2;
@@ -365,6 +377,15 @@ struct EventAcc {
         if (ok) sum += (double)p;
         mn = fminf(mn, ok ? p : CUDART_INF_F);
         // top-2 with the first-index tie rule: strict > keeps the smallest index among equal values, for both places
+        const bool gt1 = p > b1, gt2 = p > b2;
+        i2 = gt1 ? i1 : (gt2 ? k : i2);
+        i1 = gt1 ? k : i1;
+        b2 = gt1 ? b1 : (gt2 ? p : b2);
+        b1 = gt1 ? p : b1;
+    }
+    // top-2 part of push for a value that counts
+    __device__ __forceinline__ void push_top(float p, int k)
+    {
         const bool gt1 = p > b1, gt2 = p > b2;
         i2 = gt1 ? i1 : (gt2 ? k : i2);
         i1 = gt1 ? k : i1;
@@ -682,6 +703,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             const int kq0 = eo.q0 - qb, nq = (HAS_EL && live) ? eo.q1 - eo.q0 : 0;
             const int l0 = live ? km0 + kq0 : 0;
             const int c = nm + nq;          // every lepton gets a list entry; unselected ones can never match
+            const unsigned longm = __ballot_sync(0xffffffffu, nj > TAIL_CUT);   // events whose tail the warp shares
             // bucket the event's jets by its lepton count: position inside the bucket from a shared-memory
             // counter (any order inside a bucket will do), bucket bases from the eight totals
             const int key = c < N_BUCKETS - 1 ? c : N_BUCKETS - 1;
@@ -723,10 +745,20 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                 {
                     // per jet: byte offset in its column [10:0], byte offset [23:11] and byte length [31:24] of the list
                     unsigned int word = (unsigned)(kj0 << 2) | ((unsigned)l0 << 14) | ((unsigned)c << 27);
-                    uint32_t a = order_a + 4u * (unsigned)(base + pos);
-                    const uint32_t aend = a + 4u * (unsigned)nj;
+                    const uint32_t a0 = order_a + 4u * (unsigned)(base + pos);
+                    uint32_t a = a0;
+                    const uint32_t aend = a + 4u * (unsigned)(nj < TAIL_CUT ? nj : TAIL_CUT);
+                    const unsigned int word0 = word;
 #pragma unroll 1
                     for (; a != aend; a += 4, word += 4) sts_u32(a, word);
+                    // long events: the rest of their words, one per lane
+                    for (unsigned lm = longm; lm; lm &= lm - 1) {
+                        const int src = __ffs(lm) - 1;
+                        const uint32_t as = __shfl_sync(0xffffffffu, a0, src);
+                        const unsigned int ws = __shfl_sync(0xffffffffu, word0, src);
+                        const int ns = __shfl_sync(0xffffffffu, nj, src);
+                        for (int k = TAIL_CUT + lane; k < ns; k += 32) sts_u32(as + 4u * (unsigned)k, ws + 4u * (unsigned)k);
+                    }
                 }
                 __syncwarp();
 
@@ -795,14 +827,51 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         // at the end stays inside the staging buffer's slack)
                         uint32_t ap = a_ev;
                         float pn = lds_f32(ap), cn = CALIB ? lds_f32(ap + d_corr) : 1.0f;
+                        const int nmain = nj < TAIL_CUT ? nj : TAIL_CUT;
 #pragma unroll 1
-                        for (int k = 0; k != nj; ++k) {
+                        for (int k = 0; k != nmain; ++k) {
                             float p = pn;
                             if (CALIB) p = __fmul_rn(p, __fmul_rn(cn, sv));     // NaN when the jet failed eta / dR
                             ap += 4;
                             pn = lds_f32(ap);
                             if (CALIB) cn = lds_f32(ap + d_corr);
                             a.push_lean(p, P.jet_pt_min, k);
+                        }
+                    }
+                    // long events: jets beyond TAIL_CUT, 32 at a time, one per lane, reduced over the warp and folded
+                    // into the owner's state (their indices are larger than every index seen so far, and the two
+                    // best are pushed in (value desc, index asc) order, so the first-index tie rule still holds)
+                    for (unsigned lm = longm; lm; lm &= lm - 1) {
+                        const int src = __ffs(lm) - 1;
+                        const uint32_t as = __shfl_sync(0xffffffffu, a_ev, src);
+                        const int ns = __shfl_sync(0xffffffffu, nj, src);
+                        for (int kb = TAIL_CUT; kb < ns; kb += 32) {
+                            const int k = kb + lane;
+                            float p = -CUDART_INF_F;
+                            if (k < ns) {
+                                p = lds_f32(as + 4u * (unsigned)k);
+                                if (CALIB) p = __fmul_rn(p, __fmul_rn(lds_f32(as + 4u * (unsigned)k + d_corr), sv));
+                            }
+                            const bool ok = p > P.jet_pt_min;
+                            const unsigned okm = __ballot_sync(0xffffffffu, ok);
+                            if (okm == 0u) continue;
+                            double ps = ok ? (double)p : 0.0;
+#pragma unroll
+                            for (int o = 16; o >= 1; o >>= 1) ps += __shfl_xor_sync(0xffffffffu, ps, o);
+                            const unsigned u = ok ? ord_key(p) : 0u;
+                            const unsigned k1 = __reduce_max_sync(0xffffffffu, u);
+                            const int j1 = __reduce_min_sync(0xffffffffu, u == k1 ? k : 0x7fffffff);
+                            const unsigned u2 = k == j1 ? 0u : u;
+                            const unsigned k2 = __reduce_max_sync(0xffffffffu, u2);
+                            const int j2 = __reduce_min_sync(0xffffffffu, (u2 == k2 && u2 != 0u) ? k : 0x7fffffff);
+                            const unsigned kmin = __reduce_min_sync(0xffffffffu, ok ? u : 0xffffffffu);
+                            if (lane == src) {
+                                a.cnt += __popc(okm);
+                                a.sum += ps;
+                                a.mn = fminf(a.mn, ord_value(kmin));
+                                a.push_top(ord_value(k1), j1);
+                                if (k2 != 0u) a.push_top(ord_value(k2), j2);
+                            }
                         }
                     }
                     float e1 = 0, p1 = 0, m1 = 0, e2 = 0, p2 = 0, m2 = 0;
