@@ -52,6 +52,8 @@ def parse_args():
     ap.add_argument("--impl", default="hepk", choices=["hepk", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--single-kernels", action="store_true",
+                    help="time each single kernel (SURVEY.md 8(a) rows a1-a6) instead of the fused chain; one JSON line")
     ap.add_argument("--tune", default="", help="chain tuning knobs, e.g. warps_per_sm=20,ctas_per_sm=1 (testing only)")
     ap.add_argument("--ref-sample", type=int, default=1_000_000, help="events per step of the reference arm")
     return ap.parse_args()
@@ -321,9 +323,68 @@ def run_hepk(args):
         dist.destroy_process_group()
 
 
+def run_single_kernels(args):
+    """Side measurement (BASELINE.json: "single-kernel throughput"): every hepk_* single kernel on the jets /
+    muons of one config, CUDA events over K launches, algorithmic bytes per SURVEY.md 8(d)."""
+    import torch
+
+    import hepgen
+    from paper_1906_06242_b200 import binding as hk
+
+    torch.cuda.set_device(0)
+    hk.lib()
+    wl = hepgen.generate(args.config, n_events=args.events)
+    inp = hk.upload(wl)
+    j, m = inp.jets, inp.muons
+    N, Mj, Mm = wl.n_events, j.pt.numel(), m.pt.numel()
+    peak, peak_src = measured_peak()
+    jsel = hk.select_mask(j.pt, j.eta, 30.0, 2.4)
+    msel = hk.select_mask(m.pt, None, 20.0, float("inf"))
+    edges = inp.axes["ht"]
+    w = inp.weights[0] if inp.weights is not None else None
+    ht = hk.segmented_reduce_sum(j.pt, j.offsets, None, jsel)
+    sumw = torch.zeros(edges.numel() + 1, dtype=torch.float32, device="cuda")
+    counts = torch.zeros(edges.numel() + 1, dtype=torch.int64, device="cuda")
+    cal = inp.calib
+    if cal is None:
+        g = hepgen.generate(3, n_events=1000)
+        cal = {k: torch.from_numpy(g.calib[k]).cuda() for k in ("pt_edges", "eta_edges", "table")}
+    cases = {
+        "select_mask": (lambda: hk.select_mask(j.pt, j.eta, 30.0, 2.4, out=jsel), 9 * Mj),
+        "segmented_reduce_sum[warp-per-event]": (lambda: hk.segmented_reduce_sum(j.pt, j.offsets, None, jsel, variant=1), 12 * N + 5 * Mj),
+        "segmented_reduce_sum[block-per-tile]": (lambda: hk.segmented_reduce_sum(j.pt, j.offsets, None, jsel, variant=2), 12 * N + 5 * Mj),
+        "segmented_reduce_max": (lambda: hk.segmented_reduce_max(j.pt, j.offsets, None, jsel), 12 * N + 5 * Mj),
+        "segmented_reduce_count": (lambda: hk.segmented_reduce_count(None, j.offsets, None, jsel), 12 * N + Mj),
+        "segmented_reduce_argmax": (lambda: hk.segmented_reduce_argmax(j.pt, j.offsets, None, jsel), 12 * N + 5 * Mj),
+        "deltar_mask": (lambda: hk.deltar_mask(j.eta, j.phi, j.offsets, jsel, m.eta, m.phi, m.offsets, msel, 0.4), 16 * N + 9 * Mj + 9 * Mm + Mj),
+        "pair_invmass": (lambda: hk.pair_invmass(j.pt, j.eta, j.phi, j.mass, j.offsets, jsel), 8 * N + 17 * Mj + 12 * N),
+        "lookup_binned": (lambda: hk.lookup_binned(j.pt, j.eta, cal["pt_edges"], cal["eta_edges"], cal["table"]), 12 * Mj),
+        "fill_histogram": (lambda: hk.fill_histogram(ht, w, edges, sumw=sumw, counts=counts), (8 if w is not None else 4) * N),
+    }
+    out = {}
+    for name, (fn, nbytes) in cases.items():
+        for _ in range(max(args.warmup, 3)):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        out[name] = {"ms": ms, "algorithmic_bytes": nbytes, "GBps": nbytes / ms / 1e6, "frac_of_peak": nbytes / ms / 1e6 / peak}
+    print(json.dumps({"metric": "single-kernel throughput (algorithmic GB/s; side measurement)", "unit": "GB/s",
+                      "config": {"workload": workload_name(args.config, wl), "events": N, "jets": Mj, "muons": Mm,
+                                 "l2": "config 1 (132 MB) is L2-resident on B200; use --config 2 for HBM figures"},
+                      "peak": peak, "peak_source": peak_src, "steps": args.steps, "kernels": out}))
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.single_kernels:
+        run_single_kernels(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_hepk(args)
