@@ -22,6 +22,7 @@
 // Privatised histograms are merged into float64 global accumulators every few thousand events.
 // A tile that does not fit its staging region (giant events, misaligned or out-of-range slices) takes the
 // paper's own loop shape (Listing 1): one lane per event, straight from global memory.
+#include <stdlib.h>
 #include <string.h>
 
 #include "hepk_common.cuh"
@@ -213,6 +214,17 @@ __device__ __forceinline__ float dr2_min(float eta_a, float phi_a, float eta_b, 
     const float t = __fsub_rn(fabsf(d), HEPK_TWO_PI_F);
     const float w = fminf(fabsf(d), fabsf(t));
     return __fadd_rn(__fmul_rn(deta, deta), __fmul_rn(w, w));
+}
+
+// The same value from packed float32x2 operations (FADD2 / FMUL2 round each half like FADD / FMUL): `jet` is
+// (eta, phi) of the jet, `nlep` is (-eta, -phi) of the lepton, so one packed add yields (deta, dphi).
+__device__ __forceinline__ float dr2_packed(float2 jet, float2 nlep)
+{
+    float2 d = __fadd2_rn(jet, nlep);
+    const float t = __fsub_rn(fabsf(d.y), HEPK_TWO_PI_F);
+    d.y = fminf(fabsf(d.y), fabsf(t));
+    const float2 q = __fmul2_rn(d, d);
+    return __fadd_rn(q.x, q.y);
 }
 
 // pair_mass_fast (hepk_common.cuh) with the hardware approximations (ex2, rcp, sqrt: 1-2 ulp each) in place of
@@ -716,7 +728,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             mbar_wait(bar, parity);
             parity ^= 1u;
             if (staged) {
-                // combined (eta, phi) list of the event: muons then electrons; eta = +inf marks "not selected"
+                // combined (-eta, -phi) list of the event: muons then electrons; -eta = -inf marks "not selected"
                 // (deta^2 = inf, so dR^2 = inf or NaN and the minimum below ignores it)
                 uint32_t out = lep_a + 8u * (unsigned)l0;      // (l0 <= MAX_LIST by the capacities)
                 {
@@ -725,7 +737,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
 #pragma unroll 1
                     for (; a != aend; a += 4, out += 8) {
                         const float pt = lds_f32(a), eta = lds_f32(a + ms), phi = lds_f32(a + 2 * ms);
-                        sts_v2(out, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                        sts_v2(out, pt > P.lep_pt_min ? -eta : -CUDART_INF_F, -phi);
                     }
                 }
                 if (HAS_EL) {
@@ -734,7 +746,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
 #pragma unroll 1
                     for (; a != aend; a += 4, out += 8) {
                         const float pt = lds_f32(a), eta = lds_f32(a + es), phi = lds_f32(a + 2 * es);
-                        sts_v2(out, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                        sts_v2(out, pt > P.lep_pt_min ? -eta : -CUDART_INF_F, -phi);
                     }
                 }
                 __syncwarp();       // bucket totals complete
@@ -774,7 +786,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     float dmin = CUDART_INF_F;
                     if (word & (8u << 24)) {            // odd count: one lepton first, then pairs
                         const float2 l = lds_v2(al);
-                        dmin = dr2_min(eta, phi, l.x, l.y);
+                        dmin = dr2_packed(make_float2(eta, phi), l);
                         al += 8;
                     }
                     {
@@ -785,7 +797,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                             const float2 l0_ = l, m0_ = m;
                             al += 16;
                             l = lds_v2(al); m = lds_v2(al + 8);
-                            dmin = fminf(dmin, fminf(dr2_min(eta, phi, l0_.x, l0_.y), dr2_min(eta, phi, m0_.x, m0_.y)));
+                            dmin = fminf(dmin, fminf(dr2_packed(make_float2(eta, phi), l0_), dr2_packed(make_float2(eta, phi), m0_)));
                         }
                     }
                     const bool base_ok = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
@@ -1124,7 +1136,11 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
 #define HEPK_PICK(MAXT)                                                                                              \
     (calib ? (has_el ? dev::chain_kernel<true, true, MAXT> : dev::chain_kernel<true, false, MAXT>)                 \
            : (has_el ? dev::chain_kernel<false, true, MAXT> : dev::chain_kernel<false, false, MAXT>))
-    if (wpc <= 16) kern = HEPK_PICK(512);
+    const char* force = getenv("HEPK_FORCE_MAXT");      // experiment hook: register budget variant
+    const int fm = force ? atoi(force) : 0;
+    if (fm == 640 && wpc <= 20) kern = HEPK_PICK(640);
+    else if (fm == 768) kern = HEPK_PICK(768);
+    else if (wpc <= 16) kern = HEPK_PICK(512);
     else if (wpc <= 20) kern = HEPK_PICK(640);
     else kern = HEPK_PICK(768);
 #undef HEPK_PICK
