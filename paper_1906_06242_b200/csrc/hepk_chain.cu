@@ -220,11 +220,26 @@ __device__ __forceinline__ float dr2_min(float eta_a, float phi_a, float eta_b, 
 // (eta, phi) of the jet, `nlep` is (-eta, -phi) of the lepton, so one packed add yields (deta, dphi).
 __device__ __forceinline__ float dr2_packed(float2 jet, float2 nlep)
 {
-    float2 d = __fadd2_rn(jet, nlep);
-    const float t = __fsub_rn(fabsf(d.y), HEPK_TWO_PI_F);
-    d.y = fminf(fabsf(d.y), fabsf(t));
-    const float2 q = __fmul2_rn(d, d);
-    return __fadd_rn(q.x, q.y);
+    float r;
+    asm("{\n\t"
+        ".reg .b64 j, l, d, q;\n\t"
+        ".reg .f32 dx, dy, ay, t, at, w, qx, qy;\n\t"
+        "mov.b64 j, {%1, %2};\n\t"
+        "mov.b64 l, {%3, %4};\n\t"
+        "add.rn.f32x2 d, j, l;\n\t"
+        "mov.b64 {dx, dy}, d;\n\t"
+        "abs.f32 ay, dy;\n\t"
+        "add.rn.f32 t, ay, 0fC0C90FDB;\n\t"      // |dphi| - 2PI_F
+        "abs.f32 at, t;\n\t"
+        "min.f32 w, ay, at;\n\t"
+        "mov.b64 d, {dx, w};\n\t"
+        "mul.rn.f32x2 q, d, d;\n\t"
+        "mov.b64 {qx, qy}, q;\n\t"
+        "add.rn.f32 %0, qx, qy;\n\t"
+        "}"
+        : "=f"(r)
+        : "f"(jet.x), "f"(jet.y), "f"(nlep.x), "f"(nlep.y));
+    return r;
 }
 
 // pair_mass_fast (hepk_common.cuh) with the hardware approximations (ex2, rcp, sqrt: 1-2 ulp each) in place of
@@ -789,16 +804,10 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         dmin = dr2_packed(make_float2(eta, phi), l);
                         al += 8;
                     }
-                    {
-                        // pairs, the next pair loaded ahead (over-read at the end stays inside the list buffer's slack)
-                        float2 l = lds_v2(al), m = lds_v2(al + 8);
 #pragma unroll 1
-                        for (; al != alend;) {
-                            const float2 l0_ = l, m0_ = m;
-                            al += 16;
-                            l = lds_v2(al); m = lds_v2(al + 8);
-                            dmin = fminf(dmin, fminf(dr2_packed(make_float2(eta, phi), l0_), dr2_packed(make_float2(eta, phi), m0_)));
-                        }
+                    for (; al != alend; al += 16) {
+                        const float2 l = lds_v2(al), m = lds_v2(al + 8);
+                        dmin = fminf(dmin, fminf(dr2_packed(make_float2(eta, phi), l), dr2_packed(make_float2(eta, phi), m)));
                     }
                     const bool base_ok = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
                     if (!CALIB) {
