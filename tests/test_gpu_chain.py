@@ -142,7 +142,9 @@ def test_chain_ties_and_threshold_values(hk):
     assert (ref["argmax"][0] >= 0).sum() > 1000
 
 
-def test_chain_misaligned_columns_and_content_base(hk):
+@pytest.mark.parametrize("shifts", [((1, 2, 3, 1), (3, 0, 1, 2), (2, 2, 1, 0)),        # columns disagree: per-event path
+                                    ((1, 1, 1, 1), (3, 3, 3, 3), (2, 2, 2, 2))])       # staged path with a shift
+def test_chain_misaligned_columns_and_content_base(hk, shifts):
     """Columns that are only 4-byte aligned, and an event range given as an offsets slice plus content_base."""
     wl = hepgen.generate(2, n_events=20_000, seed=4)
     e0, e1 = 4_001, 17_777
@@ -159,9 +161,9 @@ def test_chain_misaligned_columns_and_content_base(hk):
         g0, g1 = int(wlc.offsets[e0]), int(wlc.offsets[e1])
         cols = [shifted(getattr(c, nm)[g0:g1].contiguous(), s) for nm, s in zip(("pt", "eta", "phi", "mass"), shifts)]
         return hk.DeviceCollection(c.offsets[e0:e1 + 1].contiguous(), *cols, content_base=g0)
-    inp.jets = cut(inp.jets, wl.jets, (1, 2, 3, 1))
-    inp.muons = cut(inp.muons, wl.muons, (3, 0, 1, 2))
-    inp.electrons = cut(inp.electrons, wl.electrons, (2, 2, 1, 0))
+    inp.jets = cut(inp.jets, wl.jets, shifts[0])
+    inp.muons = cut(inp.muons, wl.muons, shifts[1])
+    inp.electrons = cut(inp.electrons, wl.electrons, shifts[2])
     inp.weights = inp.weights[:, e0:e1].contiguous()
     inp.n_events = e1 - e0
     out, plan = hk.analysis_chain(inp, want_mask=True)
@@ -169,6 +171,41 @@ def test_chain_misaligned_columns_and_content_base(hk):
     g0, g1 = int(wl.jets.offsets[e0]), int(wl.jets.offsets[e1])
     ref["jet_mask"] = ref["jet_mask"][:, g0:g1]
     compare(out, ref, wl)
+
+
+def test_chain_irregular_axes_and_odd_weights(hk):
+    """Histogram axes the arithmetic bin guess cannot be used on (binary-search path), and weights the
+    fixed-point bins cannot hold (non-finite -> float path) or that span many orders of magnitude."""
+    wl = hepgen.generate(4, n_events=20_000, seed=11)
+    rng = np.random.default_rng(5)
+    for name, hi in (("ht", 1000.0), ("mjj", 1000.0), ("njet", 50.0)):
+        nb = wl.axes[name].size - 1
+        e = np.sort(rng.uniform(0.0, hi, nb - 1)).astype(np.float32)
+        wl.axes[name] = np.unique(np.concatenate([[np.float32(0)], e, [np.float32(hi)]])).astype(np.float32)
+    ref = hepo.analysis_chain(wl, want_mask=False)
+    out, _ = hk.analysis_chain(hk.upload(wl))
+    torch.cuda.synchronize()
+    assert_exact(to_np(out["hist_counts"]), ref["hist_counts"], "irregular axes counts")
+    assert_tol(to_np(out["hist_sumw"]), ref["hist_sumw"], "irregular axes sumw")
+    # weights with a wide but same-signed range: every bin within tolerance of the float64 sum
+    wl = hepgen.generate(2, n_events=30_000, seed=12)
+    wl.weights = (wl.weights * np.float32(3.0e-7)).astype(np.float32)
+    ref = hepo.analysis_chain(wl, want_mask=False)
+    out, _ = hk.analysis_chain(hk.upload(wl))
+    torch.cuda.synchronize()
+    got, want = to_np(out["hist_sumw"]).astype(np.float64), ref["hist_sumw"].astype(np.float64)
+    assert np.all(np.abs(got - want) <= 1e-5 * np.abs(want) + 1e-12), "tiny weights"
+    # one infinite weight: the launch falls back to float bins; only that event's bins become inf
+    wl = hepgen.generate(1, n_events=5_000, seed=13)
+    wl.weights[0, 1234] = np.float32(np.inf)
+    ref = hepo.analysis_chain(wl, want_mask=False)
+    out, _ = hk.analysis_chain(hk.upload(wl))
+    torch.cuda.synchronize()
+    got, want = to_np(out["hist_sumw"]), ref["hist_sumw"]
+    assert_exact(np.isinf(got), np.isinf(want), "inf bins")
+    fin = np.isfinite(want)
+    assert_tol(got[fin], want[fin], "finite bins next to an inf weight")
+    assert_exact(to_np(out["hist_counts"]), ref["hist_counts"])
 
 
 def test_chain_optional_outputs(hk):
