@@ -75,6 +75,7 @@ struct ChainParams {
     int region_bytes, shared_bytes;      // per-warp region; CTA-shared part in front of the regions
     int flush_events;                    // a CTA flushes its histograms to the global accumulators every this many events
     const unsigned int* wmax_bits;       // [0] bits of max |weight| over the launch, [1] != 0: a weight is not finite
+    unsigned int* tile_counter;          // zeroed per launch: tiles beyond the first one of each warp are handed out dynamically (nullptr: static)
 };
 
 namespace dev {
@@ -183,24 +184,24 @@ __device__ __forceinline__ float sqrt_approx(float x)
 // Histogram slot (0 underflow, 1+b, nbins+1 overflow/NaN).  inv != 0 means the kernel has verified at start-up
 // that |(edges[i] - lo) * inv - i| <= 0.5 for every edge; the same monotone float32 expression applied to x then
 // lands within one bin of the right one, and a single +-1 step against the edges makes the result exact.
-__device__ __forceinline__ int slot_lean(float x, const float* edges, int nb, float lo, float inv)
+__device__ __forceinline__ int slot_lean(float x, uint32_t edges_a, int nb, float lo, float inv)
 {
     if (inv == 0.0f) {       // irregular axis: binary search on the edges
-        if (x < edges[0]) return 0;
-        if (!(x < edges[nb])) return nb + 1;
+        if (x < lds_f32(edges_a)) return 0;
+        if (!(x < lds_f32(edges_a + 4u * (unsigned)nb))) return nb + 1;
         int a = 0, b = nb;
         while (b - a > 1) {
             const int mid = (a + b) >> 1;
-            if (x >= edges[mid]) a = mid; else b = mid;
+            if (x >= lds_f32(edges_a + 4u * (unsigned)mid)) a = mid; else b = mid;
         }
         return 1 + a;
     }
     int g = (int)((x - lo) * inv);                 // NaN -> 0, +-inf saturate
     g = max(0, min(g, nb - 1));
-    const float a = edges[g], b = edges[g + 1];
+    const float2 ab = make_float2(lds_f32(edges_a + 4u * (unsigned)g), lds_f32(edges_a + 4u * (unsigned)g + 4u));
     int s = g + 1;
-    s += (x >= b) ? 1 : 0;
-    s -= (x < a) ? 1 : 0;
+    s += (x >= ab.y) ? 1 : 0;
+    s -= (x < ab.x) ? 1 : 0;
     return (x != x) ? nb + 1 : s;
 }
 
@@ -314,7 +315,8 @@ __device__ __forceinline__ uint32_t obs_bin(const ChainParams& P, const ChainSha
 {
     if (!(feat & (F_OBS0 << OB))) return 0u;
     const int nb = P.axis_nbins[OB];
-    const int slot = slot_lean(x, S.edges + P.edge_prefix[OB], nb, S.axis_lo[OB], S.axis_inv[OB]);
+    const int slot = slot_lean(x, smem_u32(S.edges) + 4u * (unsigned)P.edge_prefix[OB], nb, lds_f32(smem_u32(S.axis_lo) + 4u * OB),
+                               lds_f32(smem_u32(S.axis_inv) + 4u * OB));
     const int spv = P.obs_prefix[HEPK_N_OBS], pre = P.obs_prefix[OB];
     if (feat & F_COUNTS) red_add_shared_u32(smem_u32(S.h_cnt) + 4u * (unsigned)(v * spv + pre + slot), 1u);
     return smem_u32(S.h_sumw) + 4u * (unsigned)((v * spv + pre) * P.W + slot);
@@ -337,7 +339,7 @@ __device__ __forceinline__ void add_weight(const ChainParams& P, unsigned feat, 
 
 // Per event and variant: leading-pair mass, outputs, histograms.  Shared by the staged path and the per-event
 // path.  The leading jets' (eta, phi, mass) are passed in by value; i2 < 0 means fewer than two clean jets.
-__device__ __forceinline__ void finish_event(const ChainParams& P, const ChainShared& S, unsigned feat, long long ev, int v,
+__device__ __forceinline__ void finish_event(const ChainParams& P, const ChainShared& S, unsigned feat, long long ev, int v, float wt0,
                                              int cnt, float sum, float mn, float b1, float b2, int i1, int i2,
                                              float eta1, float phi1, float m1, float eta2, float phi2, float m2)
 {
@@ -348,12 +350,13 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
         mjj = pair_mass_lean(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
         if (hists && (feat & (F_OBS0 << HEPK_OBS_MJJ))) {
             // the bin of mjj is decided by the float64-defined value: refine when the fast value is near an edge
-            const float* ed = S.edges + P.edge_prefix[HEPK_OBS_MJJ];
+            const uint32_t ed = smem_u32(S.edges) + 4u * (unsigned)P.edge_prefix[HEPK_OBS_MJJ];
             const int nb = P.axis_nbins[HEPK_OBS_MJJ];
-            const int s = slot_lean(mjj, ed, nb, S.axis_lo[HEPK_OBS_MJJ], S.axis_inv[HEPK_OBS_MJJ]);
+            const int s = slot_lean(mjj, ed, nb, lds_f32(smem_u32(S.axis_lo) + 4u * HEPK_OBS_MJJ),
+                                    lds_f32(smem_u32(S.axis_inv) + 4u * HEPK_OBS_MJJ));
             const float band = fmaf(mjj, HEPK_MASS_GUARD_REL, HEPK_MASS_GUARD_ABS);
-            const bool near_lo = s >= 1 && mjj - ed[s - 1] <= band;
-            const bool near_hi = s <= nb && ed[s] - mjj <= band;
+            const bool near_lo = s >= 1 && mjj - lds_f32(ed + 4u * (unsigned)(s - 1)) <= band;
+            const bool near_hi = s <= nb && lds_f32(ed + 4u * (unsigned)s) - mjj <= band;
             if (near_lo || near_hi) mjj = pair_mass_f64(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
         }
     }
@@ -374,9 +377,9 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     bin[HEPK_OBS_MJJ] = obs_bin<HEPK_OBS_MJJ>(P, S, feat, v, mjj);
     bin[HEPK_OBS_SUBPT] = obs_bin<HEPK_OBS_SUBPT>(P, S, feat, v, subpt);
     if (!(feat & F_SUMW)) return;
-    const float wscale = S.wscale[0];
-    if (!(feat & F_WEIGHTS)) { add_weight(P, feat, bin, 0, 1.0f, wscale); return; }
-    add_weight(P, feat, bin, 0, __ldg(P.weights + ev), wscale);
+    const float wscale = lds_f32(smem_u32(S.wscale));
+    add_weight(P, feat, bin, 0, wt0, wscale);
+    if (!(feat & F_WEIGHTS)) return;
     for (int w = 1; w < P.W; ++w) add_weight(P, feat, bin, w, __ldg(P.weights + (long long)w * P.n_events + ev), wscale);
 }
 
@@ -492,7 +495,7 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, const Chai
             e1 = P.jeta[x]; p1 = P.jphi[x]; m1 = P.jmass[x];
             e2 = P.jeta[y]; p2 = P.jphi[y]; m2 = P.jmass[y];
         }
-        finish_event(P, S, chain_features(P), ev, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
+        finish_event(P, S, chain_features(P), ev, v, P.weights ? __ldg(P.weights + ev) : 1.0f, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
     }
 }
 
@@ -695,12 +698,22 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         cur_lo = lo;
     }
 
-    for (; tile < P.n_tiles; tile += GW) {
+    // Tiles after a warp's first are handed out by a global counter (the per-tile cost varies with the events, and
+    // static striding leaves warps waiting at the end); the counter is read two tiles ahead so that its latency
+    // and the next tile's bounds are both covered by the current tile.
+    const bool dyn = P.tile_counter != nullptr;
+    unsigned int raw = 0;
+    if (dyn && lane == 0) raw = atomicAdd(P.tile_counter, 1u);
+    long long tile_next = dyn ? GW + (long long)__shfl_sync(0xffffffffu, raw, 0) : tile + GW;
+
+    for (; tile < P.n_tiles;) {
+        if (dyn && lane == 0) raw = atomicAdd(P.tile_counter, 1u);      // becomes tile_next at the bottom
         const long long e0 = tile * TILE_EVENTS;
         const long long rest = P.n_events - e0;
         const int ne = rest < TILE_EVENTS ? (int)rest : TILE_EVENTS;
-        const long long tile_next = tile + GW;
         const bool has_next = tile_next < P.n_tiles;
+        float wt0 = 1.0f;                                                // weight column 0 of the lane's event, loaded early
+        if ((feat & (F_SUMW | F_WEIGHTS)) == (F_SUMW | F_WEIGHTS) && lane < ne) wt0 = __ldg(P.weights + e0 + lane);
         long long nlo = 0, nhi = 0;
         EventOffsets neo;
         neo.j0 = neo.j1 = neo.m0 = neo.m1 = neo.q0 = neo.q1 = 0;
@@ -909,7 +922,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         released = true;
                     }
                     if (live)
-                        finish_event(P, S, feat, e0 + lane, v, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
+                        finish_event(P, S, feat, e0 + lane, v, wt0, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
                 }
             }
             bsel ^= 1;
@@ -923,10 +936,12 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         __syncwarp();
         eo = neo;
         cur_lo = nlo;
+        tile = tile_next;
+        tile_next = dyn ? GW + (long long)__shfl_sync(0xffffffffu, raw, 0) : tile_next + GW;
 
         {   // the warp whose tile takes the CTA's event count across a multiple of flush_events flushes the histograms
             unsigned int c = 0;
-            if (lane == 0) c = atomicAdd(S.since, (unsigned)ne);
+            if (lane == 0) c = atom_add_shared_u32(smem_u32(S.since), (unsigned)ne);
             c = __shfl_sync(0xffffffffu, c, 0);
             if ((c & ~(unsigned)(P.flush_events - 1)) != ((c + (unsigned)ne) & ~(unsigned)(P.flush_events - 1))) flush_hist(P, S, lane, 32);
         }
@@ -1139,6 +1154,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     const size_t smem = (size_t)shared_bytes + (size_t)wpc * region;
     P.flush_events = 1024;
     P.wmax_bits = want_sumw ? (const unsigned int*)((const double*)workspace + n_sumw) : nullptr;
+    P.tile_counter = want_sumw ? (unsigned int*)((double*)workspace + n_sumw) + 2 : nullptr;
 
     // three register budgets: up to 16 warps per CTA (128 registers per thread), 20 (102) or 24 (85)
     void (*kern)(ChainParams);
