@@ -119,6 +119,14 @@ __device__ __forceinline__ unsigned int atom_add_shared_u32(uint32_t addr, unsig
     asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(r) : "r"(addr), "r"(v) : "memory");
     return r;
 }
+// global atomic add whose result is not needed at once (the compiler's own atomicAdd aggregates over the warp and
+// shuffles the result out immediately, which exposes the whole round trip)
+__device__ __forceinline__ unsigned int atom_add_global_u32(unsigned int* p, unsigned int v)
+{
+    unsigned int r;
+    asm volatile("atom.global.add.u32 %0, [%1], %2;" : "=r"(r) : "l"(p), "r"(v) : "memory");
+    return r;
+}
 __device__ __forceinline__ void red_add_shared_u32(uint32_t addr, unsigned int v)
 {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
@@ -465,8 +473,10 @@ __device__ inline bool match_global(const ChainParams& P, float eta, float phi, 
 // Path for the events of a tile that does not fit the staging region: the paper's own loop shape
 // (Listing 1), one lane per event, everything from global memory.  Slow; only unusual tiles get here.
 template <bool CALIB>
-__device__ __noinline__ void chain_event_global(const ChainParams& P, const ChainShared& S, long long ev)
+__device__ __noinline__ void chain_event_global(const ChainParams& P, unsigned char* smem_base, long long ev)
 {
+    ChainShared S;          // rebuilt here: passing the caller's by reference would force it into local memory
+    chain_shared_layout(P, CALIB, smem_base, &S);
     const long long g0 = P.off[0][ev], g1 = P.off[0][ev + 1];
     for (int v = 0; v < P.V; ++v) {
         EventAcc a;
@@ -703,11 +713,11 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     // and the next tile's bounds are both covered by the current tile.
     const bool dyn = P.tile_counter != nullptr;
     unsigned int raw = 0;
-    if (dyn && lane == 0) raw = atomicAdd(P.tile_counter, 1u);
+    if (dyn && lane == 0) raw = atom_add_global_u32(P.tile_counter, 1u);
     long long tile_next = dyn ? GW + (long long)__shfl_sync(0xffffffffu, raw, 0) : tile + GW;
 
     for (; tile < P.n_tiles;) {
-        if (dyn && lane == 0) raw = atomicAdd(P.tile_counter, 1u);      // becomes tile_next at the bottom
+        if (dyn && lane == 0) raw = atom_add_global_u32(P.tile_counter, 1u);      // becomes tile_next at the bottom
         const long long e0 = tile * TILE_EVENTS;
         const long long rest = P.n_events - e0;
         const int ne = rest < TILE_EVENTS ? (int)rest : TILE_EVENTS;
@@ -932,7 +942,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             __syncwarp();
             if (has_next && P.n_col > 0) fit = issue_tile(col, lane, nlo, nhi, bar);
         }
-        if (!staged && lane < ne) chain_event_global<CALIB>(P, S, e0 + lane);
+        if (!staged && lane < ne) chain_event_global<CALIB>(P, smem_raw, e0 + lane);
         __syncwarp();
         eo = neo;
         cur_lo = nlo;
