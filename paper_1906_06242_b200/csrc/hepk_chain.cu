@@ -708,16 +708,20 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         cur_lo = lo;
     }
 
-    // Tiles after a warp's first are handed out by a global counter (the per-tile cost varies with the events, and
-    // static striding leaves warps waiting at the end); the counter is read two tiles ahead so that its latency
-    // and the next tile's bounds are both covered by the current tile.
+    // The per-tile cost varies with the events, and purely static striding leaves warps waiting at the end.
+    // The first 7/8 of the tiles are strided statically; the rest is handed out by a global counter (ptxas turns the
+    // atomic into vote + leader + shuffle, i.e. an immediate wait for the round trip, so it is kept off most tiles).
     const bool dyn = P.tile_counter != nullptr;
-    unsigned int raw = 0;
-    if (dyn && lane == 0) raw = atom_add_global_u32(P.tile_counter, 1u);
-    long long tile_next = dyn ? GW + (long long)__shfl_sync(0xffffffffu, raw, 0) : tile + GW;
+    long long n_static = dyn ? (P.n_tiles - P.n_tiles / 8) / GW * GW : P.n_tiles;
+    if (dyn && n_static < GW) n_static = GW;          // every warp's first tile is static
+    long long tile_next = tile + GW;
+    if (tile_next >= n_static && dyn) {
+        unsigned int raw = 0;
+        if (lane == 0) raw = atom_add_global_u32(P.tile_counter, 1u);
+        tile_next = n_static + (long long)__shfl_sync(0xffffffffu, raw, 0);
+    }
 
     for (; tile < P.n_tiles;) {
-        if (dyn && lane == 0) raw = atom_add_global_u32(P.tile_counter, 1u);      // becomes tile_next at the bottom
         const long long e0 = tile * TILE_EVENTS;
         const long long rest = P.n_events - e0;
         const int ne = rest < TILE_EVENTS ? (int)rest : TILE_EVENTS;
@@ -947,7 +951,12 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         eo = neo;
         cur_lo = nlo;
         tile = tile_next;
-        tile_next = dyn ? GW + (long long)__shfl_sync(0xffffffffu, raw, 0) : tile_next + GW;
+        tile_next += GW;
+        if (tile_next >= n_static && dyn) {
+            unsigned int raw = 0;
+            if (lane == 0) raw = atom_add_global_u32(P.tile_counter, 1u);
+            tile_next = n_static + (long long)__shfl_sync(0xffffffffu, raw, 0);
+        }
 
         {   // the warp whose tile takes the CTA's event count across a multiple of flush_events flushes the histograms
             unsigned int c = 0;
