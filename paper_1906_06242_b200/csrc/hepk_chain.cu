@@ -231,7 +231,7 @@ __device__ __forceinline__ float dr2_packed(float2 jet, float2 nlep)
 {
     float r;
     asm("{\n\t"
-        ".reg .b64 j, l, d, q;\n\t"
+        ".reg .b64 j, l, d;\n\t"
         ".reg .f32 dx, dy, ay, t, at, w, qx, qy;\n\t"
         "mov.b64 j, {%1, %2};\n\t"
         "mov.b64 l, {%3, %4};\n\t"
@@ -241,9 +241,8 @@ __device__ __forceinline__ float dr2_packed(float2 jet, float2 nlep)
         "add.rn.f32 t, ay, 0fC0C90FDB;\n\t"      // |dphi| - 2PI_F
         "abs.f32 at, t;\n\t"
         "min.f32 w, ay, at;\n\t"
-        "mov.b64 d, {dx, w};\n\t"
-        "mul.rn.f32x2 q, d, d;\n\t"
-        "mov.b64 {qx, qy}, q;\n\t"
+        "mul.rn.f32 qx, dx, dx;\n\t"             // (a packed multiply of a pair by itself costs two register moves)
+        "mul.rn.f32 qy, w, w;\n\t"
         "add.rn.f32 %0, qx, qy;\n\t"
         "}"
         : "=f"(r)
