@@ -45,7 +45,7 @@ NVML_REASONS = {
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1..4)")
     ap.add_argument("--events", type=int, default=None, help="override the number of events (testing only)")
@@ -85,7 +85,7 @@ def algorithmic_bytes(wl, n_outputs=len(BENCH_OUTPUTS), event_outputs=True):
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
-    def __init__(self, index, period=0.05):
+    def __init__(self, index, period=0.005):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], 0, None
@@ -273,7 +273,7 @@ def run_hepk(args):
                    "l2": f"inputs {alg_bytes / 1e9:.2f} GB per step >> 126 MB L2, no flush needed",
                    "outputs": list(BENCH_OUTPUTS) if not hists_only else "histograms only"},
         "roofline": roofline, "clocks": sampler.summary(),
-        "gpu_launches": 2 * args.steps,     # chain_kernel + chain_finalize_hist per step (the memset is not a kernel)
+        "gpu_launches": 3 * args.steps,     # chain_wmax_kernel + chain_kernel + chain_finalize_hist per step (the memset is not a kernel)
     }
 
     # ---- end to end through the C ABI with HOST buffers (rank-local; max over ranks)
