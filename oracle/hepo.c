@@ -433,3 +433,78 @@ int32_t hepo_analysis_chain(const hepo_chain_desc* d)
     free(ptv); free(matched); free(clean); free(corr);
     return 0;
 }
+
+/* ---- SURVEY.md 8(f-1) ---------------------------------------------------------------------------------- */
+
+/* position (column index) of the index-th counted element of row e, or -1 */
+static int64_t nth_position(const int64_t* offsets, int64_t e, int64_t content_base, const uint8_t* mask_content, int32_t index)
+{
+    int32_t seen = 0;
+    for (int64_t g = offsets[e]; g < offsets[e + 1]; ++g) {
+        const int64_t i = g - content_base;
+        if (mask_content && !mask_content[i]) continue;
+        if (seen == index) return i;
+        ++seen;
+    }
+    return -1;
+}
+
+int32_t hepo_get_in_offsets(const float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                            const uint8_t* mask_rows, const uint8_t* mask_content, int32_t index, float fill, float* out)
+{
+    if (!seg_args_ok(offsets, n_events, out) || index < 0) return -1;
+    for (int64_t e = 0; e < n_events; ++e) {
+        out[e] = fill;
+        if (mask_rows && !mask_rows[e]) continue;
+        const int64_t i = nth_position(offsets, e, content_base, mask_content, index);
+        if (i >= 0) out[e] = data[i];
+    }
+    return 0;
+}
+
+int32_t hepo_set_in_offsets(float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                            const uint8_t* mask_rows, const uint8_t* mask_content, int32_t index,
+                            const float* values, float value)
+{
+    if (!seg_args_ok(offsets, n_events, data) || index < 0) return -1;
+    for (int64_t e = 0; e < n_events; ++e) {
+        if (mask_rows && !mask_rows[e]) continue;
+        const int64_t i = nth_position(offsets, e, content_base, mask_content, index);
+        if (i >= 0) data[i] = values ? values[e] : value;
+    }
+    return 0;
+}
+
+int32_t hepo_select_opposite_sign(const float* pt, const int32_t* charge, const int64_t* offsets, int64_t n_events,
+                                  int64_t content_base, const uint8_t* mask_rows, const uint8_t* mask_content,
+                                  uint8_t* out_mask)
+{
+    if (!seg_args_ok(offsets, n_events, out_mask) || !charge) return -1;
+    for (int64_t e = 0; e < n_events; ++e) {
+        const int64_t g0 = offsets[e], g1 = offsets[e + 1];
+        for (int64_t g = g0; g < g1; ++g) out_mask[g - content_base] = 0;
+        if (mask_rows && !mask_rows[e]) continue;
+        /* leading object: strict > keeps the first index among equal pt */
+        int64_t lead = -1;
+        for (int64_t g = g0; g < g1; ++g) {
+            const int64_t i = g - content_base;
+            if (mask_content && !mask_content[i]) continue;
+            if (pt[i] != pt[i]) continue;
+            if (lead < 0 || pt[i] > pt[lead]) lead = i;
+        }
+        if (lead < 0) continue;
+        /* highest-pt object of the opposite sign */
+        int64_t part = -1;
+        for (int64_t g = g0; g < g1; ++g) {
+            const int64_t i = g - content_base;
+            if (mask_content && !mask_content[i]) continue;
+            if (pt[i] != pt[i]) continue;
+            if ((int64_t)charge[i] * (int64_t)charge[lead] >= 0) continue;
+            if (part < 0 || pt[i] > pt[part]) part = i;
+        }
+        if (part < 0) continue;
+        out_mask[lead] = 1;
+        out_mask[part] = 1;
+    }
+    return 0;
+}

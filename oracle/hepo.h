@@ -111,6 +111,33 @@ typedef struct {
 int32_t hepo_analysis_chain(const hepo_chain_desc* d);
 size_t  hepo_chain_desc_size(void);
 
+/* ---- the remaining generic kernels of the paper's list ------------------------------
+ *
+ * get_in_offsets ("given jagged data with offsets, retrieves the n-th elements for all rows ...
+ * to create a contiguous array of e.g. the leading jet pT").  out[e] = the index-th element of row e, counting
+ * only elements with mask_content set (mask_content == NULL: every element); rows with mask_rows clear or with
+ * fewer than index+1 counted elements get `fill`.  index >= 0.  (Counting through the content mask and the
+ * fill value are readings: the paper says neither.  parity unpinned for those two conventions.) */
+int32_t hepo_get_in_offsets(const float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                            const uint8_t* mask_rows, const uint8_t* mask_content, int32_t index, float fill,
+                            float* out);
+
+/* set_in_offsets ("as above, but sets the n-th element to a value ... to selectively mask
+ * objects in a collection").  data[position of the index-th counted element of row e] = values ? values[e]
+ * : value, for rows with mask_rows set (or NULL) that have that element; everything else is left untouched. */
+int32_t hepo_set_in_offsets(float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                            const uint8_t* mask_rows, const uint8_t* mask_content, int32_t index,
+                            const float* values, float value);
+
+/* select_opposite_sign_muons ("given a collection of objects with charge (i.e. muons),
+ * masks all but the first two objects ordered by pT which are of opposite charge").  Per event, over the
+ * objects with mask_content set: the leading object by pt (first index among equal pt) and the highest-pt
+ * object whose charge has the opposite sign (charge * charge_lead < 0; first index among equal pt) get 1,
+ * everything else 0; an event without such a pair (or with mask_rows clear) gets all 0.  NaN pt is skipped. */
+int32_t hepo_select_opposite_sign(const float* pt, const int32_t* charge, const int64_t* offsets, int64_t n_events,
+                                  int64_t content_base, const uint8_t* mask_rows, const uint8_t* mask_content,
+                                  uint8_t* out_mask);
+
 #ifdef __cplusplus
 }
 #endif

@@ -102,6 +102,40 @@ def pair_invmass(pt, eta, phi, mass, offsets, mask_content=None, content_base=0)
     return m, i1, i2
 
 
+def get_in_offsets(data, offsets, index, mask_rows=None, mask_content=None, fill=0.0, content_base=0):
+    data, offsets = _f32(data), _i64(offsets)
+    mask_rows, mask_content = _u8(mask_rows), _u8(mask_content)
+    n = offsets.shape[0] - 1
+    out = np.empty(n, dtype=np.float32)
+    _check(lib().hepo_get_in_offsets(_p(data, np.float32), _p(offsets, np.int64), C.c_int64(n), C.c_int64(content_base),
+                                     _p(mask_rows, np.uint8), _p(mask_content, np.uint8), C.c_int32(index),
+                                     C.c_float(fill), _p(out, np.float32)))
+    return out
+
+
+def set_in_offsets(data, offsets, index, values=None, value=0.0, mask_rows=None, mask_content=None, content_base=0):
+    """Returns a modified copy of `data`."""
+    data, offsets, values = _f32(data).copy(), _i64(offsets), _f32(values)
+    mask_rows, mask_content = _u8(mask_rows), _u8(mask_content)
+    n = offsets.shape[0] - 1
+    _check(lib().hepo_set_in_offsets(_p(data, np.float32), _p(offsets, np.int64), C.c_int64(n), C.c_int64(content_base),
+                                     _p(mask_rows, np.uint8), _p(mask_content, np.uint8), C.c_int32(index),
+                                     _p(values, np.float32), C.c_float(value)))
+    return data
+
+
+def select_opposite_sign(pt, charge, offsets, mask_rows=None, mask_content=None, content_base=0):
+    pt, offsets = _f32(pt), _i64(offsets)
+    charge = np.ascontiguousarray(charge, dtype=np.int32)
+    mask_rows, mask_content = _u8(mask_rows), _u8(mask_content)
+    n = offsets.shape[0] - 1
+    out = np.zeros(pt.shape[0], dtype=np.uint8)
+    _check(lib().hepo_select_opposite_sign(_p(pt, np.float32), _p(charge, np.int32), _p(offsets, np.int64), C.c_int64(n),
+                                           C.c_int64(content_base), _p(mask_rows, np.uint8), _p(mask_content, np.uint8),
+                                           _p(out, np.uint8)))
+    return out
+
+
 def lookup_binned(x, y, edges_x, edges_y, table):
     x, y, edges_x, edges_y = _f32(x), _f32(y), _f32(edges_x), _f32(edges_y)
     table = _f32(table)
