@@ -345,6 +345,8 @@ def run_single_kernels(args):
     ht = hk.segmented_reduce_sum(j.pt, j.offsets, None, jsel)
     sumw = torch.zeros(edges.numel() + 1, dtype=torch.float32, device="cuda")
     counts = torch.zeros(edges.numel() + 1, dtype=torch.int64, device="cuda")
+    scratch = j.pt.clone()
+    charge = torch.randint(0, 2, (Mm,), device="cuda", dtype=torch.int32) * 2 - 1
     cal = inp.calib
     if cal is None:
         g = hepgen.generate(3, n_events=1000)
@@ -360,6 +362,10 @@ def run_single_kernels(args):
         "pair_invmass": (lambda: hk.pair_invmass(j.pt, j.eta, j.phi, j.mass, j.offsets, jsel), 8 * N + 17 * Mj + 12 * N),
         "lookup_binned": (lambda: hk.lookup_binned(j.pt, j.eta, cal["pt_edges"], cal["eta_edges"], cal["table"]), 12 * Mj),
         "fill_histogram": (lambda: hk.fill_histogram(ht, w, edges, sumw=sumw, counts=counts), (8 if w is not None else 4) * N),
+        # 8 B/event of offsets + one 32-byte sector per touched element + the output
+        "get_in_offsets[index 0]": (lambda: hk.get_in_offsets(j.pt, j.offsets, 0, fill=0.0), 8 * N + 32 * N + 4 * N),
+        "set_in_offsets[index 0]": (lambda: hk.set_in_offsets(scratch, j.offsets, 0, value=1.0), 8 * N + 2 * 32 * N),
+        "select_opposite_sign[muons]": (lambda: hk.select_opposite_sign(m.pt, charge, m.offsets), 8 * N + 9 * Mm),
     }
     out = {}
     for name, (fn, nbytes) in cases.items():

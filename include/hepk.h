@@ -235,6 +235,37 @@ int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t batch_events,
                                  void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * The remaining generic kernels of the paper's list.  All pointers are DEVICE pointers.
+ *
+ * get_in_offsets ("given jagged data with offsets, retrieves the n-th elements for all rows ...
+ * to create a contiguous array of e.g. the leading jet pT"):
+ *   out[e] = the index-th element of row e, counting only elements with mask_content set (NULL: all);
+ *   rows with mask_rows clear, or with fewer than index+1 counted elements, get `fill`.
+ * data: float32[M]; offsets: int64[n_events+1]; out: float32[n_events]; index >= 0 else HEPK_ERR_INVALID. */
+int32_t hepk_get_in_offsets(const float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                            const uint8_t* mask_rows, const uint8_t* mask_content, int32_t index, float fill,
+                            float* out, void* stream);
+
+/* set_in_offsets ("as above, but sets the n-th element to a value ... to selectively mask
+ * objects in a collection"):
+ *   data[position of the index-th counted element of row e] = values ? values[e] : value
+ * for rows with mask_rows set (or NULL) that have that element; everything else is left untouched.
+ * data: float32[M], modified in place; values: float32[n_events] or NULL. */
+int32_t hepk_set_in_offsets(float* data, const int64_t* offsets, int64_t n_events, int64_t content_base,
+                            const uint8_t* mask_rows, const uint8_t* mask_content, int32_t index,
+                            const float* values, float value, void* stream);
+
+/* select_opposite_sign_muons ("given a collection of objects with charge (i.e. muons),
+ * masks all but the first two objects ordered by pT which are of opposite charge"):
+ *   per event, over the objects with mask_content set (NULL: all): the leading object by pt (first index
+ *   among equal pt; NaN skipped) and the highest-pt object whose charge has the opposite sign get 1,
+ *   everything else 0; an event without such a pair, or with mask_rows clear, gets all 0.
+ * pt: float32[M]; charge: int32[M]; out_mask: uint8[M], every element of every event is written. */
+int32_t hepk_select_opposite_sign(const float* pt, const int32_t* charge, const int64_t* offsets, int64_t n_events,
+                                  int64_t content_base, const uint8_t* mask_rows, const uint8_t* mask_content,
+                                  uint8_t* out_mask, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Device-side timing of the dominant kernel (measurement hook for bench.py; no part of the method).
  * Between hepk_profile_begin() and hepk_profile_end() every hepk_analysis_chain call records a CUDA event
  * pair on its launch stream directly around the fused chain kernel (at most 4096 launches are kept).

@@ -198,6 +198,38 @@ def pair_invmass(pt, eta, phi, mass, offsets, mask_content=None, content_base=0,
     return m, i1, i2
 
 
+def get_in_offsets(data, offsets, index, mask_rows=None, mask_content=None, fill=0.0, content_base=0, out=None, stream=None):
+    n = offsets.numel() - 1
+    if out is None:
+        out = torch.empty(n, dtype=torch.float32, device=offsets.device)
+    _check(lib().hepk_get_in_offsets(_ptr(data, torch.float32), _ptr(offsets, torch.int64), C.c_int64(n), C.c_int64(content_base),
+                                     _ptr(_mask(mask_rows), torch.uint8), _ptr(_mask(mask_content), torch.uint8),
+                                     C.c_int32(index), C.c_float(fill), _ptr(out, torch.float32), _stream(stream)),
+           "get_in_offsets")
+    return out
+
+
+def set_in_offsets(data, offsets, index, values=None, value=0.0, mask_rows=None, mask_content=None, content_base=0, stream=None):
+    """In place on `data`; returns it."""
+    n = offsets.numel() - 1
+    _check(lib().hepk_set_in_offsets(_ptr(data, torch.float32), _ptr(offsets, torch.int64), C.c_int64(n), C.c_int64(content_base),
+                                     _ptr(_mask(mask_rows), torch.uint8), _ptr(_mask(mask_content), torch.uint8),
+                                     C.c_int32(index), _ptr(values, torch.float32), C.c_float(value), _stream(stream)),
+           "set_in_offsets")
+    return data
+
+
+def select_opposite_sign(pt, charge, offsets, mask_rows=None, mask_content=None, content_base=0, out=None, stream=None):
+    n = offsets.numel() - 1
+    if out is None:
+        out = torch.empty(pt.numel(), dtype=torch.uint8, device=pt.device)
+    _check(lib().hepk_select_opposite_sign(_ptr(pt, torch.float32), _ptr(charge, torch.int32), _ptr(offsets, torch.int64),
+                                           C.c_int64(n), C.c_int64(content_base), _ptr(_mask(mask_rows), torch.uint8),
+                                           _ptr(_mask(mask_content), torch.uint8), _ptr(out, torch.uint8), _stream(stream)),
+           "select_opposite_sign")
+    return out
+
+
 def lookup_binned(x, y, edges_x, edges_y, table, out=None, stream=None):
     n = x.numel()
     if out is None:

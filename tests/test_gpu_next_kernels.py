@@ -1,0 +1,99 @@
+"""Parity of the SURVEY.md 8(f-1) CUDA kernels (hepk_get_in_offsets, hepk_set_in_offsets, hepk_select_opposite_sign,
+through the C ABI) against the CPU oracle on the same seeded inputs.  All three are exact class: bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import hepgen
+from oracle import hepo
+from _util import assert_exact, to_np
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hk():
+    from paper_1906_06242_b200 import binding
+    binding.lib()
+    return binding
+
+
+def cu(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def charges(rng, m):
+    q = rng.choice([-1, 1], m).astype(np.int32)
+    q[rng.random(m) < 0.01] = 0
+    return q
+
+
+@pytest.mark.parametrize("config,n", [(0, None), (2, 300_011)])
+def test_get_and_set_in_offsets(hk, config, n):
+    wl = hepgen.generate(config, n_events=n)
+    rng = np.random.default_rng(7)
+    j = wl.jets
+    N, M = wl.n_events, j.pt.size
+    mc = (rng.random(M) < 0.7).astype(np.uint8)
+    mr = (rng.random(N) < 0.85).astype(np.uint8)
+    vals = rng.normal(size=N).astype(np.float32)
+    d_pt, d_off, d_mc, d_mr = cu(j.pt), cu(j.offsets), cu(mc), cu(mr)
+    for index in (0, 1, 5, 39, 200):
+        for rows, cont in ((None, None), (mr, mc)):
+            want = hepo.get_in_offsets(j.pt, j.offsets, index, rows, cont, fill=-1.5)
+            got = hk.get_in_offsets(d_pt, d_off, index, None if rows is None else d_mr, None if cont is None else d_mc, fill=-1.5)
+            assert_exact(to_np(got), want, f"get index={index} masks={rows is not None}")
+            want = hepo.set_in_offsets(j.pt, j.offsets, index, values=vals, mask_rows=rows, mask_content=cont)
+            buf = d_pt.clone()
+            hk.set_in_offsets(buf, d_off, index, values=cu(vals), mask_rows=None if rows is None else d_mr,
+                              mask_content=None if cont is None else d_mc)
+            assert_exact(to_np(buf), want, f"set index={index}")
+    want = hepo.set_in_offsets(j.pt, j.offsets, 0, value=3.25)
+    buf = d_pt.clone()
+    hk.set_in_offsets(buf, d_off, 0, value=3.25)
+    assert_exact(to_np(buf), want, "set scalar")
+    torch.cuda.synchronize()
+
+
+def test_get_in_offsets_content_base_and_edges(hk):
+    wl = hepgen.generate(2, n_events=5_000, seed=3)
+    j = wl.jets
+    e0, e1 = 1_000, 4_321
+    g0, g1 = int(j.offsets[e0]), int(j.offsets[e1])
+    want = hepo.get_in_offsets(j.pt[g0:g1], j.offsets[e0:e1 + 1], 2, fill=0.0, content_base=g0)
+    got = hk.get_in_offsets(cu(j.pt[g0:g1]), cu(j.offsets[e0:e1 + 1]), 2, fill=0.0, content_base=g0)
+    assert_exact(to_np(got), want)
+    assert_exact(want, hepo.get_in_offsets(j.pt, j.offsets, 2, fill=0.0)[e0:e1])
+    empty = np.zeros(1, np.int64)                               # no events at all
+    assert hk.get_in_offsets(cu(np.zeros(0, np.float32)), cu(empty), 0).numel() == 0
+    off = np.zeros(101, np.int64)                               # 100 empty events
+    got = hk.get_in_offsets(cu(np.zeros(0, np.float32)), cu(off), 0, fill=9.0)
+    assert (to_np(got) == 9.0).all()
+    with pytest.raises(hk.HepkError):
+        hk.get_in_offsets(cu(j.pt), cu(j.offsets), -1)
+
+
+@pytest.mark.parametrize("config,n", [(0, None), (2, 400_003)])
+def test_select_opposite_sign(hk, config, n):
+    wl = hepgen.generate(config, n_events=n)
+    rng = np.random.default_rng(8)
+    m = wl.muons
+    N, M = wl.n_events, m.pt.size
+    pt = m.pt.copy()
+    pt[rng.random(M) < 0.1] = np.float32(33.0)                  # ties
+    pt[rng.random(M) < 0.001] = np.float32(np.nan)
+    q = charges(rng, M)
+    mc = (rng.random(M) < 0.8).astype(np.uint8)
+    mr = (rng.random(N) < 0.9).astype(np.uint8)
+    for rows, cont in ((None, None), (mr, mc)):
+        want = hepo.select_opposite_sign(pt, q, m.offsets, rows, cont)
+        got = hk.select_opposite_sign(cu(pt), cu(q), cu(m.offsets), None if rows is None else cu(rows),
+                                      None if cont is None else cu(cont))
+        assert_exact(to_np(got), want)
+        per = np.add.reduceat(np.concatenate([want, [0]]).astype(np.int64), m.offsets[:-1])[:N]
+        per = np.where(np.diff(m.offsets) > 0, per, 0)
+        assert set(np.unique(per)) <= {0, 2}
+    # the same on the jets of config 2 (long rows, 30-40 objects)
+    j = wl.jets
+    qj = charges(rng, j.pt.size)
+    assert_exact(to_np(hk.select_opposite_sign(cu(j.pt), cu(qj), cu(j.offsets))), hepo.select_opposite_sign(j.pt, qj, j.offsets))
