@@ -508,3 +508,43 @@ int32_t hepo_select_opposite_sign(const float* pt, const int32_t* charge, const 
     }
     return 0;
 }
+
+/* ---- SURVEY.md 8(f-2) ---------------------------------------------------------------------------------- */
+
+int32_t hepo_lookup_interp(const float* x, int64_t n, const float* xs, const float* ys, int32_t nk, float* out)
+{
+    if (n < 0 || nk < 2 || !xs || !ys || (n > 0 && (!x || !out))) return -1;
+    for (int64_t i = 0; i < n; ++i) {
+        const float v = x[i];
+        if (v != v) { out[i] = v; continue; }
+        if (v <= xs[0]) { out[i] = ys[0]; continue; }
+        if (v >= xs[nk - 1]) { out[i] = ys[nk - 1]; continue; }
+        int32_t lo = 0, hi = nk - 1;               /* xs[lo] <= v < xs[hi] */
+        while (hi - lo > 1) {
+            const int32_t mid = (lo + hi) / 2;
+            if (v >= xs[mid]) lo = mid; else hi = mid;
+        }
+        const double x0 = xs[lo], x1 = xs[lo + 1], y0 = ys[lo], y1 = ys[lo + 1];
+        out[i] = (float)(y0 + ((double)v - x0) * (y1 - y0) / (x1 - x0));
+    }
+    return 0;
+}
+
+int32_t hepo_fill_histogram_2d(const float* x, const float* y, const float* weights, int64_t n,
+                               const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                               float* sumw, int64_t* counts)
+{
+    if (n < 0 || nx < 1 || ny < 1 || !edges_x || !edges_y || (n > 0 && (!x || !y))) return -1;
+    const size_t slots = ((size_t)nx + 2) * ((size_t)ny + 2);
+    double* acc = (double*)calloc(slots, sizeof(double));
+    if (!acc) return -1;
+    for (int64_t i = 0; i < n; ++i) {
+        const size_t s = (size_t)hist_slot(x[i], edges_x, nx) * ((size_t)ny + 2) + (size_t)hist_slot(y[i], edges_y, ny);
+        acc[s] += weights ? (double)weights[i] : 1.0;
+        if (counts) counts[s] += 1;
+    }
+    if (sumw)
+        for (size_t s = 0; s < slots; ++s) sumw[s] = (float)((double)sumw[s] + acc[s]);
+    free(acc);
+    return 0;
+}

@@ -138,6 +138,22 @@ int32_t hepo_select_opposite_sign(const float* pt, const int32_t* charge, const 
                                   int64_t content_base, const uint8_t* mask_rows, const uint8_t* mask_content,
                                   uint8_t* out_mask);
 
+/* ---- lookup / histogram variants ------------------------------------------------------
+ *
+ * Linear-interpolated correction ("systematic corrections based on linear interpolations").
+ * Knots xs[0..nk) ascending with values ys[0..nk):  out = ys[b] + (x - xs[b]) * (ys[b+1] - ys[b]) / (xs[b+1] - xs[b])
+ * for xs[b] <= x < xs[b+1], evaluated in float64 and rounded once; x <= xs[0] -> ys[0], x >= xs[nk-1] -> ys[nk-1]
+ * (constant extrapolation), NaN -> NaN.  Tolerance class.  nk >= 2. */
+int32_t hepo_lookup_interp(const float* x, int64_t n, const float* xs, const float* ys, int32_t nk, float* out);
+
+/* Two-dimensional weighted histogram ("Extension to multidimensional histograms is
+ * straightforward").  Slot = sx * (ny + 2) + sy with sx, sy the one-dimensional slots of hepo_fill_histogram
+ * (under/overflow kept per axis, NaN -> overflow); sumw [nx+2][ny+2] accumulates in float64 per call and is added
+ * to the float32 array; counts int64 [nx+2][ny+2]. */
+int32_t hepo_fill_histogram_2d(const float* x, const float* y, const float* weights, int64_t n,
+                               const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                               float* sumw, int64_t* counts);
+
 #ifdef __cplusplus
 }
 #endif

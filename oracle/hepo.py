@@ -161,6 +161,28 @@ def fill_histogram(data, weights, edges, sumw=None, counts=None):
     return sumw, counts
 
 
+def lookup_interp(x, xs, ys):
+    x, xs, ys = _f32(x), _f32(xs), _f32(ys)
+    out = np.empty(x.shape[0], dtype=np.float32)
+    _check(lib().hepo_lookup_interp(_p(x, np.float32), C.c_int64(x.shape[0]), _p(xs, np.float32), _p(ys, np.float32),
+                                    C.c_int32(xs.shape[0]), _p(out, np.float32)))
+    return out
+
+
+def fill_histogram_2d(x, y, weights, edges_x, edges_y, sumw=None, counts=None):
+    """Returns (sumw float32[nx+2][ny+2], counts int64[nx+2][ny+2]); both accumulate into the arrays passed in."""
+    x, y, weights, edges_x, edges_y = _f32(x), _f32(y), _f32(weights), _f32(edges_x), _f32(edges_y)
+    nx, ny = edges_x.shape[0] - 1, edges_y.shape[0] - 1
+    if sumw is None:
+        sumw = np.zeros((nx + 2, ny + 2), dtype=np.float32)
+    if counts is None:
+        counts = np.zeros((nx + 2, ny + 2), dtype=np.int64)
+    _check(lib().hepo_fill_histogram_2d(_p(x, np.float32), _p(y, np.float32), _p(weights, np.float32), C.c_int64(x.shape[0]),
+                                        _p(edges_x, np.float32), C.c_int32(nx), _p(edges_y, np.float32), C.c_int32(ny),
+                                        _p(sumw, np.float32), _p(counts, np.int64)))
+    return sumw, counts
+
+
 class Collection(C.Structure):
     _fields_ = [("offsets", C.c_void_p), ("content_base", C.c_int64), ("n_objects", C.c_int64),
                 ("pt", C.c_void_p), ("eta", C.c_void_p), ("phi", C.c_void_p), ("mass", C.c_void_p)]

@@ -107,3 +107,53 @@ def test_select_opposite_sign_brute_force_and_hand_cases():
     per = np.add.reduceat(np.concatenate([got, [0]]).astype(np.int64), off[:-1])[:800] if m else np.zeros(800)
     per = np.where(np.diff(off) > 0, per, 0)
     assert set(np.unique(per)) <= {0, 2}
+
+
+def test_lookup_interp_against_numpy_and_closed_forms():
+    rng = np.random.default_rng(3)
+    xs = np.sort(rng.uniform(20, 3000, 40)).astype(np.float32)
+    ys = rng.uniform(0.9, 1.1, 40).astype(np.float32)
+    x = np.concatenate([rng.uniform(0, 3500, 20_000), xs, [np.nan, -np.inf, np.inf]]).astype(np.float32)
+    got = hepo.lookup_interp(x, xs, ys).astype(np.float64)
+    want = np.interp(x.astype(np.float64), xs.astype(np.float64), ys.astype(np.float64))
+    fin = ~np.isnan(x)
+    assert np.all(np.abs(got[fin] - want[fin]) <= 1e-6 * np.abs(want[fin]))      # float32 rounding of the float64 value
+    assert np.isnan(got[~fin]).all()
+    np.testing.assert_array_equal(hepo.lookup_interp(xs, xs, ys), ys)             # exact at the knots
+    # a straight line is reproduced, and constant extrapolation holds the end values
+    line = (2.0 + 0.5 * xs.astype(np.float64)).astype(np.float32)
+    mid = (0.5 * (xs[:-1].astype(np.float64) + xs[1:])).astype(np.float32)
+    g = hepo.lookup_interp(mid, xs, line).astype(np.float64)
+    assert np.all(np.abs(g - (2.0 + 0.5 * mid.astype(np.float64))) <= 2e-6 * np.abs(g))
+    assert hepo.lookup_interp(np.float32([1.0]), xs, ys)[0] == ys[0] and hepo.lookup_interp(np.float32([1e9]), xs, ys)[0] == ys[-1]
+
+
+def test_fill_histogram_2d_against_numpy_and_marginals():
+    rng = np.random.default_rng(4)
+    n = 50_000
+    x = rng.normal(0, 1.5, n).astype(np.float32)
+    y = rng.exponential(40, n).astype(np.float32)
+    x[:5] = np.nan
+    w = rng.normal(1, 0.1, n).astype(np.float32)
+    ex = np.linspace(-2.5, 2.5, 21).astype(np.float32)
+    ey = np.geomspace(5, 300, 13).astype(np.float32)
+    sw, ct = hepo.fill_histogram_2d(x, y, w, ex, ey)
+    assert ct.shape == (22, 14) and ct.sum() == n
+    assert abs(sw.astype(np.float64).sum() - w.astype(np.float64).sum()) <= 1e-5 * n
+    # inner bins == numpy (right-open bins; no entry sits exactly on a last edge here)
+    h, _, _ = np.histogram2d(x, y, bins=[ex, ey])
+    np.testing.assert_array_equal(ct[1:-1, 1:-1], h.astype(np.int64))
+    hw, _, _ = np.histogram2d(x[5:], y[5:], bins=[ex, ey], weights=w[5:].astype(np.float64))
+    assert np.all(np.abs(sw[1:-1, 1:-1] - hw) <= 1e-5 * np.abs(hw) + 1e-6)
+    # marginals == the one-dimensional histograms of each axis (flow bins included, NaN -> overflow)
+    sx, cx = hepo.fill_histogram(x, w, ex)
+    sy, cy = hepo.fill_histogram(y, w, ey)
+    np.testing.assert_array_equal(ct.sum(axis=1), cx)
+    np.testing.assert_array_equal(ct.sum(axis=0), cy)
+    assert np.all(np.abs(sw.astype(np.float64).sum(axis=1) - sx) <= 1e-5 * np.abs(sx) + 1e-5)
+    assert ct[-1, :].sum() >= 5                                                    # the NaNs went to x overflow
+    # two calls == one call on the concatenation
+    sw2, ct2 = hepo.fill_histogram_2d(x[: n // 2], y[: n // 2], w[: n // 2], ex, ey)
+    hepo.fill_histogram_2d(x[n // 2:], y[n // 2:], w[n // 2:], ex, ey, sumw=sw2, counts=ct2)
+    np.testing.assert_array_equal(ct2, ct)
+    assert np.all(np.abs(sw2 - sw) <= 1e-5 * np.abs(sw) + 1e-6)
