@@ -346,6 +346,8 @@ def run_single_kernels(args):
     sumw = torch.zeros(edges.numel() + 1, dtype=torch.float32, device="cuda")
     counts = torch.zeros(edges.numel() + 1, dtype=torch.int64, device="cuda")
     scratch = j.pt.clone()
+    sumw2d = torch.zeros((22, 32), dtype=torch.float32, device="cuda")
+    counts2d = torch.zeros((22, 32), dtype=torch.int64, device="cuda")
     charge = torch.randint(0, 2, (Mm,), device="cuda", dtype=torch.int32) * 2 - 1
     cal = inp.calib
     if cal is None:
@@ -366,6 +368,10 @@ def run_single_kernels(args):
         "get_in_offsets[index 0]": (lambda: hk.get_in_offsets(j.pt, j.offsets, 0, fill=0.0), 8 * N + 32 * N + 4 * N),
         "set_in_offsets[index 0]": (lambda: hk.set_in_offsets(scratch, j.offsets, 0, value=1.0), 8 * N + 2 * 32 * N),
         "select_opposite_sign[muons]": (lambda: hk.select_opposite_sign(m.pt, charge, m.offsets), 8 * N + 9 * Mm),
+        # SURVEY.md 8(f-2)
+        "lookup_interp[50 knots]": (lambda: hk.lookup_interp(j.pt, cal["pt_edges"][:50].contiguous(), cal["table"][:50].contiguous()), 8 * Mj),
+        "fill_histogram_2d[20x30]": (lambda: hk.fill_histogram_2d(j.eta, j.pt, None, cal["eta_edges"], cal["pt_edges"][:31].contiguous(),
+                                                                  sumw=sumw2d, counts=counts2d), 8 * Mj),
     }
     out = {}
     for name, (fn, nbytes) in cases.items():

@@ -266,6 +266,27 @@ int32_t hepk_select_opposite_sign(const float* pt, const int32_t* charge, const 
                                   uint8_t* out_mask, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Lookup / histogram variants.  All array pointers are DEVICE pointers.
+ *
+ * Linear-interpolated correction ("systematic corrections based on linear interpolations"):
+ *   knots xs[0..nk) ascending with values ys[0..nk), nk >= 2;
+ *   out[i] = ys[b] + (x[i] - xs[b]) * (ys[b+1] - ys[b]) / (xs[b+1] - xs[b])  for xs[b] <= x[i] < xs[b+1];
+ *   x <= xs[0] -> ys[0], x >= xs[nk-1] -> ys[nk-1] (constant extrapolation), NaN -> NaN.
+ * Tolerance class (float32 evaluation).  8*nk bytes of shared memory, more than 200 KB -> HEPK_ERR_UNSUPPORTED. */
+int32_t hepk_lookup_interp(const float* x, int64_t n, const float* xs, const float* ys, int32_t nk, float* out, void* stream);
+
+/* Two-dimensional weighted histogram ("Extension to multidimensional histograms is straightforward"):
+ *   slot = sx * (ny + 2) + sy, sx / sy the hepk_fill_histogram slots of x / y on their axes (flow bins kept per axis);
+ *   sumw[slot] += w (1 if weights == NULL), counts[slot] += 1.  sumw: float32[(nx+2)*(ny+2)] or NULL,
+ *   counts: int64[(nx+2)*(ny+2)] or NULL; both accumulate.  Bins are privatised per CTA in shared memory and merged
+ *   into float64 accumulators in `workspace` (device, >= hepk_hist2d_workspace_bytes(nx, ny) bytes, needed when sumw
+ *   is given).  (nx+2)*(ny+2) <= 16384, else HEPK_ERR_UNSUPPORTED. */
+size_t  hepk_hist2d_workspace_bytes(int32_t nx, int32_t ny);
+int32_t hepk_fill_histogram_2d(const float* x, const float* y, const float* weights, int64_t n,
+                               const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                               float* sumw, int64_t* counts, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Device-side timing of the dominant kernel (measurement hook for bench.py; no part of the method).
  * Between hepk_profile_begin() and hepk_profile_end() every hepk_analysis_chain call records a CUDA event
  * pair on its launch stream directly around the fused chain kernel (at most 4096 launches are kept).

@@ -230,6 +230,35 @@ def select_opposite_sign(pt, charge, offsets, mask_rows=None, mask_content=None,
     return out
 
 
+def lookup_interp(x, xs, ys, out=None, stream=None):
+    n = x.numel()
+    if out is None:
+        out = torch.empty(n, dtype=torch.float32, device=x.device)
+    _check(lib().hepk_lookup_interp(_ptr(x, torch.float32), C.c_int64(n), _ptr(xs, torch.float32), _ptr(ys, torch.float32),
+                                    C.c_int32(xs.numel()), _ptr(out, torch.float32), _stream(stream)), "lookup_interp")
+    return out
+
+
+def fill_histogram_2d(x, y, weights, edges_x, edges_y, sumw=None, counts=None, want_sumw=True, want_counts=True, stream=None):
+    """Returns (sumw float32[nx+2][ny+2] or None, counts int64[nx+2][ny+2] or None); both accumulate."""
+    nx, ny = edges_x.numel() - 1, edges_y.numel() - 1
+    dev = x.device
+    if sumw is None and want_sumw:
+        sumw = torch.zeros((nx + 2, ny + 2), dtype=torch.float32, device=dev)
+    if counts is None and want_counts:
+        counts = torch.zeros((nx + 2, ny + 2), dtype=torch.int64, device=dev)
+    L = lib()
+    L.hepk_hist2d_workspace_bytes.restype = C.c_size_t
+    nbytes = L.hepk_hist2d_workspace_bytes(C.c_int32(nx), C.c_int32(ny))
+    ws = torch.empty(max(int(nbytes), 8), dtype=torch.uint8, device=dev)
+    _check(L.hepk_fill_histogram_2d(_ptr(x, torch.float32), _ptr(y, torch.float32), _ptr(weights, torch.float32),
+                                    C.c_int64(x.numel()), _ptr(edges_x, torch.float32), C.c_int32(nx),
+                                    _ptr(edges_y, torch.float32), C.c_int32(ny), _ptr(sumw, torch.float32),
+                                    _ptr(counts, torch.int64), C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()),
+                                    _stream(stream)), "fill_histogram_2d")
+    return sumw, counts
+
+
 def lookup_binned(x, y, edges_x, edges_y, table, out=None, stream=None):
     n = x.numel()
     if out is None:

@@ -141,3 +141,144 @@ extern "C" int32_t hepk_select_opposite_sign(const float* pt, const int32_t* cha
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
+
+// ------------------------------------------------------------------------------------------ SURVEY.md 8(f-2)
+// hepk_lookup_interp and hepk_fill_histogram_2d.  Both stream their inputs once
+// (4 B in + 4 B out per element; 8-12 B per entry) with the knots / edges / bins in shared memory.
+namespace hepk {
+namespace dev {
+
+__global__ void __launch_bounds__(256) lookup_interp_kernel(const float* __restrict__ x, long long n, const float* __restrict__ xs,
+                                                            const float* __restrict__ ys, int nk, float* __restrict__ out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* s_x = (float*)smem_raw;
+    float* s_y = s_x + nk;
+    for (int i = threadIdx.x; i < nk; i += blockDim.x) { s_x[i] = xs[i]; s_y[i] = ys[i]; }
+    __syncthreads();
+    const float x_lo = s_x[0], x_hi = s_x[nk - 1];
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float v = __ldg(x + i);
+        float r;
+        if (v != v) r = v;
+        else if (v <= x_lo) r = s_y[0];
+        else if (v >= x_hi) r = s_y[nk - 1];
+        else {
+            int lo = 0, hi = nk - 1;               // s_x[lo] <= v < s_x[hi]
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (v >= s_x[mid]) lo = mid; else hi = mid;
+            }
+            const float x0 = s_x[lo], y0 = s_y[lo];
+            const float t = (v - x0) / (s_x[lo + 1] - x0);      // tolerance class: a few float32 roundings
+            r = fmaf(t, s_y[lo + 1] - y0, y0);
+        }
+        out[i] = r;
+    }
+}
+
+__global__ void __launch_bounds__(256) fill_hist2d_kernel(const float* __restrict__ x, const float* __restrict__ y,
+                                                          const float* __restrict__ w, long long n,
+                                                          const float* __restrict__ edges_x, int nx,
+                                                          const float* __restrict__ edges_y, int ny,
+                                                          double* __restrict__ acc, unsigned long long* __restrict__ counts)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* s_ex = (float*)smem_raw;
+    float* s_ey = s_ex + (nx + 1);
+    float* s_sumw = s_ey + (ny + 1);
+    const int slots = (nx + 2) * (ny + 2);
+    unsigned int* s_cnt = (unsigned int*)(s_sumw + slots);
+    for (int i = threadIdx.x; i <= nx; i += blockDim.x) s_ex[i] = edges_x[i];
+    for (int i = threadIdx.x; i <= ny; i += blockDim.x) s_ey[i] = edges_y[i];
+    for (int i = threadIdx.x; i < slots; i += blockDim.x) { s_sumw[i] = 0.f; s_cnt[i] = 0u; }
+    __syncthreads();
+    const float lox = s_ex[0], invx = (float)nx / (s_ex[nx] - lox);
+    const float loy = s_ey[0], invy = (float)ny / (s_ey[ny] - loy);
+    auto flush = [&]() {
+        __syncthreads();
+        for (int i = threadIdx.x; i < slots; i += blockDim.x) {
+            if (acc) { const float v = s_sumw[i]; if (v != 0.f) { atomicAdd(acc + i, (double)v); s_sumw[i] = 0.f; } }
+            if (counts) { const unsigned int c = s_cnt[i]; if (c) { atomicAdd(counts + i, (unsigned long long)c); s_cnt[i] = 0u; } }
+        }
+        __syncthreads();
+    };
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long iters = (n + stride - 1) / stride;
+    for (long long it = 0; it < iters; ++it) {
+        const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x + it * stride;
+        if (i < n) {
+            const int s = hist_slot(__ldg(x + i), s_ex, nx, lox, invx) * (ny + 2) + hist_slot(__ldg(y + i), s_ey, ny, loy, invy);
+            if (acc) atomicAdd(&s_sumw[s], w ? __ldg(w + i) : 1.f);
+            if (counts) atomicAdd(&s_cnt[s], 1u);
+        }
+        if ((it + 1) % 64 == 0) flush();      // bounded float32 partial sums
+    }
+    flush();
+}
+
+// sumw[i] = float32(float64(sumw[i]) + acc[i])
+__global__ void hist2d_finalize(float* __restrict__ sumw, const double* __restrict__ acc, int n)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) sumw[i] = (float)((double)sumw[i] + acc[i]);
+}
+
+}  // namespace dev
+}  // namespace hepk
+
+extern "C" int32_t hepk_lookup_interp(const float* x, int64_t n, const float* xs, const float* ys, int32_t nk, float* out,
+                                      void* stream)
+{
+    HEPK_REQUIRE(n >= 0, "n < 0");
+    HEPK_REQUIRE(xs && ys && nk >= 2, "knots are NULL or fewer than 2");
+    if ((size_t)nk * 8 > 200 * 1024) {
+        set_error("hepk_lookup_interp: %d knots do not fit 200 KB of shared memory", nk);
+        return HEPK_ERR_UNSUPPORTED;
+    }
+    if (n == 0) return HEPK_OK;
+    HEPK_REQUIRE(x && out, "x/out is NULL");
+    const size_t smem = (size_t)nk * 8;
+    HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::lookup_interp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dev::lookup_interp_kernel<<<grid_for(n), 256, smem, (cudaStream_t)stream>>>(x, n, xs, ys, nk, out);
+    HEPK_CUDA_TRY(cudaGetLastError());
+    return HEPK_OK;
+}
+
+extern "C" size_t hepk_hist2d_workspace_bytes(int32_t nx, int32_t ny)
+{
+    if (nx < 1 || ny < 1) return 0;
+    return (size_t)(nx + 2) * (size_t)(ny + 2) * sizeof(double);
+}
+
+extern "C" int32_t hepk_fill_histogram_2d(const float* x, const float* y, const float* weights, int64_t n,
+                                          const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                                          float* sumw, int64_t* counts, void* workspace, size_t workspace_bytes, void* stream)
+{
+    HEPK_REQUIRE(n >= 0, "n < 0");
+    HEPK_REQUIRE(edges_x && edges_y && nx >= 1 && ny >= 1, "edges are NULL or an axis has no bins");
+    const long long slots = (long long)(nx + 2) * (ny + 2);
+    if (slots > 16384) {
+        set_error("hepk_fill_histogram_2d: (nx+2)*(ny+2) = %lld exceeds 16384", slots);
+        return HEPK_ERR_UNSUPPORTED;
+    }
+    if (n == 0 || (!sumw && !counts)) return HEPK_OK;
+    HEPK_REQUIRE(x && y, "x/y is NULL");
+    if (sumw) {
+        HEPK_REQUIRE(workspace != nullptr, "workspace is NULL");
+        HEPK_REQUIRE(workspace_bytes >= hepk_hist2d_workspace_bytes(nx, ny), "workspace too small");
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t smem = ((size_t)(nx + 1) + (size_t)(ny + 1) + 2 * (size_t)slots) * 4;
+    HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::fill_hist2d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (sumw) HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)slots * sizeof(double), st));
+    unsigned grid = grid_for((n + 3) / 4);
+    dev::fill_hist2d_kernel<<<grid, 256, smem, st>>>(x, y, weights, n, edges_x, nx, edges_y, ny, sumw ? (double*)workspace : nullptr,
+                                                     (unsigned long long*)counts);
+    HEPK_CUDA_TRY(cudaGetLastError());
+    if (sumw) {
+        dev::hist2d_finalize<<<(unsigned)((slots + 255) / 256), 256, 0, st>>>(sumw, (const double*)workspace, (int)slots);
+        HEPK_CUDA_TRY(cudaGetLastError());
+    }
+    return HEPK_OK;
+}

@@ -97,3 +97,47 @@ def test_select_opposite_sign(hk, config, n):
     j = wl.jets
     qj = charges(rng, j.pt.size)
     assert_exact(to_np(hk.select_opposite_sign(cu(j.pt), cu(qj), cu(j.offsets))), hepo.select_opposite_sign(j.pt, qj, j.offsets))
+
+
+def test_lookup_interp(hk):
+    from _util import assert_tol
+    wl = hepgen.generate(2, n_events=200_003)
+    rng = np.random.default_rng(9)
+    xs = np.sort(rng.uniform(20, 600, 30)).astype(np.float32)
+    ys = rng.uniform(0.9, 1.1, 30).astype(np.float32)
+    x = wl.jets.pt.copy()
+    x[:40] = np.resize(xs, 40)                               # exactly on knots
+    x[40:44] = [np.nan, -np.inf, np.inf, 0.0]
+    want = hepo.lookup_interp(x, xs, ys)
+    got = to_np(hk.lookup_interp(cu(x), cu(xs), cu(ys)))
+    assert_tol(got, want, "lookup_interp")
+    assert_exact(got[:40], want[:40], "knots are exact")
+    two = hk.lookup_interp(cu(x), cu(xs[:2]), cu(ys[:2]))    # the smallest table
+    assert_tol(to_np(two), hepo.lookup_interp(x, xs[:2], ys[:2]))
+    with pytest.raises(hk.HepkError):
+        hk.lookup_interp(cu(x), cu(xs[:1]), cu(ys[:1]))
+
+
+@pytest.mark.parametrize("n", [0, 1, 1000, 1_000_003])
+def test_fill_histogram_2d(hk, n):
+    from _util import assert_tol
+    rng = np.random.default_rng(10)
+    x = rng.normal(0, 1.5, n).astype(np.float32)
+    y = (20 + rng.exponential(30, n)).astype(np.float32)
+    if n > 10:
+        x[:3] = np.nan
+        y[3:6] = [np.inf, -np.inf, 500.0]
+        x[6], y[6] = np.float32(2.5), np.float32(20.0)       # on the last x edge -> x overflow
+    w = rng.normal(1, 0.1, n).astype(np.float32)
+    ex = np.linspace(-2.5, 2.5, 21).astype(np.float32)
+    ey = np.geomspace(20, 500, 31).astype(np.float32)         # non-uniform axis
+    for weights in (w, None):
+        sw_ref, ct_ref = hepo.fill_histogram_2d(x, y, weights, ex, ey)
+        sw, ct = hk.fill_histogram_2d(cu(x), cu(y), None if weights is None else cu(w), cu(ex), cu(ey))
+        assert_exact(to_np(ct), ct_ref, "2d counts")
+        assert_tol(to_np(sw), sw_ref, "2d sumw")
+        hk.fill_histogram_2d(cu(x), cu(y), None if weights is None else cu(w), cu(ex), cu(ey), sumw=sw, counts=ct)   # accumulates
+        assert_exact(to_np(ct), 2 * ct_ref)
+        assert_tol(to_np(sw), 2.0 * sw_ref.astype(np.float64))
+    _, only = hk.fill_histogram_2d(cu(x), cu(y), None, cu(ex), cu(ey), want_sumw=False)
+    assert_exact(to_np(only), hepo.fill_histogram_2d(x, y, None, ex, ey)[1])
