@@ -84,6 +84,7 @@ namespace dev {
 struct ChainShared {
     float *edges, *axis_lo, *axis_inv;   // axis_inv == 0: the axis is not uniform enough for the arithmetic bin guess
     float *cal_pt_edges, *cal_eta_edges, *cal_table;
+    float* cal_axis;                     // per calibration axis (pt, eta): [mode (0 search, 1 linear, 2 log2), lo, inv, unused]
     float* h_sumw;                       // int32 fixed point (w * 2^k) when wscale[0] != 0, else float
     unsigned int* h_cnt;
     float* wscale;                       // [0] 2^k or 0, [1] 2^-k
@@ -104,6 +105,7 @@ __host__ __device__ inline size_t chain_shared_layout(const ChainParams& P, bool
     r = take(calib ? (size_t)(P.cal_npt + 1) * 4 : 0, 4); if (s) s->cal_pt_edges = (float*)(base + r);
     r = take(calib ? (size_t)(P.cal_neta + 1) * 4 : 0, 4); if (s) s->cal_eta_edges = (float*)(base + r);
     r = take(calib ? (size_t)P.cal_npt * P.cal_neta * 4 : 0, 4); if (s) s->cal_table = (float*)(base + r);
+    r = take(calib ? 32 : 0, 16); if (s) s->cal_axis = (float*)(base + r);
     const size_t spv = (size_t)P.obs_prefix[HEPK_N_OBS];
     r = take(P.hist_acc ? spv * P.V * P.W * 4 : 0, 4); if (s) s->h_sumw = (float*)(base + r);
     r = take(P.hist_counts ? spv * P.V * 4 : 0, 4); if (s) s->h_cnt = (unsigned int*)(base + r);
@@ -211,6 +213,33 @@ __device__ __forceinline__ int slot_lean(float x, uint32_t edges_a, int nb, floa
     s += (x >= ab.y) ? 1 : 0;
     s -= (x < ab.x) ? 1 : 0;
     return (x != x) ? nb + 1 : s;
+}
+
+// B(v) of the lookup tables (clamped bin, include/hepk.h hepk_lookup_binned) without a search: for an axis the
+// kernel has verified at start-up to be uniform in v (mode 1) or in log2 v (mode 2) to within 0.45 bins, the
+// arithmetic guess lands within one bin of the right one (the log2 approximation is good to 1e-5 bins), and one
+// +-1 step against the edges makes it exact.  mode 0: binary search.
+__device__ __forceinline__ int find_bin_fast(float v, uint32_t edges_a, int n, uint32_t axis_a)
+{
+    const float mode = lds_f32(axis_a);
+    if (mode == 0.0f) {
+        if (v < lds_f32(edges_a)) return 0;
+        if (!(v < lds_f32(edges_a + 4u * (unsigned)n))) return n - 1;
+        int lo = 0, hi = n;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (v >= lds_f32(edges_a + 4u * (unsigned)mid)) lo = mid; else hi = mid;
+        }
+        return lo;
+    }
+    const float pos = mode == 1.0f ? v : __log2f(v);
+    int g = (int)((pos - lds_f32(axis_a + 4u)) * lds_f32(axis_a + 8u));       // NaN -> 0, +-inf saturate
+    g = max(0, min(g, n - 1));
+    const float a = lds_f32(edges_a + 4u * (unsigned)g), b = lds_f32(edges_a + 4u * (unsigned)g + 4u);
+    g += (v >= b) ? 1 : 0;
+    g -= (v < a) ? 1 : 0;
+    g = max(0, min(g, n - 1));
+    return (v != v) ? n - 1 : g;
 }
 
 // dR^2, exact class.  Same value as dr2_exact: with a = |dphi| and t = a - 2PI_F, the wrapped magnitude is
@@ -670,6 +699,29 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             S.axis_inv[ob] = ok ? inv : 0.0f;
         }
     }
+    if (CALIB) {
+#pragma unroll
+        for (int ax = 0; ax < 2; ++ax) {
+            const float* ed = ax == 0 ? S.cal_pt_edges : S.cal_eta_edges;
+            const int nb = ax == 0 ? P.cal_npt : P.cal_neta;
+            const float lo = ed[0], hi = ed[nb];
+            const float inv1 = (float)nb / (hi - lo);
+            const float l0 = __log2f(lo), inv2 = (float)nb / (__log2f(hi) - l0);
+            bool ok1 = (hi > lo) && (inv1 > 0.0f) && (inv1 < CUDART_INF_F);
+            bool ok2 = (lo > 0.0f) && (hi > lo) && (inv2 > 0.0f) && (inv2 < CUDART_INF_F);
+            for (int i = tid; i <= nb; i += nthr) {
+                ok1 = ok1 && (fabsf((ed[i] - lo) * inv1 - (float)i) <= 0.45f);
+                ok2 = ok2 && (fabsf((__log2f(ed[i]) - l0) * inv2 - (float)i) <= 0.45f);
+            }
+            ok1 = __syncthreads_and(ok1);
+            ok2 = __syncthreads_and(ok2);
+            if (tid == 0) {
+                S.cal_axis[4 * ax + 0] = ok1 ? 1.0f : (ok2 ? 2.0f : 0.0f);
+                S.cal_axis[4 * ax + 1] = ok1 ? lo : l0;
+                S.cal_axis[4 * ax + 2] = ok1 ? inv1 : inv2;
+            }
+        }
+    }
     LaneCol col;
     col.ptr = nullptr; col.off = nullptr; col.base = 0; col.n = 0; col.mis = 0; col.cap = 0; col.dst = 0;
     if (lane < P.n_col) {
@@ -839,9 +891,9 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     if (!CALIB) {
                         sts_f32(aj, (base_ok && (pt > P.jet_pt_min)) ? pt : -CUDART_INF_F);
                     } else {
-                        const int bx = find_bin_clamped(pt, S.cal_pt_edges, P.cal_npt);
-                        const int by = find_bin_clamped(eta, S.cal_eta_edges, P.cal_neta);
-                        sts_f32(aj + d_corr0, S.cal_table[bx * P.cal_neta + by]);
+                        const int bx = find_bin_fast(pt, smem_u32(S.cal_pt_edges), P.cal_npt, smem_u32(S.cal_axis));
+                        const int by = find_bin_fast(eta, smem_u32(S.cal_eta_edges), P.cal_neta, smem_u32(S.cal_axis) + 16u);
+                        sts_f32(aj + d_corr0, lds_f32(smem_u32(S.cal_table) + 4u * (unsigned)(bx * P.cal_neta + by)));
                         if (!base_ok) sts_f32(aj, CUDART_NAN_F);
                     }
                 }

@@ -208,6 +208,28 @@ def test_chain_irregular_axes_and_odd_weights(hk):
     assert_exact(to_np(out["hist_counts"]), ref["hist_counts"])
 
 
+def test_chain_calibration_axis_modes(hk):
+    """Calibration tables on a log-spaced x uniform grid (arithmetic bin guess), on irregular edges (binary search),
+    and with jets sitting exactly on edges and outside the table."""
+    rng = np.random.default_rng(21)
+    for kind in ("regular", "irregular", "linear_pt"):
+        wl = hepgen.generate(3, n_events=30_000, seed=22)
+        if kind == "irregular":
+            wl.calib["pt_edges"] = np.unique(np.concatenate([[20.0], np.sort(rng.uniform(20, 3000, 49)), [3000.0]])).astype(np.float32)
+            wl.calib["eta_edges"] = np.unique(np.concatenate([[-2.5], np.sort(rng.uniform(-2.5, 2.5, 19)), [2.5]])).astype(np.float32)
+            wl.calib["table"] = rng.uniform(0.9, 1.1, (wl.calib["pt_edges"].size - 1, wl.calib["eta_edges"].size - 1)).astype(np.float32)
+        if kind == "linear_pt":
+            wl.calib["pt_edges"] = np.linspace(25.0, 400.0, 51).astype(np.float32)     # jets below and above the table
+        pe, ee = wl.calib["pt_edges"], wl.calib["eta_edges"]
+        k = rng.integers(0, wl.jets.pt.size, 4000)
+        wl.jets.pt[k] = pe[rng.integers(0, pe.size, 4000)]                             # exactly on pt edges
+        k = rng.integers(0, wl.jets.pt.size, 4000)
+        wl.jets.eta[k] = ee[rng.integers(0, ee.size, 4000)]                            # exactly on eta edges
+        ref = hepo.analysis_chain(wl)
+        out, _ = run_gpu(hk, wl)
+        compare(out, ref, wl, what=f"calib {kind} ")
+
+
 def test_chain_optional_outputs(hk):
     wl = hepgen.generate(1, n_events=20_000)
     ref = hepo.analysis_chain(wl, want_mask=False)
