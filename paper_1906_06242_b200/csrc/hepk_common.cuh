@@ -173,6 +173,46 @@ __device__ __forceinline__ int find_bin_clamped(float v, const float* edges, int
     return lo;
 }
 
+// ---- lookup axes without a search --------------------------------------------------------------------
+// An axis whose edges are uniform in v (mode 1) or in log2 v (mode 2) to within 0.45 bins lets B(v) be guessed
+// arithmetically to within one bin (the log2 approximation is good to ~1e-5 bins) and fixed with one +-1 step
+// against the edges, which makes the result exact.  classify_axis is called by ALL threads of the CTA (it uses
+// __syncthreads_and) on edges already staged in shared memory.
+struct AxisGuess { int mode; float lo, inv; };      // mode 0: binary search
+
+__device__ __forceinline__ AxisGuess classify_axis(const float* s_edges, int n)
+{
+    const float lo = s_edges[0], hi = s_edges[n];
+    const float inv1 = (float)n / (hi - lo);
+    const float l0 = __log2f(lo), inv2 = (float)n / (__log2f(hi) - l0);
+    bool ok1 = (hi > lo) && (inv1 > 0.0f) && (inv1 < CUDART_INF_F);
+    bool ok2 = (lo > 0.0f) && (hi > lo) && (inv2 > 0.0f) && (inv2 < CUDART_INF_F);
+    for (int i = threadIdx.x; i <= n; i += blockDim.x) {
+        ok1 = ok1 && (fabsf((s_edges[i] - lo) * inv1 - (float)i) <= 0.45f);
+        ok2 = ok2 && (fabsf((__log2f(s_edges[i]) - l0) * inv2 - (float)i) <= 0.45f);
+    }
+    ok1 = __syncthreads_and(ok1);
+    ok2 = __syncthreads_and(ok2);
+    AxisGuess a;
+    a.mode = ok1 ? 1 : (ok2 ? 2 : 0);
+    a.lo = ok1 ? lo : l0;
+    a.inv = ok1 ? inv1 : inv2;
+    return a;
+}
+
+__device__ __forceinline__ int find_bin_guess(float v, const float* edges, int n, const AxisGuess& a)
+{
+    if (a.mode == 0) return find_bin_clamped(v, edges, n);
+    const float pos = a.mode == 1 ? v : __log2f(v);
+    int g = (int)((pos - a.lo) * a.inv);              // NaN -> 0, +-inf saturate
+    g = max(0, min(g, n - 1));
+    const float e0 = edges[g], e1 = edges[g + 1];
+    g += (v >= e1) ? 1 : 0;
+    g -= (v < e0) ? 1 : 0;
+    g = max(0, min(g, n - 1));
+    return (v != v) ? n - 1 : g;
+}
+
 // Histogram slot: 0 underflow, 1+b, nbins+1 overflow/NaN.  Arithmetic guess for (near-)uniform axes,
 // verified against the edges; anything the guess gets wrong falls back to the binary search, so the
 // result is exact for any ascending edges.

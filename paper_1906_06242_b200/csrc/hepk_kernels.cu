@@ -74,9 +74,13 @@ __global__ void __launch_bounds__(256) lookup_kernel(const float* __restrict__ x
     if (y) for (int i = threadIdx.x; i <= ny; i += blockDim.x) s_ey[i] = edges_y[i];
     for (int i = threadIdx.x; i < nx * nyy; i += blockDim.x) s_t[i] = table[i];
     __syncthreads();
+    const AxisGuess ax = classify_axis(s_ex, nx);
+    AxisGuess ay;
+    ay.mode = 0; ay.lo = 0.f; ay.inv = 0.f;
+    if (y) ay = classify_axis(s_ey, ny);
     auto look = [&](float xv, float yv) {
-        const int bx = find_bin_clamped(xv, s_ex, nx);
-        const int by = y ? find_bin_clamped(yv, s_ey, ny) : 0;
+        const int bx = find_bin_guess(xv, s_ex, nx, ax);
+        const int by = y ? find_bin_guess(yv, s_ey, ny, ay) : 0;
         return s_t[bx * nyy + by];
     };
     const long long stride = (long long)gridDim.x * blockDim.x;

@@ -321,6 +321,17 @@ def test_lookup_binned(hk, wl2):
     want = hepo.lookup_binned(xs, None, cal["pt_edges"], None, t1)
     got = hk.lookup_binned(misaligned(xs, 3), None, dev(cal["pt_edges"]), None, dev(t1))
     assert_exact(to_np(got), want)
+    # irregular edges (binary-search path) and a uniform pt axis (linear guess)
+    rng = np.random.default_rng(4)
+    pe = np.unique(np.concatenate([[20.0], np.sort(rng.uniform(20, 3000, 37)), [3000.0]])).astype(np.float32)
+    tab = rng.uniform(0.9, 1.1, (pe.size - 1, 20)).astype(np.float32)
+    x[100:100 + pe.size] = pe
+    assert_exact(to_np(hk.lookup_binned(dev(x), dev(y), dev(pe), dev(cal["eta_edges"]), dev(tab))),
+                 hepo.lookup_binned(x, y, pe, cal["eta_edges"], tab))
+    pl = np.linspace(25.0, 500.0, 51).astype(np.float32)
+    x[200:251] = pl
+    assert_exact(to_np(hk.lookup_binned(dev(x), dev(y), dev(pl), dev(cal["eta_edges"]), dev(cal["table"]))),
+                 hepo.lookup_binned(x, y, pl, cal["eta_edges"], cal["table"]))
 
 
 # --------------------------------------------------------------------------- fill_histogram
