@@ -548,3 +548,54 @@ int32_t hepo_fill_histogram_2d(const float* x, const float* y, const float* weig
     free(acc);
     return 0;
 }
+
+/* ---- SURVEY.md 8(f-3) ---------------------------------------------------------------------------------- */
+
+int32_t hepo_triplet_mass(const float* pt, const float* eta, const float* phi, const float* mass,
+                          const int64_t* offsets, int64_t n_events, int64_t content_base,
+                          const uint8_t* mask_rows, const uint8_t* mask_content, float target,
+                          float* out_mass, int32_t* out_idx)
+{
+    if (!seg_args_ok(offsets, n_events, out_mass)) return -1;
+    for (int64_t e = 0; e < n_events; ++e) {
+        out_mass[e] = 0.0f;
+        if (out_idx) { out_idx[3 * e] = out_idx[3 * e + 1] = out_idx[3 * e + 2] = -1; }
+        if (mask_rows && !mask_rows[e]) continue;
+        const int64_t g0 = offsets[e], g1 = offsets[e + 1];
+        double best = 0.0, best_m = 0.0;
+        int have = 0;
+        for (int64_t a = g0; a < g1; ++a) {
+            if (mask_content && !mask_content[a - content_base]) continue;
+            for (int64_t b = a + 1; b < g1; ++b) {
+                if (mask_content && !mask_content[b - content_base]) continue;
+                for (int64_t c = b + 1; c < g1; ++c) {
+                    if (mask_content && !mask_content[c - content_base]) continue;
+                    const int64_t id[3] = {a - content_base, b - content_base, c - content_base};
+                    double E = 0, px = 0, py = 0, pz = 0;
+                    for (int t = 0; t < 3; ++t) {
+                        const double p = pt[id[t]], m = mass[id[t]];
+                        const double ch = cosh((double)eta[id[t]]);
+                        px += p * cos((double)phi[id[t]]);
+                        py += p * sin((double)phi[id[t]]);
+                        pz += p * sinh((double)eta[id[t]]);
+                        E += sqrt(p * p * ch * ch + m * m);
+                    }
+                    double m2 = E * E - px * px - py * py - pz * pz;
+                    if (!(m2 > 0.0)) m2 = 0.0;
+                    const double M = sqrt(m2);
+                    const double d = fabs(M - (double)target);
+                    if (!have || d < best) {            /* strict <: the first triplet in (i, j, k) order wins ties */
+                        have = 1; best = d; best_m = M;
+                        if (out_idx) {
+                            out_idx[3 * e] = (int32_t)(a - g0);
+                            out_idx[3 * e + 1] = (int32_t)(b - g0);
+                            out_idx[3 * e + 2] = (int32_t)(c - g0);
+                        }
+                    }
+                }
+            }
+        }
+        if (have) out_mass[e] = (float)best_m;
+    }
+    return 0;
+}

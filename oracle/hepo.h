@@ -154,6 +154,20 @@ int32_t hepo_fill_histogram_2d(const float* x, const float* y, const float* weig
                                const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
                                float* sumw, int64_t* counts);
 
+/* ---- jet-triplet candidate -------------------------------------------------------------
+ *
+ * PAPER.md:L136 "high-level variable reconstruction: top quark candidate from jet triplet with invariant mass
+ * closest to M = 172 GeV".  Per event, over all triplets i < j < k of the objects with mask_content set (local
+ * indices): M_ijk = sqrt(max(0, (E_i+E_j+E_k)^2 - |p_i+p_j+p_k|^2)) from the four-vectors of hepo_pair_invmass
+ * (float64), and the triplet minimising |M_ijk - target| is kept; among equal distances the lexicographically
+ * first (i, j, k).  out_mass = (float)M of that triplet, out_idx[3*e..] its local indices; fewer than three
+ * selected objects (or mask_rows clear): mass 0.0f, indices -1.  (The formula, the tie rule and the "< 3" value
+ * are readings: the paper gives one phrase.)  Tolerance class; which triplet wins is decided in float64 here. */
+int32_t hepo_triplet_mass(const float* pt, const float* eta, const float* phi, const float* mass,
+                          const int64_t* offsets, int64_t n_events, int64_t content_base,
+                          const uint8_t* mask_rows, const uint8_t* mask_content, float target,
+                          float* out_mass, int32_t* out_idx);
+
 #ifdef __cplusplus
 }
 #endif

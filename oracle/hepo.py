@@ -183,6 +183,19 @@ def fill_histogram_2d(x, y, weights, edges_x, edges_y, sumw=None, counts=None):
     return sumw, counts
 
 
+def triplet_mass(pt, eta, phi, mass, offsets, target, mask_rows=None, mask_content=None, content_base=0):
+    """Returns (mass float32[n_events], indices int32[n_events][3])."""
+    pt, eta, phi, mass, offsets = _f32(pt), _f32(eta), _f32(phi), _f32(mass), _i64(offsets)
+    mask_rows, mask_content = _u8(mask_rows), _u8(mask_content)
+    n = offsets.shape[0] - 1
+    out = np.zeros(n, dtype=np.float32)
+    idx = np.full((n, 3), -1, dtype=np.int32)
+    _check(lib().hepo_triplet_mass(_p(pt, np.float32), _p(eta, np.float32), _p(phi, np.float32), _p(mass, np.float32),
+                                   _p(offsets, np.int64), C.c_int64(n), C.c_int64(content_base), _p(mask_rows, np.uint8),
+                                   _p(mask_content, np.uint8), C.c_float(target), _p(out, np.float32), _p(idx, np.int32)))
+    return out, idx
+
+
 class Collection(C.Structure):
     _fields_ = [("offsets", C.c_void_p), ("content_base", C.c_int64), ("n_objects", C.c_int64),
                 ("pt", C.c_void_p), ("eta", C.c_void_p), ("phi", C.c_void_p), ("mass", C.c_void_p)]

@@ -157,3 +157,49 @@ def test_fill_histogram_2d_against_numpy_and_marginals():
     hepo.fill_histogram_2d(x[n // 2:], y[n // 2:], w[n // 2:], ex, ey, sumw=sw2, counts=ct2)
     np.testing.assert_array_equal(ct2, ct)
     assert np.all(np.abs(sw2 - sw) <= 1e-5 * np.abs(sw) + 1e-6)
+
+
+def test_triplet_mass_closed_forms_and_brute_force():
+    import itertools
+    # closed form: three massless jets at eta = 0, phi = 0, 2pi/3, 4pi/3 with equal pt: total momentum 0, M = 3 pt
+    phi = np.float32([0.0, 2 * np.pi / 3, 4 * np.pi / 3 - 2 * np.pi])
+    pt = np.float32([50, 50, 50]); z = np.zeros(3, np.float32)
+    m, idx = hepo.triplet_mass(pt, z, phi, z, np.int64([0, 3]), 172.0)
+    assert abs(m[0] - 150.0) < 1e-3 and list(idx[0]) == [0, 1, 2]
+    # three identical four-vectors: M = 3 m
+    m, _ = hepo.triplet_mass(np.float32([40] * 3), np.float32([0.7] * 3), np.float32([1.1] * 3), np.float32([5.0] * 3), np.int64([0, 3]), 172.0)
+    assert abs(m[0] - 15.0) < 1e-4
+    # fewer than three (selected) objects
+    m, idx = hepo.triplet_mass(pt, z, phi, z, np.int64([0, 2, 3]), 172.0)
+    assert (m == 0).all() and (idx == -1).all()
+    m, idx = hepo.triplet_mass(pt, z, phi, z, np.int64([0, 3]), 172.0, mask_content=np.uint8([1, 0, 1]))
+    assert m[0] == 0 and (idx == -1).all()
+    # brute force with numpy float64 four-vectors on random events
+    rng = np.random.default_rng(6)
+    off = _jagged(rng, 300, 4.5, cap=9)
+    n = int(off[-1])
+    pt = (20 + rng.exponential(30, n)).astype(np.float32)
+    eta = rng.uniform(-2.5, 2.5, n).astype(np.float32)
+    phi = rng.uniform(-np.pi, np.pi, n).astype(np.float32)
+    mass = rng.exponential(10, n).astype(np.float32)
+    mc = rng.random(n) < 0.8
+    got_m, got_i = hepo.triplet_mass(pt, eta, phi, mass, off, 172.0, mask_content=mc)
+    p64, e64, f64, m64 = (a.astype(np.float64) for a in (pt, eta, phi, mass))
+    vec = np.stack([np.sqrt(p64 ** 2 * np.cosh(e64) ** 2 + m64 ** 2), p64 * np.cos(f64), p64 * np.sin(f64), p64 * np.sinh(e64)], axis=1)
+    for e in range(300):
+        sel = [i for i in range(off[e], off[e + 1]) if mc[i]]
+        if len(sel) < 3:
+            assert got_m[e] == 0 and (got_i[e] == -1).all()
+            continue
+        best = None
+        for tri in itertools.combinations(sel, 3):
+            v = vec[list(tri)].sum(axis=0)
+            M = np.sqrt(max(v[0] ** 2 - v[1] ** 2 - v[2] ** 2 - v[3] ** 2, 0.0))
+            if best is None or abs(M - 172.0) < best[0]:
+                best = (abs(M - 172.0), M, tri)
+        assert abs(got_m[e] - best[1]) <= 1e-5 * best[1] + 1e-6
+        assert tuple(got_i[e] + off[e]) == best[2]
+    # invariance of the chosen mass under a common phi rotation
+    rot = ((phi + np.float32(0.9) + np.pi) % (2 * np.pi) - np.pi).astype(np.float32)
+    rm, _ = hepo.triplet_mass(pt, eta, rot, mass, off, 172.0, mask_content=mc)
+    assert np.all(np.abs(rm - got_m) <= 2e-4 * np.abs(got_m) + 1e-4)
