@@ -368,6 +368,8 @@ def run_single_kernels(args):
         "get_in_offsets[index 0]": (lambda: hk.get_in_offsets(j.pt, j.offsets, 0, fill=0.0), 8 * N + 32 * N + 4 * N),
         "set_in_offsets[index 0]": (lambda: hk.set_in_offsets(scratch, j.offsets, 0, value=1.0), 8 * N + 2 * 32 * N),
         "select_opposite_sign[muons]": (lambda: hk.select_opposite_sign(m.pt, charge, m.offsets), 8 * N + 9 * Mm),
+        # ALU-bound on long events; bytes are the selected jets' four columns + offsets + outputs
+        "triplet_mass[selected jets]": (lambda: hk.triplet_mass(j.pt, j.eta, j.phi, j.mass, j.offsets, 172.0, None, jsel), 8 * N + 17 * Mj + 16 * N),
         # SURVEY.md 8(f-2)
         "lookup_interp[50 knots]": (lambda: hk.lookup_interp(j.pt, cal["pt_edges"][:50].contiguous(), cal["table"][:50].contiguous()), 8 * Mj),
         "fill_histogram_2d[20x30]": (lambda: hk.fill_histogram_2d(j.eta, j.pt, None, cal["eta_edges"], cal["pt_edges"][:31].contiguous(),

@@ -287,6 +287,19 @@ int32_t hepk_fill_histogram_2d(const float* x, const float* y, const float* weig
                                float* sumw, int64_t* counts, void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Jet-triplet candidate ("top quark candidate from jet triplet with invariant
+ * mass closest to M = 172 GeV").  Per event, over all triplets i < j < k of the objects with mask_content set:
+ *   M_ijk = sqrt(max(0, (E_i+E_j+E_k)^2 - |p_i+p_j+p_k|^2)), four-vectors as in hepk_pair_invmass, float64;
+ *   the triplet minimising |M_ijk - target| is kept (equal distances: the lexicographically first (i, j, k)).
+ * out_mass[e] = (float)M of that triplet; out_idx[3e..3e+2] its local indices (may be NULL); fewer than three
+ * selected objects or mask_rows clear: 0.0f and -1.  Tolerance class: when two triplets are equally close to
+ * within the float64 rounding of the transcendental functions, either is a valid answer.
+ * All array pointers are DEVICE pointers. */
+int32_t hepk_triplet_mass(const float* pt, const float* eta, const float* phi, const float* mass,
+                          const int64_t* offsets, int64_t n_events, int64_t content_base, const uint8_t* mask_rows,
+                          const uint8_t* mask_content, float target, float* out_mass, int32_t* out_idx, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Device-side timing of the dominant kernel (measurement hook for bench.py; no part of the method).
  * Between hepk_profile_begin() and hepk_profile_end() every hepk_analysis_chain call records a CUDA event
  * pair on its launch stream directly around the fused chain kernel (at most 4096 launches are kept).

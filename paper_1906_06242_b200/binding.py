@@ -259,6 +259,20 @@ def fill_histogram_2d(x, y, weights, edges_x, edges_y, sumw=None, counts=None, w
     return sumw, counts
 
 
+def triplet_mass(pt, eta, phi, mass, offsets, target, mask_rows=None, mask_content=None, content_base=0, want_indices=True,
+                 stream=None):
+    """Returns (mass float32[n_events], indices int32[n_events][3] or None)."""
+    n = offsets.numel() - 1
+    out = torch.empty(n, dtype=torch.float32, device=offsets.device)
+    idx = torch.empty((n, 3), dtype=torch.int32, device=offsets.device) if want_indices else None
+    _check(lib().hepk_triplet_mass(_ptr(pt, torch.float32), _ptr(eta, torch.float32), _ptr(phi, torch.float32),
+                                   _ptr(mass, torch.float32), _ptr(offsets, torch.int64), C.c_int64(n), C.c_int64(content_base),
+                                   _ptr(_mask(mask_rows), torch.uint8), _ptr(_mask(mask_content), torch.uint8),
+                                   C.c_float(target), _ptr(out, torch.float32), _ptr(idx, torch.int32), _stream(stream)),
+           "triplet_mass")
+    return out, idx
+
+
 def lookup_binned(x, y, edges_x, edges_y, table, out=None, stream=None):
     n = x.numel()
     if out is None:

@@ -282,3 +282,139 @@ extern "C" int32_t hepk_fill_histogram_2d(const float* x, const float* y, const 
     }
     return HEPK_OK;
 }
+
+// ------------------------------------------------------------------------------------------ SURVEY.md 8(f-3)
+// hepk_triplet_mass: one warp per event.  The selected jets' four-vectors are built once per event
+// (one lane per jet, float64) into shared memory; lanes then take the (a, b) pairs round-robin and run over c > b,
+// so every triplet costs four float64 adds, four multiply-adds and a square root; the best triplet per lane is
+// reduced over the warp by (distance, a, b, c).  ALU-bound on long events, launch/latency-bound on short ones.
+namespace hepk {
+namespace dev {
+
+constexpr int TRIPLET_CAP = 96;      // selected jets of one event held in shared memory (more: recomputed on the fly)
+constexpr int TRIPLET_WARPS = 4;
+
+struct Vec4 { double e, x, y, z; };
+
+__device__ __forceinline__ Vec4 four_vector(float pt, float eta, float phi, float m)
+{
+    const double p = pt, mm = m;
+    double s, c;
+    sincos((double)phi, &s, &c);
+    const double ch = cosh((double)eta);
+    Vec4 v;
+    v.e = sqrt(p * p * ch * ch + mm * mm);
+    v.x = p * c; v.y = p * s; v.z = p * sinh((double)eta);
+    return v;
+}
+
+__global__ void __launch_bounds__(32 * TRIPLET_WARPS) triplet_kernel(const float* __restrict__ pt, const float* __restrict__ eta,
+                                                                      const float* __restrict__ phi, const float* __restrict__ mass,
+                                                                      const long long* __restrict__ offsets, long long n_events,
+                                                                      long long base, const unsigned char* __restrict__ mask_rows,
+                                                                      const unsigned char* __restrict__ mask_content, float target,
+                                                                      float* __restrict__ out_mass, int* __restrict__ out_idx)
+{
+    __shared__ Vec4 s_vec[TRIPLET_WARPS][TRIPLET_CAP];
+    __shared__ int s_loc[TRIPLET_WARPS][TRIPLET_CAP];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    Vec4* vec = s_vec[warp];
+    int* loc = s_loc[warp];
+    const long long nw = (long long)gridDim.x * TRIPLET_WARPS;
+    for (long long e = (long long)blockIdx.x * TRIPLET_WARPS + warp; e < n_events; e += nw) {
+        const long long g0 = __ldg(offsets + e), g1 = __ldg(offsets + e + 1);
+        const bool row = !mask_rows || mask_rows[e];
+        // ---- selected jets -> local index list (and four-vectors while they fit)
+        int nsel = 0;
+        if (row) {
+            for (long long c0 = g0; c0 < g1; c0 += 32) {
+                const long long g = c0 + lane;
+                const bool sel = g < g1 && (!mask_content || mask_content[g - base]);
+                const unsigned m = __ballot_sync(0xffffffffu, sel);
+                const int at = nsel + __popc(m & ((1u << lane) - 1u));
+                if (sel && at < TRIPLET_CAP) {
+                    const long long i = g - base;
+                    loc[at] = (int)(g - g0);
+                    vec[at] = four_vector(__ldg(pt + i), __ldg(eta + i), __ldg(phi + i), __ldg(mass + i));
+                }
+                nsel += __popc(m);
+            }
+        }
+        __syncwarp();
+        const bool cached = nsel <= TRIPLET_CAP;
+        // local index and four-vector of the s-th selected jet (slow way when the event does not fit the cache)
+        auto local_of = [&](int s) -> int {
+            if (cached) return loc[s];
+            int seen = 0;
+            for (long long g = g0; g < g1; ++g)
+                if (!mask_content || mask_content[g - base]) { if (seen == s) return (int)(g - g0); ++seen; }
+            return -1;
+        };
+        auto vec_of = [&](int s) -> Vec4 {
+            if (cached) return vec[s];
+            const long long i = g0 - base + local_of(s);
+            return four_vector(__ldg(pt + i), __ldg(eta + i), __ldg(phi + i), __ldg(mass + i));
+        };
+        // ---- triplets: lane takes pairs (a, b) round-robin, runs over c
+        double best = CUDART_INF;
+        double best_m = 0.0;
+        int ba = 0x7fffffff, bb = 0x7fffffff, bc = 0x7fffffff;
+        const long long npairs = (long long)nsel * (nsel - 1) / 2;
+        for (long long p = lane; p < npairs; p += 32) {
+            int a = 0;
+            long long r = p;
+            while (r >= nsel - 1 - a) { r -= nsel - 1 - a; ++a; }
+            const int b = a + 1 + (int)r;
+            const Vec4 va = vec_of(a), vb = vec_of(b);
+            const double e2 = va.e + vb.e, x2 = va.x + vb.x, y2 = va.y + vb.y, z2 = va.z + vb.z;
+            for (int c = b + 1; c < nsel; ++c) {
+                const Vec4 vc = vec_of(c);
+                const double E = e2 + vc.e, X = x2 + vc.x, Y = y2 + vc.y, Z = z2 + vc.z;
+                double m2 = E * E - X * X - Y * Y - Z * Z;
+                if (!(m2 > 0.0)) m2 = 0.0;
+                const double M = sqrt(m2);
+                const double d = fabs(M - (double)target);
+                if (d < best) { best = d; best_m = M; ba = a; bb = b; bc = c; }     // visited in (a, b, c) order per lane
+            }
+        }
+        // ---- warp argmin by (distance, a, b, c)
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) {
+            const double od = __shfl_xor_sync(0xffffffffu, best, o);
+            const double om = __shfl_xor_sync(0xffffffffu, best_m, o);
+            const int oa = __shfl_xor_sync(0xffffffffu, ba, o), ob = __shfl_xor_sync(0xffffffffu, bb, o),
+                      oc = __shfl_xor_sync(0xffffffffu, bc, o);
+            const bool take = od < best || (od == best && (oa < ba || (oa == ba && (ob < bb || (ob == bb && oc < bc)))));
+            if (take) { best = od; best_m = om; ba = oa; bb = ob; bc = oc; }
+        }
+        if (lane == 0) {
+            const bool have = nsel >= 3;
+            out_mass[e] = have ? (float)best_m : 0.0f;
+            if (out_idx) {
+                out_idx[3 * e] = have ? local_of(ba) : -1;
+                out_idx[3 * e + 1] = have ? local_of(bb) : -1;
+                out_idx[3 * e + 2] = have ? local_of(bc) : -1;
+            }
+        }
+        __syncwarp();
+    }
+}
+
+}  // namespace dev
+}  // namespace hepk
+
+extern "C" int32_t hepk_triplet_mass(const float* pt, const float* eta, const float* phi, const float* mass,
+                                     const int64_t* offsets, int64_t n_events, int64_t content_base, const uint8_t* mask_rows,
+                                     const uint8_t* mask_content, float target, float* out_mass, int32_t* out_idx, void* stream)
+{
+    HEPK_REQUIRE(n_events >= 0, "n_events < 0");
+    if (n_events == 0) return HEPK_OK;
+    HEPK_REQUIRE(offsets && out_mass, "offsets/out_mass is NULL");
+    long long blocks = (n_events + dev::TRIPLET_WARPS - 1) / dev::TRIPLET_WARPS;
+    const long long maxb = (long long)sm_count() * 12;
+    if (blocks > maxb) blocks = maxb;
+    dev::triplet_kernel<<<(unsigned)blocks, 32 * dev::TRIPLET_WARPS, 0, (cudaStream_t)stream>>>(
+        pt, eta, phi, mass, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, target, out_mass, out_idx);
+    HEPK_CUDA_TRY(cudaGetLastError());
+    return HEPK_OK;
+}

@@ -141,3 +141,66 @@ def test_fill_histogram_2d(hk, n):
         assert_tol(to_np(sw), 2.0 * sw_ref.astype(np.float64))
     _, only = hk.fill_histogram_2d(cu(x), cu(y), None, cu(ex), cu(ey), want_sumw=False)
     assert_exact(to_np(only), hepo.fill_histogram_2d(x, y, None, ex, ey)[1])
+
+
+def _triplet_check(got_m, got_i, ref_m, ref_i, pt, eta, phi, mass, off, sel, target):
+    """Tolerance-class comparison of an argmin: the distance reached must equal the oracle's within tolerance, the
+    returned triplet must be a valid one whose float64 mass is the returned mass; indices equal except at near-ties."""
+    n = off.size - 1
+    p, e, f, m = (a.astype(np.float64) for a in (pt, eta, phi, mass))
+    vec = np.stack([np.sqrt(p ** 2 * np.cosh(e) ** 2 + m ** 2), p * np.cos(f), p * np.sin(f), p * np.sinh(e)], axis=1)
+    none = ref_i[:, 0] < 0
+    assert_exact(got_i[none], ref_i[none], "events without a triplet")
+    assert (got_m[none] == 0).all()
+    ok = ~none
+    gi = got_i[ok].astype(np.int64) + off[:-1][ok, None]
+    assert (got_i[ok][:, 0] < got_i[ok][:, 1]).all() and (got_i[ok][:, 1] < got_i[ok][:, 2]).all()
+    assert (gi < off[1:][ok, None]).all()
+    if sel is not None:
+        assert sel[gi].all()
+    v = vec[gi].sum(axis=1)
+    M = np.sqrt(np.maximum(v[:, 0] ** 2 - v[:, 1] ** 2 - v[:, 2] ** 2 - v[:, 3] ** 2, 0.0))
+    tol = 1e-5 * np.maximum(M, 1.0) + 1e-6
+    assert np.all(np.abs(got_m[ok] - M) <= tol), "returned mass is the mass of the returned triplet"
+    assert np.all(np.abs(np.abs(M - target) - np.abs(ref_m[ok].astype(np.float64) - target)) <= 2 * tol), "distance reached"
+    same = (got_i[ok] == ref_i[ok]).all(axis=1).mean()
+    assert same > 0.999, same
+
+
+@pytest.mark.parametrize("config,n", [(0, None), (2, 200_003)])
+def test_triplet_mass(hk, config, n):
+    wl = hepgen.generate(config, n_events=n)
+    j = wl.jets
+    rng = np.random.default_rng(12)
+    sel = (j.pt > 30) & (np.abs(j.eta) < 2.4)
+    mr = (rng.random(wl.n_events) < 0.9).astype(np.uint8)
+    for rows, cont in ((None, None), (mr, sel.astype(np.uint8))):
+        ref_m, ref_i = hepo.triplet_mass(j.pt, j.eta, j.phi, j.mass, j.offsets, 172.0, rows, cont)
+        got_m, got_i = hk.triplet_mass(cu(j.pt), cu(j.eta), cu(j.phi), cu(j.mass), cu(j.offsets), 172.0,
+                                       None if rows is None else cu(rows), None if cont is None else cu(cont))
+        _triplet_check(to_np(got_m), to_np(got_i), ref_m, ref_i, j.pt, j.eta, j.phi, j.mass, j.offsets,
+                       None if cont is None else cont.astype(bool), 172.0)
+        if rows is not None:
+            assert (to_np(got_m)[mr == 0] == 0).all()
+
+
+def test_triplet_mass_long_events(hk):
+    """Events larger than the kernel's shared-memory cache (96 selected jets) and exact ties."""
+    rng = np.random.default_rng(13)
+    counts = np.array([0, 2, 3, 120, 5, 97, 96, 1, 40], np.int64)
+    off = np.zeros(counts.size + 1, np.int64)
+    off[1:] = np.cumsum(counts)
+    m = int(off[-1])
+    pt = (20 + rng.exponential(30, m)).astype(np.float32)
+    eta = rng.uniform(-2.5, 2.5, m).astype(np.float32)
+    phi = rng.uniform(-np.pi, np.pi, m).astype(np.float32)
+    mass = rng.exponential(10, m).astype(np.float32)
+    pt[off[4]:off[5]] = 45.0; eta[off[4]:off[5]] = 0.3; phi[off[4]:off[5]] = 1.0; mass[off[4]:off[5]] = 4.0   # five identical jets: all triplets tie
+    ref_m, ref_i = hepo.triplet_mass(pt, eta, phi, mass, off, 172.0)
+    got_m, got_i = hk.triplet_mass(cu(pt), cu(eta), cu(phi), cu(mass), cu(off), 172.0)
+    gm, gi = to_np(got_m), to_np(got_i)
+    assert list(gi[4]) == [0, 1, 2] and list(ref_i[4]) == [0, 1, 2]             # first triplet wins an exact tie
+    _triplet_check(gm, gi, ref_m, ref_i, pt, eta, phi, mass, off, None, 172.0)
+    only_m, none = hk.triplet_mass(cu(pt), cu(eta), cu(phi), cu(mass), cu(off), 172.0, want_indices=False)
+    assert none is None
+    assert_exact(to_np(only_m), gm)
