@@ -284,15 +284,17 @@ extern "C" int32_t hepk_fill_histogram_2d(const float* x, const float* y, const 
 }
 
 // ------------------------------------------------------------------------------------------ SURVEY.md 8(f-3)
-// hepk_triplet_mass: one warp per event.  The selected jets' four-vectors are built once per event
-// (one lane per jet, float64) into shared memory; lanes then take the (a, b) pairs round-robin and run over c > b,
+// hepk_triplet_mass: eight lanes per event, four events per warp.  The selected jets' four-vectors are
+// built once per event (one lane per jet, float64) into shared memory; lanes take the (a, b) pairs round-robin and run over c > b,
 // so every triplet costs four float64 adds, four multiply-adds and a square root; the best triplet per lane is
 // reduced over the warp by (distance, a, b, c).  ALU-bound on long events, launch/latency-bound on short ones.
 namespace hepk {
 namespace dev {
 
-constexpr int TRIPLET_CAP = 96;      // selected jets of one event held in shared memory (more: recomputed on the fly)
+constexpr int TRIPLET_CAP = 64;      // selected jets of one event held in shared memory (more: recomputed on the fly)
 constexpr int TRIPLET_WARPS = 4;
+constexpr int TRIPLET_GROUP = 8;     // lanes per event: four events per warp (a typical event has ~10 pairs)
+constexpr int TRIPLET_GPW = 32 / TRIPLET_GROUP;
 
 struct Vec4 { double e, x, y, z; };
 
@@ -315,30 +317,36 @@ __global__ void __launch_bounds__(32 * TRIPLET_WARPS) triplet_kernel(const float
                                                                       const unsigned char* __restrict__ mask_content, float target,
                                                                       float* __restrict__ out_mass, int* __restrict__ out_idx)
 {
-    __shared__ Vec4 s_vec[TRIPLET_WARPS][TRIPLET_CAP];
-    __shared__ int s_loc[TRIPLET_WARPS][TRIPLET_CAP];
+    __shared__ Vec4 s_vec[TRIPLET_WARPS * TRIPLET_GPW][TRIPLET_CAP];
+    __shared__ int s_loc[TRIPLET_WARPS * TRIPLET_GPW][TRIPLET_CAP];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    Vec4* vec = s_vec[warp];
-    int* loc = s_loc[warp];
-    const long long nw = (long long)gridDim.x * TRIPLET_WARPS;
-    for (long long e = (long long)blockIdx.x * TRIPLET_WARPS + warp; e < n_events; e += nw) {
-        const long long g0 = __ldg(offsets + e), g1 = __ldg(offsets + e + 1);
-        const bool row = !mask_rows || mask_rows[e];
-        // ---- selected jets -> local index list (and four-vectors while they fit)
+    const int grp = lane / TRIPLET_GROUP, sl = lane % TRIPLET_GROUP;
+    Vec4* vec = s_vec[warp * TRIPLET_GPW + grp];
+    int* loc = s_loc[warp * TRIPLET_GPW + grp];
+    const long long ng = (long long)gridDim.x * TRIPLET_WARPS * TRIPLET_GPW;
+    const long long g_first = ((long long)blockIdx.x * TRIPLET_WARPS + warp) * TRIPLET_GPW + grp;
+    // all four groups of a warp run the same number of rounds (warp-wide votes and shuffles below)
+    const long long rounds = (n_events + ng - 1) / ng;
+    for (long long r = 0; r < rounds; ++r) {
+        const long long e = g_first + r * ng;
+        const bool live = e < n_events;
+        const long long g0 = live ? __ldg(offsets + e) : 0, g1 = live ? __ldg(offsets + e + 1) : 0;
+        const bool row = live && (!mask_rows || mask_rows[e]);
+        // ---- selected jets -> local index list (and four-vectors while they fit), eight jets per step
         int nsel = 0;
-        if (row) {
-            for (long long c0 = g0; c0 < g1; c0 += 32) {
-                const long long g = c0 + lane;
-                const bool sel = g < g1 && (!mask_content || mask_content[g - base]);
-                const unsigned m = __ballot_sync(0xffffffffu, sel);
-                const int at = nsel + __popc(m & ((1u << lane) - 1u));
-                if (sel && at < TRIPLET_CAP) {
-                    const long long i = g - base;
-                    loc[at] = (int)(g - g0);
-                    vec[at] = four_vector(__ldg(pt + i), __ldg(eta + i), __ldg(phi + i), __ldg(mass + i));
-                }
-                nsel += __popc(m);
+        const long long span = row ? g1 - g0 : 0;
+        const long long steps = __reduce_max_sync(0xffffffffu, (unsigned)((span + TRIPLET_GROUP - 1) / TRIPLET_GROUP));
+        for (long long st = 0; st < steps; ++st) {
+            const long long g = g0 + st * TRIPLET_GROUP + sl;
+            const bool sel = row && g < g1 && (!mask_content || mask_content[g - base]);
+            const unsigned m = (__ballot_sync(0xffffffffu, sel) >> (TRIPLET_GROUP * grp)) & ((1u << TRIPLET_GROUP) - 1u);
+            const int at = nsel + __popc(m & ((1u << sl) - 1u));
+            if (sel && at < TRIPLET_CAP) {
+                const long long i = g - base;
+                loc[at] = (int)(g - g0);
+                vec[at] = four_vector(__ldg(pt + i), __ldg(eta + i), __ldg(phi + i), __ldg(mass + i));
             }
+            nsel += __popc(m);
         }
         __syncwarp();
         const bool cached = nsel <= TRIPLET_CAP;
@@ -355,16 +363,16 @@ __global__ void __launch_bounds__(32 * TRIPLET_WARPS) triplet_kernel(const float
             const long long i = g0 - base + local_of(s);
             return four_vector(__ldg(pt + i), __ldg(eta + i), __ldg(phi + i), __ldg(mass + i));
         };
-        // ---- triplets: lane takes pairs (a, b) round-robin, runs over c
+        // ---- triplets: a lane of the group takes pairs (a, b) round-robin, runs over c
         double best = CUDART_INF;
         double best_m = 0.0;
         int ba = 0x7fffffff, bb = 0x7fffffff, bc = 0x7fffffff;
         const long long npairs = (long long)nsel * (nsel - 1) / 2;
-        for (long long p = lane; p < npairs; p += 32) {
+        for (long long p = sl; p < npairs; p += TRIPLET_GROUP) {
             int a = 0;
-            long long r = p;
-            while (r >= nsel - 1 - a) { r -= nsel - 1 - a; ++a; }
-            const int b = a + 1 + (int)r;
+            long long q = p;
+            while (q >= nsel - 1 - a) { q -= nsel - 1 - a; ++a; }
+            const int b = a + 1 + (int)q;
             const Vec4 va = vec_of(a), vb = vec_of(b);
             const double e2 = va.e + vb.e, x2 = va.x + vb.x, y2 = va.y + vb.y, z2 = va.z + vb.z;
             for (int c = b + 1; c < nsel; ++c) {
@@ -377,9 +385,10 @@ __global__ void __launch_bounds__(32 * TRIPLET_WARPS) triplet_kernel(const float
                 if (d < best) { best = d; best_m = M; ba = a; bb = b; bc = c; }     // visited in (a, b, c) order per lane
             }
         }
-        // ---- warp argmin by (distance, a, b, c)
+        __syncwarp();
+        // ---- argmin over the group's lanes by (distance, a, b, c)
 #pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) {
+        for (int o = TRIPLET_GROUP / 2; o >= 1; o >>= 1) {
             const double od = __shfl_xor_sync(0xffffffffu, best, o);
             const double om = __shfl_xor_sync(0xffffffffu, best_m, o);
             const int oa = __shfl_xor_sync(0xffffffffu, ba, o), ob = __shfl_xor_sync(0xffffffffu, bb, o),
@@ -387,7 +396,7 @@ __global__ void __launch_bounds__(32 * TRIPLET_WARPS) triplet_kernel(const float
             const bool take = od < best || (od == best && (oa < ba || (oa == ba && (ob < bb || (ob == bb && oc < bc)))));
             if (take) { best = od; best_m = om; ba = oa; bb = ob; bc = oc; }
         }
-        if (lane == 0) {
+        if (sl == 0 && live) {
             const bool have = nsel >= 3;
             out_mass[e] = have ? (float)best_m : 0.0f;
             if (out_idx) {
@@ -410,7 +419,8 @@ extern "C" int32_t hepk_triplet_mass(const float* pt, const float* eta, const fl
     HEPK_REQUIRE(n_events >= 0, "n_events < 0");
     if (n_events == 0) return HEPK_OK;
     HEPK_REQUIRE(offsets && out_mass, "offsets/out_mass is NULL");
-    long long blocks = (n_events + dev::TRIPLET_WARPS - 1) / dev::TRIPLET_WARPS;
+    const long long per_block = dev::TRIPLET_WARPS * dev::TRIPLET_GPW;
+    long long blocks = (n_events + per_block - 1) / per_block;
     const long long maxb = (long long)sm_count() * 12;
     if (blocks > maxb) blocks = maxb;
     dev::triplet_kernel<<<(unsigned)blocks, 32 * dev::TRIPLET_WARPS, 0, (cudaStream_t)stream>>>(
