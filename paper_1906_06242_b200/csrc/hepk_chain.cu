@@ -22,7 +22,6 @@
 // Privatised histograms are merged into float64 global accumulators every few thousand events.
 // A tile that does not fit its staging region (giant events, misaligned or out-of-range slices) takes the
 // paper's own loop shape (Listing 1): one lane per event, straight from global memory.
-#include <stdlib.h>
 #include <string.h>
 
 #include "hepk_common.cuh"
@@ -1231,11 +1230,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
 #define HEPK_PICK(MAXT)                                                                                              \
     (calib ? (has_el ? dev::chain_kernel<true, true, MAXT> : dev::chain_kernel<true, false, MAXT>)                 \
            : (has_el ? dev::chain_kernel<false, true, MAXT> : dev::chain_kernel<false, false, MAXT>))
-    const char* force = getenv("HEPK_FORCE_MAXT");      // experiment hook: register budget variant
-    const int fm = force ? atoi(force) : 0;
-    if (fm == 640 && wpc <= 20) kern = HEPK_PICK(640);
-    else if (fm == 768) kern = HEPK_PICK(768);
-    else if (wpc <= 16) kern = HEPK_PICK(512);
+    if (wpc <= 16) kern = HEPK_PICK(512);
     else if (wpc <= 20) kern = HEPK_PICK(640);
     else kern = HEPK_PICK(768);
 #undef HEPK_PICK

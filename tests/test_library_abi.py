@@ -76,3 +76,21 @@ def test_product_path_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "hepo" not in text and "import oracle" not in text and "from oracle" not in text, f
+
+
+def test_bench_algorithmic_bytes_matches_survey_8d():
+    """bench.py's algorithmic bytes per event equal SURVEY.md 8(d)'s table (config 2: 210.3 B/event) on a sample."""
+    import importlib.util
+    import hepgen
+    spec = importlib.util.spec_from_file_location("bench", os.path.join(ROOT, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    wl = hepgen.generate(2, n_events=200_000)
+    per_event = bench.algorithmic_bytes(wl) / wl.n_events
+    nj = wl.jets.n_objects / wl.n_events
+    nm = wl.muons.n_objects / wl.n_events
+    ne = wl.electrons.n_objects / wl.n_events
+    want = 24 + 16 * nj + 12 * nm + 12 * ne + 4 + 20
+    assert abs(per_event - want) < 0.01
+    assert 205 < per_event < 216                       # SURVEY.md 8(d): 210.3 B/event for config 2
+    assert bench.algorithmic_bytes(wl, event_outputs=False) == bench.algorithmic_bytes(wl) - 20 * wl.n_events
