@@ -322,7 +322,7 @@ __device__ __forceinline__ float pair_mass_lean(float pt1, float eta1, float phi
 // What the launch asked for, as one register of flags (tested with one instruction instead of a pointer compare).
 enum : unsigned {
     F_NJET = 1u << 0, F_ARGMAX = 1u << 1, F_HT = 1u << 2, F_MAXPT = 1u << 3, F_MINPT = 1u << 4, F_MJJ = 1u << 5,
-    F_SUBPT = 1u << 6, F_OBS0 = 1u << 8 /* .. << 13 */, F_COUNTS = 1u << 16, F_SUMW = 1u << 17, F_WEIGHTS = 1u << 18
+    F_SUBPT = 1u << 6, F_OBS0 = 1u << 8 /* .. << 13 */, F_COUNTS = 1u << 16, F_SUMW = 1u << 17, F_WEIGHTS = 1u << 18, F_MULTIW = 1u << 19 /* more than one weight column */
 };
 __device__ __forceinline__ unsigned chain_features(const ChainParams& P)
 {
@@ -340,6 +340,7 @@ __device__ __forceinline__ unsigned chain_features(const ChainParams& P)
     if (P.hist_counts) f |= F_COUNTS;
     if (P.hist_acc) f |= F_SUMW;
     if (P.weights) f |= F_WEIGHTS;
+    if (P.W > 1) f |= F_MULTIW;
     return f;
 }
 
@@ -414,7 +415,7 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     if (!(feat & F_SUMW)) return;
     const float wscale = lds_f32(smem_u32(S.wscale));
     add_weight(P, feat, bin, 0, wt0, wscale);
-    if (!(feat & F_WEIGHTS)) return;
+    if ((feat & (F_WEIGHTS | F_MULTIW)) != (F_WEIGHTS | F_MULTIW)) return;
     for (int w = 1; w < P.W; ++w) add_weight(P, feat, bin, w, __ldg(P.weights + (long long)w * P.n_events + ev), wscale);
 }
 
@@ -459,8 +460,33 @@ struct EventAcc {
     }
     // The same update for a jet that counts iff p > pt_min (p may be anything, NaN included, otherwise), written
     // with predicated instructions: 3 compares, 1 convert and 9 predicated operations.
+    __device__ __forceinline__ void push_lean_nomin(float p, float pt_min, int k)
+    {
+        asm("{\n\t"
+            ".reg .pred ok, g1, g2;\n\t"
+            ".reg .f64 pd;\n\t"
+            ".reg .f32 pz;\n\t"
+            "setp.gt.f32 ok, %7, %8;\n\t"
+            "setp.gt.and.f32 g1, %7, %4, ok;\n\t"
+            "setp.gt.and.f32 g2, %7, %5, ok;\n\t"
+            "selp.f32 pz, %7, 0f00000000, ok;\n\t"
+            "cvt.f64.f32 pd, pz;\n\t"
+            "@ok add.s32 %0, %0, 1;\n\t"
+            "add.f64 %1, %1, pd;\n\t"
+            "@g2 mov.b32 %6, %9;\n\t"
+            "@g1 mov.b32 %6, %3;\n\t"
+            "@g1 mov.b32 %3, %9;\n\t"
+            "@g2 mov.f32 %5, %7;\n\t"
+            "@g1 mov.f32 %5, %4;\n\t"
+            "@g1 mov.f32 %4, %7;\n\t"
+            "}"
+            : "+r"(cnt), "+d"(sum), "+f"(mn), "+r"(i1), "+f"(b1), "+f"(b2), "+r"(i2)
+            : "f"(p), "f"(pt_min), "r"(k));
+    }
+    template <bool NEED_MIN>
     __device__ __forceinline__ void push_lean(float p, float pt_min, int k)
     {
+        if (!NEED_MIN) { push_lean_nomin(p, pt_min, k); return; }
         asm("{\n\t"
             ".reg .pred ok, g1, g2;\n\t"
             ".reg .f64 pd;\n\t"
@@ -633,7 +659,7 @@ __device__ __forceinline__ bool issue_tile(const LaneCol& c, int lane, long long
     return true;
 }
 
-template <bool CALIB, bool HAS_EL, int MAXT>
+template <bool CALIB, bool HAS_EL, int MAXT, int FEAT>
 __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ ChainParams P)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -740,7 +766,9 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     const uint32_t corr_a = region_a + (uint32_t)P.corr_off;
     const uint32_t bucket_a = region_a + (uint32_t)P.bucket_off;
     const int V = CALIB ? P.V : 1;
-    const unsigned feat = chain_features(P);
+    // FEAT >= 0: the launch's feature word is known at compile time (the common analysis shape; one weight column),
+    // so everything it does not ask for is compiled out
+    const unsigned feat = FEAT >= 0 ? (unsigned)FEAT : chain_features(P);
 
     const long long GW = (long long)gridDim.x * nwarp;
     long long tile = (long long)warp * gridDim.x + blockIdx.x;
@@ -933,7 +961,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                             ap += 4;
                             pn = lds_f32(ap);
                             if (CALIB) cn = lds_f32(ap + d_corr);
-                            a.push_lean(p, P.jet_pt_min, k);
+                            a.template push_lean<(FEAT < 0) || ((FEAT & (int)(F_MINPT | (F_OBS0 << HEPK_OBS_MINPT))) != 0)>(p, P.jet_pt_min, k);
                         }
                     }
                     // long events: jets beyond TAIL_CUT, 32 at a time, one per lane, reduced over the warp and folded
@@ -1227,12 +1255,33 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
 
     // three register budgets: up to 16 warps per CTA (128 registers per thread), 20 (102) or 24 (85)
     void (*kern)(ChainParams);
-#define HEPK_PICK(MAXT)                                                                                              \
-    (calib ? (has_el ? dev::chain_kernel<true, true, MAXT> : dev::chain_kernel<true, false, MAXT>)                 \
-           : (has_el ? dev::chain_kernel<false, true, MAXT> : dev::chain_kernel<false, false, MAXT>))
-    if (wpc <= 16) kern = HEPK_PICK(512);
-    else if (wpc <= 20) kern = HEPK_PICK(640);
-    else kern = HEPK_PICK(768);
+#define HEPK_PICK(MAXT, FEAT)                                                                                        \
+    (calib ? (has_el ? dev::chain_kernel<true, true, MAXT, FEAT> : dev::chain_kernel<true, false, MAXT, FEAT>)     \
+           : (has_el ? dev::chain_kernel<false, true, MAXT, FEAT> : dev::chain_kernel<false, false, MAXT, FEAT>))
+    // the common analysis shape (njet, argmax, ht, maxpt, mjj per event; HT and leading-pt histograms with counts and
+    // one weight column) has a build with its feature word as a compile-time constant
+    constexpr int FEAT_COMMON = (int)(dev::F_NJET | dev::F_ARGMAX | dev::F_HT | dev::F_MAXPT | dev::F_MJJ |
+                                      (dev::F_OBS0 << HEPK_OBS_HT) | (dev::F_OBS0 << HEPK_OBS_MAXPT) | dev::F_COUNTS |
+                                      dev::F_SUMW | dev::F_WEIGHTS);
+    unsigned feat_host = 0;
+    if (d->out_njet) feat_host |= dev::F_NJET;
+    if (d->out_argmax) feat_host |= dev::F_ARGMAX;
+    if (d->out_ht) feat_host |= dev::F_HT;
+    if (d->out_maxpt) feat_host |= dev::F_MAXPT;
+    if (d->out_minpt) feat_host |= dev::F_MINPT;
+    if (d->out_mjj) feat_host |= dev::F_MJJ;
+    if (d->out_subpt) feat_host |= dev::F_SUBPT;
+    for (int o = 0; o < HEPK_N_OBS; ++o)
+        if (d->axis_edges[o]) feat_host |= dev::F_OBS0 << o;
+    if (P.hist_counts) feat_host |= dev::F_COUNTS;
+    if (P.hist_acc) feat_host |= dev::F_SUMW;
+    if (d->weights) feat_host |= dev::F_WEIGHTS;
+    if (P.W > 1) feat_host |= dev::F_MULTIW;
+    const bool common = (int)feat_host == FEAT_COMMON && !d->out_jet_mask && has_el;
+    if (wpc <= 16) kern = common ? (calib ? dev::chain_kernel<true, true, 512, FEAT_COMMON> : dev::chain_kernel<false, true, 512, FEAT_COMMON>)
+                                 : HEPK_PICK(512, -1);
+    else if (wpc <= 20) kern = HEPK_PICK(640, -1);
+    else kern = HEPK_PICK(768, -1);
 #undef HEPK_PICK
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;

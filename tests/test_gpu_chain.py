@@ -230,6 +230,28 @@ def test_chain_calibration_axis_modes(hk):
         compare(out, ref, wl, what=f"calib {kind} ")
 
 
+@pytest.mark.parametrize("config,n", [(1, 150_001), (2, 200_003), (3, 80_001)])
+def test_chain_common_shape_build(hk, config, n):
+    """The launch shape bench.py times (njet, ht, maxpt, argmax, mjj + HT / leading-pt histograms, one weight column)
+    runs a build of the kernel with its feature word fixed at compile time: same results as the generic build."""
+    wl = hepgen.generate(config, n_events=n)
+    ref = hepo.analysis_chain(wl, want_mask=False)
+    names = ("njet", "ht", "maxpt", "argmax", "mjj")
+    out, plan = hk.analysis_chain(hk.upload(wl), want_event_outputs=names)
+    torch.cuda.synchronize()
+    assert set(out) == set(names) | {"hist_sumw", "hist_counts"}
+    for k in ("njet", "argmax", "maxpt"):
+        assert_exact(to_np(out[k]), ref[k], k)
+    for k in ("ht", "mjj"):
+        assert_tol(to_np(out[k]), ref[k], k)
+    assert_exact(to_np(out["hist_counts"]), ref["hist_counts"])
+    assert_tol(to_np(out["hist_sumw"]), ref["hist_sumw"])
+    full, _ = hk.analysis_chain(hk.upload(wl))                    # generic build
+    torch.cuda.synchronize()
+    for k in names:
+        assert_exact(to_np(out[k]), to_np(full[k]), f"common vs generic {k}")
+
+
 def test_chain_optional_outputs(hk):
     wl = hepgen.generate(1, n_events=20_000)
     ref = hepo.analysis_chain(wl, want_mask=False)
