@@ -881,8 +881,9 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     uint32_t a = a0;
                     const uint32_t aend = a + 4u * (unsigned)(nj < TAIL_CUT ? nj : TAIL_CUT);
                     const unsigned int word0 = word;
+                    if ((aend - a) & 4u) { sts_u32(a, word); a += 4; word += 4; }       // odd count: one word first, then pairs
 #pragma unroll 1
-                    for (; a != aend; a += 4, word += 4) sts_u32(a, word);
+                    for (; a != aend; a += 8, word += 8) { sts_u32(a, word); sts_u32(a + 4, word + 4); }
                     // long events: the rest of their words, one per lane
                     for (unsigned lm = longm; lm; lm &= lm - 1) {
                         const int src = __ffs(lm) - 1;
