@@ -480,7 +480,7 @@ struct EventAcc {
             "@g1 mov.f32 %5, %4;\n\t"
             "@g1 mov.f32 %4, %7;\n\t"
             "}"
-            : "+r"(cnt), "+d"(sum), "+f"(mn), "+r"(i1), "+f"(b1), "+f"(b2), "+r"(i2)
+            : "+&r"(cnt), "+&d"(sum), "+&f"(mn), "+&r"(i1), "+&f"(b1), "+&f"(b2), "+&r"(i2)
             : "f"(p), "f"(pt_min), "r"(k));
     }
     template <bool NEED_MIN>
@@ -506,7 +506,7 @@ struct EventAcc {
             "@g1 mov.f32 %5, %4;\n\t"
             "@g1 mov.f32 %4, %7;\n\t"
             "}"
-            : "+r"(cnt), "+d"(sum), "+f"(mn), "+r"(i1), "+f"(b1), "+f"(b2), "+r"(i2)
+            : "+&r"(cnt), "+&d"(sum), "+&f"(mn), "+&r"(i1), "+&f"(b1), "+&f"(b2), "+&r"(i2)
             : "f"(p), "f"(pt_min), "r"(k));
     }
 };
@@ -950,19 +950,26 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     EventAcc a;
                     a.init();
                     {
-                        // the next jet is loaded before the current one is folded in (one element of over-read
-                        // at the end stays inside the staging buffer's slack)
+                        // two jets per iteration (an odd count takes one jet first)
                         uint32_t ap = a_ev;
-                        float pn = lds_f32(ap), cn = CALIB ? lds_f32(ap + d_corr) : 1.0f;
                         const int nmain = nj < TAIL_CUT ? nj : TAIL_CUT;
-#pragma unroll 1
-                        for (int k = 0; k != nmain; ++k) {
-                            float p = pn;
-                            if (CALIB) p = __fmul_rn(p, __fmul_rn(cn, sv));     // NaN when the jet failed eta / dR
+                        int k = 0;
+                        auto value = [&](uint32_t at) {
+                            float p = lds_f32(at);
+                            if (CALIB) p = __fmul_rn(p, __fmul_rn(lds_f32(at + d_corr), sv));     // NaN when the jet failed eta / dR
+                            return p;
+                        };
+                        constexpr bool NEED_MIN = (FEAT < 0) || ((FEAT & (int)(F_MINPT | (F_OBS0 << HEPK_OBS_MINPT))) != 0);
+                        if (nmain & 1) {
+                            a.template push_lean<NEED_MIN>(value(ap), P.jet_pt_min, 0);
                             ap += 4;
-                            pn = lds_f32(ap);
-                            if (CALIB) cn = lds_f32(ap + d_corr);
-                            a.template push_lean<(FEAT < 0) || ((FEAT & (int)(F_MINPT | (F_OBS0 << HEPK_OBS_MINPT))) != 0)>(p, P.jet_pt_min, k);
+                            k = 1;
+                        }
+#pragma unroll 1
+                        for (; k != nmain; k += 2, ap += 8) {
+                            const float p0 = value(ap), p1 = value(ap + 4);
+                            a.template push_lean<NEED_MIN>(p0, P.jet_pt_min, k);
+                            a.template push_lean<NEED_MIN>(p1, P.jet_pt_min, k + 1);
                         }
                     }
                     // long events: jets beyond TAIL_CUT, 32 at a time, one per lane, reduced over the warp and folded
