@@ -643,13 +643,14 @@ __device__ __forceinline__ long long cur_lo_jets(const ChainParams&, long long c
 // aligned on both sides; the consumer recomputes the same shift.
 __device__ __forceinline__ bool issue_tile(const LaneCol& c, int lane, long long lo, long long hi, uint64_t* bar)
 {
-    const long long l0 = lo - c.base, l1 = hi - c.base;
-    const long long n = l1 - l0;
+    const long long l0 = lo - c.base;
+    const long long n64 = hi - lo;
     const int sh = ((int)l0 + c.mis) & 3;
     const long long a0 = l0 - sh;
-    const long long len = (n + sh + 3) & ~3ll;
-    const bool active = c.ptr != nullptr && n != 0;
-    const bool ok = !active || (n > 0 && n <= c.cap && a0 >= 0 && a0 + len <= c.n);
+    const bool small = (unsigned long long)n64 <= (unsigned long long)c.cap;      // also rules out n < 0
+    const int len = ((int)n64 + sh + 3) & ~3;                                      // meaningful when small
+    const bool active = c.ptr != nullptr && n64 != 0;
+    const bool ok = !active || (small && (a0 | (c.n - a0 - len)) >= 0);            // 0 <= a0 and a0 + len <= n
     if (!__all_sync(0xffffffffu, ok)) return false;
     const uint32_t bytes = active ? ((uint32_t)len << 2) : 0u;
     const uint32_t total = __reduce_add_sync(0xffffffffu, bytes);
