@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--single-kernels", action="store_true",
                     help="time each single kernel (SURVEY.md 8(a) rows a1-a6) instead of the fused chain; one JSON line")
+    ap.add_argument("--variants", type=int, default=None,
+                    help="configs 3/4: number of calibration variants (scales 1 +- k*0.0025); the paper's full-systematics scenario is 40")
     ap.add_argument("--tune", default="", help="chain tuning knobs, e.g. warps_per_sm=20,ctas_per_sm=1 (testing only)")
     ap.add_argument("--ref-sample", type=int, default=1_000_000, help="events per step of the reference arm")
     return ap.parse_args()
@@ -194,6 +196,9 @@ def run_hepk(args):
 
     # weak scaling: every rank draws its own batch of the same recipe (events are independent)
     wl = hepgen.generate(args.config, n_events=args.events, batch=rank)
+    if args.variants and wl.calib is not None:
+        import numpy as _np
+        wl.calib["scales"] = (1.0 + 0.0025 * (_np.arange(args.variants) - args.variants // 2)).astype(_np.float32)
     N = wl.n_events
     V = 1 if wl.calib is None else len(wl.calib["scales"])
     inp = hk.upload(wl)

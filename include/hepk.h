@@ -47,7 +47,7 @@ extern "C" {
 #define HEPK_ERR_UNSUPPORTED (-2)
 #define HEPK_ERR_CUDA        (-3)
 
-#define HEPK_MAX_VARIANTS 8
+#define HEPK_MAX_VARIANTS 64
 #define HEPK_MAX_WVAR     16
 
 /* Library version (major*10000 + minor*100 + patch). */

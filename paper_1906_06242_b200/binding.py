@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libhepk.so")
 
 OBSERVABLES = ("njet", "ht", "maxpt", "minpt", "mjj", "subpt")
 N_OBS = 6
-MAX_VARIANTS = 8
+MAX_VARIANTS = 64
 MAX_WVAR = 16
 VARIANT_AUTO, VARIANT_WARP_PER_EVENT, VARIANT_BLOCK_PER_TILE = 0, 1, 2
 

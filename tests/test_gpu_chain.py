@@ -252,6 +252,18 @@ def test_chain_common_shape_build(hk, config, n):
         assert_exact(to_np(out[k]), to_np(full[k]), f"common vs generic {k}")
 
 
+def test_chain_forty_variants(hk):
+    """The paper's full-systematics scenario ("increasing the computational complexity ... by about
+    40x"): 40 calibration variants in one pass."""
+    wl = hepgen.generate(3, n_events=20_011)
+    wl.calib["scales"] = (1.0 + 0.0025 * (np.arange(40) - 20)).astype(np.float32)
+    ref = hepo.analysis_chain(wl)
+    out, _ = run_gpu(hk, wl)
+    assert to_np(out["njet"]).shape == (40, wl.n_events)
+    compare(out, ref, wl, what="40 variants ")
+    assert (np.diff(ref["njet"].astype(np.int64), axis=0) >= 0).all()      # larger scale never loses a jet
+
+
 def test_chain_optional_outputs(hk):
     wl = hepgen.generate(1, n_events=20_000)
     ref = hepo.analysis_chain(wl, want_mask=False)
