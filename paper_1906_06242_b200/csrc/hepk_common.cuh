@@ -99,6 +99,17 @@ __device__ __forceinline__ void bulk_g2s_addr(uint32_t dst_smem, const void* src
                  : "memory");
 }
 
+// shared-memory reductions in the shared state space (a generic-address atomicAdd on shared memory goes through an
+// address-space dispatch first)
+__device__ __forceinline__ void red_shared_add_u32(void* p, unsigned int v)
+{
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_shared_add_f32(void* p, float v)
+{
+    asm volatile("red.shared.add.f32 [%0], %1;" ::"r"(smem_u32(p)), "f"(v) : "memory");
+}
+
 // ---- staging a slice [l0, l1) of a column into shared memory -----------------------------------
 // Element l of `col` lands at dst[l - a0], a0 <= l0 chosen so that the 16-byte aligned body of the slice
 // can be moved by ONE bulk copy; the ragged head (col not 16-byte aligned near element 0) and the tail

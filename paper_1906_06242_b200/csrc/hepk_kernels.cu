@@ -120,8 +120,8 @@ __global__ void __launch_bounds__(256) fill_hist_kernel(const float* __restrict_
     const float inv_w = (float)nbins / (s_edges[nbins] - lo);
     auto add = [&](float xv, float wv) {
         const int s = hist_slot(xv, s_edges, nbins, lo, inv_w);
-        if (sumw) atomicAdd(&s_sumw[s], wv);
-        if (counts) atomicAdd(&s_cnt[s], 1u);
+        if (sumw) red_shared_add_f32(&s_sumw[s], wv);
+        if (counts) red_shared_add_u32(&s_cnt[s], 1u);
     };
     auto flush = [&]() {
         __syncthreads();

@@ -209,8 +209,8 @@ __global__ void __launch_bounds__(256) fill_hist2d_kernel(const float* __restric
         const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x + it * stride;
         if (i < n) {
             const int s = hist_slot(__ldg(x + i), s_ex, nx, lox, invx) * (ny + 2) + hist_slot(__ldg(y + i), s_ey, ny, loy, invy);
-            if (acc) atomicAdd(&s_sumw[s], w ? __ldg(w + i) : 1.f);
-            if (counts) atomicAdd(&s_cnt[s], 1u);
+            if (acc) red_shared_add_f32(&s_sumw[s], w ? __ldg(w + i) : 1.f);
+            if (counts) red_shared_add_u32(&s_cnt[s], 1u);
         }
         if ((it + 1) % 64 == 0) flush();      // bounded float32 partial sums
     }
