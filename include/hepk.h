@@ -300,6 +300,14 @@ int32_t hepk_triplet_mass(const float* pt, const float* eta, const float* phi, c
                           const uint8_t* mask_content, float target, float* out_mass, int32_t* out_idx, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Precondition check of a jagged layout ("a contiguous offsets array of size N+1").  Every other
+ * entry assumes valid offsets; this one counts the violations among
+ *   offsets[0] >= content_base,  offsets[e] <= offsets[e+1] for every e,  offsets[n_events] - content_base <= n_objects
+ * into *n_bad (DEVICE pointer to one int64, overwritten).  offsets: DEVICE int64[n_events+1]. */
+int32_t hepk_validate_offsets(const int64_t* offsets, int64_t n_events, int64_t content_base, int64_t n_objects,
+                              int64_t* n_bad, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Device-side timing of the dominant kernel (measurement hook for bench.py; no part of the method).
  * Between hepk_profile_begin() and hepk_profile_end() every hepk_analysis_chain call records a CUDA event
  * pair on its launch stream directly around the fused chain kernel (at most 4096 launches are kept).

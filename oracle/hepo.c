@@ -599,3 +599,15 @@ int32_t hepo_triplet_mass(const float* pt, const float* eta, const float* phi, c
     }
     return 0;
 }
+
+int32_t hepo_validate_offsets(const int64_t* offsets, int64_t n_events, int64_t content_base, int64_t n_objects, int64_t* n_bad)
+{
+    if (!offsets || n_events < 0 || !n_bad) return -1;
+    int64_t bad = 0;
+    if (offsets[0] < content_base) ++bad;
+    for (int64_t e = 0; e < n_events; ++e)
+        if (offsets[e] > offsets[e + 1]) ++bad;
+    if (offsets[n_events] - content_base > n_objects) ++bad;
+    *n_bad = bad;
+    return 0;
+}

@@ -168,6 +168,11 @@ int32_t hepo_triplet_mass(const float* pt, const float* eta, const float* phi, c
                           const uint8_t* mask_rows, const uint8_t* mask_content, float target,
                           float* out_mass, int32_t* out_idx);
 
+/* Precondition check of a jagged layout ("a contiguous offsets array of size N+1" indexing
+ * contiguous data arrays): returns in *n_bad the number of violations among
+ *   offsets[0] >= content_base,  offsets[e] <= offsets[e+1] for every e,  offsets[n_events] - content_base <= n_objects. */
+int32_t hepo_validate_offsets(const int64_t* offsets, int64_t n_events, int64_t content_base, int64_t n_objects, int64_t* n_bad);
+
 #ifdef __cplusplus
 }
 #endif

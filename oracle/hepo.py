@@ -196,6 +196,15 @@ def triplet_mass(pt, eta, phi, mass, offsets, target, mask_rows=None, mask_conte
     return out, idx
 
 
+def validate_offsets(offsets, n_objects, content_base=0):
+    """Number of violations of the jagged-layout preconditions (0 = valid)."""
+    offsets = _i64(offsets)
+    bad = C.c_int64(0)
+    _check(lib().hepo_validate_offsets(_p(offsets, np.int64), C.c_int64(offsets.shape[0] - 1), C.c_int64(content_base),
+                                       C.c_int64(n_objects), C.byref(bad)))
+    return bad.value
+
+
 class Collection(C.Structure):
     _fields_ = [("offsets", C.c_void_p), ("content_base", C.c_int64), ("n_objects", C.c_int64),
                 ("pt", C.c_void_p), ("eta", C.c_void_p), ("phi", C.c_void_p), ("mass", C.c_void_p)]

@@ -273,6 +273,14 @@ def triplet_mass(pt, eta, phi, mass, offsets, target, mask_rows=None, mask_conte
     return out, idx
 
 
+def validate_offsets(offsets, n_objects, content_base=0, stream=None):
+    """Number of violations of the jagged-layout preconditions (synchronises to read the count back)."""
+    out = torch.zeros(1, dtype=torch.int64, device=offsets.device)
+    _check(lib().hepk_validate_offsets(_ptr(offsets, torch.int64), C.c_int64(offsets.numel() - 1), C.c_int64(content_base),
+                                       C.c_int64(n_objects), _ptr(out, torch.int64), _stream(stream)), "validate_offsets")
+    return int(out.item())
+
+
 def lookup_binned(x, y, edges_x, edges_y, table, out=None, stream=None):
     n = x.numel()
     if out is None:

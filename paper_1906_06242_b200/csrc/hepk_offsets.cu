@@ -428,3 +428,35 @@ extern "C" int32_t hepk_triplet_mass(const float* pt, const float* eta, const fl
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
+
+// ------------------------------------------------------------------------------------------ hepk_validate_offsets
+namespace hepk {
+namespace dev {
+__global__ void validate_offsets_kernel(const long long* __restrict__ off, long long n_events, long long base, long long n_objects,
+                                        unsigned long long* __restrict__ n_bad)
+{
+    unsigned long long bad = 0;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_events; e += (long long)gridDim.x * blockDim.x)
+        if (__ldg(off + e) > __ldg(off + e + 1)) ++bad;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        if (off[0] < base) ++bad;
+        if (off[n_events] - base > n_objects) ++bad;
+    }
+    bad = __reduce_add_sync(0xffffffffu, (unsigned)bad);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(n_bad, bad);
+}
+}  // namespace dev
+}  // namespace hepk
+
+extern "C" int32_t hepk_validate_offsets(const int64_t* offsets, int64_t n_events, int64_t content_base, int64_t n_objects,
+                                         int64_t* n_bad, void* stream)
+{
+    HEPK_REQUIRE(n_events >= 0, "n_events < 0");
+    HEPK_REQUIRE(offsets && n_bad, "offsets/n_bad is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    HEPK_CUDA_TRY(cudaMemsetAsync(n_bad, 0, sizeof(int64_t), st));
+    dev::validate_offsets_kernel<<<grid_for(n_events), 256, 0, st>>>((const long long*)offsets, n_events, content_base, n_objects,
+                                                                    (unsigned long long*)n_bad);
+    HEPK_CUDA_TRY(cudaGetLastError());
+    return HEPK_OK;
+}

@@ -204,3 +204,16 @@ def test_triplet_mass_long_events(hk):
     only_m, none = hk.triplet_mass(cu(pt), cu(eta), cu(phi), cu(mass), cu(off), 172.0, want_indices=False)
     assert none is None
     assert_exact(to_np(only_m), gm)
+
+
+def test_validate_offsets(hk):
+    wl = hepgen.generate(2, n_events=300_001)
+    off = wl.jets.offsets
+    m = wl.jets.pt.size
+    assert hk.validate_offsets(cu(off), m) == 0 == hepo.validate_offsets(off, m)
+    assert hk.validate_offsets(cu(off), m - 1) == 1
+    assert hk.validate_offsets(cu(off + 7), m, content_base=8) == 1
+    rng = np.random.default_rng(14)
+    broken = off.copy()
+    broken[rng.choice(np.arange(1, off.size - 1), 1000, replace=False)] -= 10_000_000
+    assert hk.validate_offsets(cu(broken), m) == hepo.validate_offsets(broken, m) > 0

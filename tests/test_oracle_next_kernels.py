@@ -203,3 +203,18 @@ def test_triplet_mass_closed_forms_and_brute_force():
     rot = ((phi + np.float32(0.9) + np.pi) % (2 * np.pi) - np.pi).astype(np.float32)
     rm, _ = hepo.triplet_mass(pt, eta, rot, mass, off, 172.0, mask_content=mc)
     assert np.all(np.abs(rm - got_m) <= 2e-4 * np.abs(got_m) + 1e-4)
+
+
+def test_validate_offsets_against_numpy():
+    rng = np.random.default_rng(8)
+    off = _jagged(rng, 1000, 3.0)
+    m = int(off[-1])
+    assert hepo.validate_offsets(off, m) == 0
+    assert hepo.validate_offsets(off, m - 1) == 1                       # last offset beyond the columns
+    assert hepo.validate_offsets(off + 5, m, content_base=5) == 0
+    assert hepo.validate_offsets(off + 5, m, content_base=6) == 1       # first offset before content_base
+    broken = off.copy()
+    idx = rng.choice(np.arange(1, 1000), 25, replace=False)
+    broken[idx] -= 1000
+    want = int((np.diff(broken) < 0).sum()) + int(broken[0] < 0) + int(broken[-1] > m)
+    assert hepo.validate_offsets(broken, m) == want and want >= 10
