@@ -210,7 +210,7 @@ typedef struct hepk_chain_desc {
     int32_t tune_cap_leptons;    /* capacity per lepton collection */
     int32_t tune_ctas_per_sm;    /* persistent CTAs per SM */
     int32_t tune_warps_per_cta;  /* warps (each owning its own tiles and staging region) per CTA, at most 24 */
-    int32_t tune_warps_per_sm;   /* resident warps per SM the launch aims for (default 16) */
+    int32_t tune_warps_per_sm;   /* resident warps per SM the launch aims for (default 20) */
 } hepk_chain_desc;
 
 /* `d` is a HOST pointer to a descriptor whose array pointers are DEVICE pointers.  `workspace` is a

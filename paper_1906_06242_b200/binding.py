@@ -14,7 +14,8 @@ from dataclasses import dataclass
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "csrc", "libhepk.so")
+# HEPK_LIBRARY overrides the path of the shared library (e.g. a build with other compile flags)
+LIB_PATH = os.environ.get("HEPK_LIBRARY") or os.path.join(_HERE, "csrc", "libhepk.so")
 
 OBSERVABLES = ("njet", "ht", "maxpt", "minpt", "mjj", "subpt")
 N_OBS = 6

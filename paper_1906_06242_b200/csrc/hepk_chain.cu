@@ -32,7 +32,8 @@ constexpr int TILE_EVENTS = 32;     // events per warp tile
 constexpr int NCOL = 10;            // staged columns: 0-3 jets pt,eta,phi,mass; 4-6 muons pt,eta,phi; 7-9 electrons
 constexpr int MAX_JETS_TILE = 512;  // byte offset of a jet inside a tile column (4 * index) fits 11 bits
 constexpr int MAX_LIST = 1023;      // byte offset of an event's lepton list (8 * start) fits 13 bits
-constexpr int MAX_LEP_EVENT = 31;   // byte length of an event's lepton list (8 * count) fits 8 bits
+constexpr int MAX_LEP_EVENT = 30;   // byte length of an event's lepton list, padded to pairs (16 * pairs), fits 8 bits
+constexpr int LIST_PAD = 36;        // list entries beyond the leptons of a tile: every event's list starts at an even entry
 constexpr int TAIL_CUT = 16;        // jets of an event beyond this many are handled by the whole warp, not by the event's lane
 constexpr int N_BUCKETS = 8;        // jets are ordered by min(selected leptons of their event, 7)
 
@@ -88,6 +89,7 @@ struct ChainShared {
     unsigned int* h_cnt;
     float* wscale;                       // [0] 2^k or 0, [1] 2^-k
     unsigned int* since;                 // events filled since the last flush
+    unsigned int* next;                  // tiles of the CTA's own range handed out so far
 };
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -110,6 +112,7 @@ __host__ __device__ inline size_t chain_shared_layout(const ChainParams& P, bool
     r = take(P.hist_counts ? spv * P.V * 4 : 0, 4); if (s) s->h_cnt = (unsigned int*)(base + r);
     r = take(8, 4); if (s) s->wscale = (float*)(base + r);
     r = take(4, 4); if (s) s->since = (unsigned int*)(base + r);
+    r = take(4, 4); if (s) s->next = (unsigned int*)(base + r);
     return align_up(o, 128);
 }
 
@@ -157,6 +160,12 @@ __device__ __forceinline__ float2 lds_v2(uint32_t a)
 {
     float2 r;
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(a) : "memory");
+    return r;
+}
+__device__ __forceinline__ float4 lds_v4(uint32_t a)
+{
+    float4 r;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "r"(a) : "memory");
     return r;
 }
 __device__ __forceinline__ int4 lds_v4i(uint32_t a)
@@ -253,9 +262,9 @@ __device__ __forceinline__ float dr2_min(float eta_a, float phi_a, float eta_b, 
     return __fadd_rn(__fmul_rn(deta, deta), __fmul_rn(w, w));
 }
 
-// The same value from packed float32x2 operations (FADD2 / FMUL2 round each half like FADD / FMUL): `jet` is
-// (eta, phi) of the jet, `nlep` is (-eta, -phi) of the lepton, so one packed add yields (deta, dphi).
-__device__ __forceinline__ float dr2_packed(float2 jet, float2 nlep)
+// The same value from packed float32x2 operations (FADD2 rounds each half like FADD): `jet` and `lep` are (eta, phi)
+// pairs, so one packed subtraction yields (deta, dphi).
+__device__ __forceinline__ float dr2_packed(float2 jet, float2 lep)
 {
     float r;
     asm("{\n\t"
@@ -263,7 +272,7 @@ __device__ __forceinline__ float dr2_packed(float2 jet, float2 nlep)
         ".reg .f32 dx, dy, ay, t, at, w, qx, qy;\n\t"
         "mov.b64 j, {%1, %2};\n\t"
         "mov.b64 l, {%3, %4};\n\t"
-        "add.rn.f32x2 d, j, l;\n\t"
+        "sub.rn.f32x2 d, j, l;\n\t"
         "mov.b64 {dx, dy}, d;\n\t"
         "abs.f32 ay, dy;\n\t"
         "add.rn.f32 t, ay, 0fC0C90FDB;\n\t"      // |dphi| - 2PI_F
@@ -274,7 +283,7 @@ __device__ __forceinline__ float dr2_packed(float2 jet, float2 nlep)
         "add.rn.f32 %0, qx, qy;\n\t"
         "}"
         : "=f"(r)
-        : "f"(jet.x), "f"(jet.y), "f"(nlep.x), "f"(nlep.y));
+        : "f"(jet.x), "f"(jet.y), "f"(lep.x), "f"(lep.y));
     return r;
 }
 
@@ -593,27 +602,6 @@ __device__ __forceinline__ void flush_hist(const ChainParams& P, const ChainShar
     }
 }
 
-// What a lane needs to stage "its" column (lanes 0..NCOL-1), loaded once into registers.
-struct LaneCol {
-    const char* ptr;            // nullptr: nothing to stage (other lanes, absent electrons)
-    const long long* off;       // the collection's offsets array
-    long long base, n;
-    int mis, cap;
-    uint32_t dst;               // shared-memory address of the staging buffer
-};
-
-// offsets[e0] and offsets[e1] of the lane's collection for tile `tile` (loaded one tile ahead of their use)
-__device__ __forceinline__ void load_bounds(const ChainParams& P, const LaneCol& c, long long tile, long long& lo, long long& hi)
-{
-    lo = hi = 0;
-    if (c.ptr) {
-        const long long e0 = tile * TILE_EVENTS;
-        const long long e1 = e0 + TILE_EVENTS < P.n_events ? e0 + TILE_EVENTS : P.n_events;
-        lo = __ldg(c.off + e0);
-        hi = __ldg(c.off + e1);
-    }
-}
-
 // Low words of offsets[e] and offsets[e+1] of the lane's event (lane = event of the tile), three collections.
 struct EventOffsets { int j0, j1, m0, m1, q0, q1; };
 
@@ -629,34 +617,49 @@ __device__ __forceinline__ void load_event_offsets(const ChainParams& P, long lo
     else { o.q0 = 0; o.q1 = 0; }
 }
 
-// offsets[e0] of the jets (64-bit): lane 0 stages a jet column, so its `lo` bound is exactly that value
-__device__ __forceinline__ long long cur_lo_jets(const ChainParams&, long long cur_lo, int)
+// Start the bulk copies of a tile whose slices start at global element lo[k] and hold cnt[k] elements (k: jets, muons,
+// electrons) into the warp's staging region; all 32 lanes call it, converged, with the same arguments in every lane.
+// Returns false (nothing issued) when a slice does not fit: capacity, 16-byte alignment at the array ends.
+// Element l of a column lands at buffer index l - a0, a0 = l0 - ((l0 + mis) mod 4), so every copy is 16-byte aligned
+// on both sides; the consumer recomputes the same shift.  One lane issues all copies: its operands are then uniform
+// by construction (a bulk copy takes uniform registers; copies issued from several lanes are serialised with a
+// register hand-over per operand and lane).
+template <bool HAS_EL>
+__device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region_a, int lane, const int (&lo)[3],
+                                           const int (&cnt)[3])
 {
-    const unsigned int a = __shfl_sync(0xffffffffu, (unsigned int)cur_lo, 0);
-    const unsigned int b = __shfl_sync(0xffffffffu, (unsigned int)((unsigned long long)cur_lo >> 32), 0);
-    return (long long)(((unsigned long long)b << 32) | a);
-}
-
-// Start the bulk copies of a tile into the warp's staging region; all 32 lanes call it, converged.
-// Returns false (nothing issued) when some slice does not fit: capacity, 16-byte alignment at the array ends.
-// Element l of a column lands at buffer index l - a0, a0 = l0 - ((l0 + mis) mod 4), so the copy is 16-byte
-// aligned on both sides; the consumer recomputes the same shift.
-__device__ __forceinline__ bool issue_tile(const LaneCol& c, int lane, long long lo, long long hi, uint64_t* bar)
-{
-    const long long l0 = lo - c.base;
-    const long long n64 = hi - lo;
-    const int sh = ((int)l0 + c.mis) & 3;
-    const long long a0 = l0 - sh;
-    const bool small = (unsigned long long)n64 <= (unsigned long long)c.cap;      // also rules out n < 0
-    const int len = ((int)n64 + sh + 3) & ~3;                                      // meaningful when small
-    const bool active = c.ptr != nullptr && n64 != 0;
-    const bool ok = !active || (small && (a0 | (c.n - a0 - len)) >= 0);            // 0 <= a0 and a0 + len <= n
-    if (!__all_sync(0xffffffffu, ok)) return false;
-    const uint32_t bytes = active ? ((uint32_t)len << 2) : 0u;
-    const uint32_t total = __reduce_add_sync(0xffffffffu, bytes);
-    if (lane == 0) mbar_arrive_expect_tx(bar, total);
-    __syncwarp();
-    if (active) bulk_g2s_addr(c.dst, c.ptr + (a0 << 2), bytes, bar);
+    int a0[3];
+    int len[3];
+    bool ok = true;
+    uint32_t total = 0;
+#pragma unroll
+    for (int k = 0; k < (HAS_EL ? 3 : 2); ++k) {
+        const int c0 = k == 0 ? 0 : (k == 1 ? 4 : 7);
+        // low words only: the staged path requires n_objects < 2^31, so offsets[e0] - content_base fits an int
+        const int l0 = (int)((unsigned)lo[k] - (unsigned)P.col_base[c0]);
+        const int sh = (l0 + P.col_mis[c0]) & 3;
+        a0[k] = l0 - sh;
+        const int ln = (cnt[k] + sh + 3) & ~3;
+        ok = ok && (cnt[k] == 0 || ((unsigned)cnt[k] <= (unsigned)P.col_cap[c0] && (a0[k] | ((int)P.col_n[c0] - a0[k] - ln)) >= 0));
+        len[k] = cnt[k] != 0 ? ln : 0;
+        total += (uint32_t)len[k] * (k == 0 ? 16u : 12u);
+    }
+    if (!ok) return false;
+    if (lane == 0) {
+        uint64_t* bar = nullptr;
+        const uint32_t bar_a = region_a;
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_a), "r"(total) : "memory");
+        (void)bar;
+#pragma unroll
+        for (int c = 0; c < (HAS_EL ? NCOL : 7); ++c) {
+            const int k = c < 4 ? 0 : (c < 7 ? 1 : 2);
+            if (len[k] != 0)
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                                 region_a + (uint32_t)P.col_dst[c]),
+                             "l"(P.col_ptr[c] + ((long long)a0[k] << 2)), "r"((uint32_t)len[k] << 2), "r"(bar_a)
+                             : "memory");
+        }
+    }
     return true;
 }
 
@@ -667,7 +670,8 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     ChainShared S;
     chain_shared_layout(P, CALIB, smem_raw, &S);
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const int warp = tid >> 5, lane = tid & 31, nwarp = nthr >> 5;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // through a shuffle: the compiler then knows it is warp-uniform
+    const int lane = tid & 31, nwarp = nthr >> 5;
     unsigned char* R = smem_raw + P.shared_bytes + (size_t)warp * P.region_bytes;   // this warp's staging region
     uint64_t* bar = (uint64_t*)R;
 
@@ -706,6 +710,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             }
             S.wscale[0] = sc; S.wscale[1] = inv;
             *S.since = 0u;
+            *S.next = 0u;
         }
     }
     __syncthreads();
@@ -748,16 +753,6 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             }
         }
     }
-    LaneCol col;
-    col.ptr = nullptr; col.off = nullptr; col.base = 0; col.n = 0; col.mis = 0; col.cap = 0; col.dst = 0;
-    if (lane < P.n_col) {
-        const int k = P.col_coll[lane];
-        col.off = P.off[k];
-        col.ptr = col.off ? P.col_ptr[lane] : nullptr;
-        col.base = P.col_base[lane]; col.n = P.col_n[lane];
-        col.mis = P.col_mis[lane]; col.cap = P.col_cap[lane];
-        col.dst = smem_u32(R + P.col_dst[lane]);
-    }
     __syncthreads();
 
     // this warp's buffers (shared-memory byte addresses)
@@ -771,34 +766,46 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     // so everything it does not ask for is compiled out
     const unsigned feat = FEAT >= 0 ? (unsigned)FEAT : chain_features(P);
 
-    const long long GW = (long long)gridDim.x * nwarp;
-    long long tile = (long long)warp * gridDim.x + blockIdx.x;
+    // Tile hand-out.  Every CTA owns a contiguous range of tiles and its warps draw from it through a shared-memory
+    // ticket, so a scheduler with one warp more than its neighbours (or a warp that met long events) simply takes
+    // fewer tiles; the last eighth of the launch is handed out by a global counter so that no SM idles at the end.
+    const bool dyn = P.tile_counter != nullptr;
+    const unsigned int per_cta = dyn ? (unsigned int)((P.n_tiles - P.n_tiles / 8) / gridDim.x)
+                                     : (unsigned int)((P.n_tiles + gridDim.x - 1) / gridDim.x);
+    const long long n_static = dyn ? (long long)per_cta * gridDim.x : P.n_tiles;
+    const long long cta_lo = (long long)blockIdx.x * per_cta;
+    const uint32_t next_a = smem_u32(S.next);
+    auto take_tile = [&]() -> long long {
+        unsigned int i = 0;
+        if (lane == 0) i = atom_add_shared_u32(next_a, 1u);
+        i = __shfl_sync(0xffffffffu, i, 0);
+        if (i < per_cta) return cta_lo + i < P.n_tiles ? cta_lo + i : P.n_tiles;
+        if (!dyn) return P.n_tiles;
+        unsigned int g = 0;
+        if (lane == 0) g = atom_add_global_u32(P.tile_counter, 1u);
+        return n_static + (long long)__shfl_sync(0xffffffffu, g, 0);
+    };
+    long long tile = take_tile();
     uint32_t parity = 0;
     int bsel = 0;
     bool fit = false;
-    long long cur_lo = 0;
     EventOffsets eo;
     eo.j0 = eo.j1 = eo.m0 = eo.m1 = eo.q0 = eo.q1 = 0;
+    // object counts of a tile from the per-lane offsets (lanes past the last event hold offsets[n_events])
+    auto tile_counts = [&](const EventOffsets& o, int (&lo)[3], int (&cnt)[3]) {
+        lo[0] = __shfl_sync(0xffffffffu, o.j0, 0); cnt[0] = __shfl_sync(0xffffffffu, o.j1, 31) - lo[0];
+        lo[1] = __shfl_sync(0xffffffffu, o.m0, 0); cnt[1] = __shfl_sync(0xffffffffu, o.m1, 31) - lo[1];
+        lo[2] = HAS_EL ? __shfl_sync(0xffffffffu, o.q0, 0) : 0;
+        cnt[2] = HAS_EL ? __shfl_sync(0xffffffffu, o.q1, 31) - lo[2] : 0;
+    };
     if (tile < P.n_tiles) {
-        long long lo, hi;
-        load_bounds(P, col, tile, lo, hi);
+        int lo[3], cnt[3];
         load_event_offsets<HAS_EL>(P, tile, lane, eo);
-        fit = P.n_col > 0 && issue_tile(col, lane, lo, hi, bar);
-        cur_lo = lo;
+        tile_counts(eo, lo, cnt);
+        fit = P.n_col > 0 && issue_tile<HAS_EL>(P, smem_u32(R), lane, lo, cnt);
     }
 
-    // The per-tile cost varies with the events, and purely static striding leaves warps waiting at the end.
-    // The first 7/8 of the tiles are strided statically; the rest is handed out by a global counter (ptxas turns the
-    // atomic into vote + leader + shuffle, i.e. an immediate wait for the round trip, so it is kept off most tiles).
-    const bool dyn = P.tile_counter != nullptr;
-    long long n_static = dyn ? (P.n_tiles - P.n_tiles / 8) / GW * GW : P.n_tiles;
-    if (dyn && n_static < GW) n_static = GW;          // every warp's first tile is static
-    long long tile_next = tile + GW;
-    if (tile_next >= n_static && dyn) {
-        unsigned int raw = 0;
-        if (lane == 0) raw = atom_add_global_u32(P.tile_counter, 1u);
-        tile_next = n_static + (long long)__shfl_sync(0xffffffffu, raw, 0);
-    }
+    long long tile_next = take_tile();
 
     for (; tile < P.n_tiles;) {
         const long long e0 = tile * TILE_EVENTS;
@@ -807,13 +814,9 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         const bool has_next = tile_next < P.n_tiles;
         float wt0 = 1.0f;                                                // weight column 0 of the lane's event, loaded early
         if ((feat & (F_SUMW | F_WEIGHTS)) == (F_SUMW | F_WEIGHTS) && lane < ne) wt0 = __ldg(P.weights + e0 + lane);
-        long long nlo = 0, nhi = 0;
         EventOffsets neo;
         neo.j0 = neo.j1 = neo.m0 = neo.m1 = neo.q0 = neo.q1 = 0;
-        if (has_next) {
-            load_bounds(P, col, tile_next, nlo, nhi);
-            load_event_offsets<HAS_EL>(P, tile_next, lane, neo);
-        }
+        if (has_next) load_event_offsets<HAS_EL>(P, tile_next, lane, neo);
         bool staged = fit;
         bool released = false;
         fit = false;
@@ -834,12 +837,15 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             const int kj0 = live ? eo.j0 - jb : 0, nj = live ? eo.j1 - eo.j0 : 0;
             const int km0 = eo.m0 - mb, nm = live ? eo.m1 - eo.m0 : 0;
             const int kq0 = eo.q0 - qb, nq = (HAS_EL && live) ? eo.q1 - eo.q0 : 0;
-            const int l0 = live ? km0 + kq0 : 0;
             const int c = nm + nq;          // every lepton gets a list entry; unselected ones can never match
+            const int npair = (c + 1) >> 1; // the list is padded to pairs with an entry that can never match
+            // every event's list starts at an even entry (16-byte aligned pairs): the running lepton count plus one
+            // possible pad entry per earlier event, rounded up to even
+            const int l0 = live ? (km0 + kq0 + lane + 1) & ~1 : 0;
             const unsigned longm = __ballot_sync(0xffffffffu, nj > TAIL_CUT);   // events whose tail the warp shares
-            // bucket the event's jets by its lepton count: position inside the bucket from a shared-memory
+            // bucket the event's jets by its number of lepton pairs: position inside the bucket from a shared-memory
             // counter (any order inside a bucket will do), bucket bases from the eight totals
-            const int key = c < N_BUCKETS - 1 ? c : N_BUCKETS - 1;
+            const int key = npair < N_BUCKETS - 1 ? npair : N_BUCKETS - 1;
             const uint32_t bk = bucket_a + (uint32_t)bsel * (4u * N_BUCKETS);
             int pos = 0;
             if (nj > 0) pos = (int)atom_add_shared_u32(bk + 4u * (unsigned)key, (unsigned)nj);
@@ -849,27 +855,42 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             mbar_wait(bar, parity);
             parity ^= 1u;
             if (staged) {
-                // combined (-eta, -phi) list of the event: muons then electrons; -eta = -inf marks "not selected"
-                // (deta^2 = inf, so dR^2 = inf or NaN and the minimum below ignores it)
-                uint32_t out = lep_a + 8u * (unsigned)l0;      // (l0 <= MAX_LIST by the capacities)
+                // combined (eta, phi) list of the event: muons then electrons; eta = +inf marks "not selected"
+                // (deta^2 = inf, so dR^2 = inf or NaN and the minimum below ignores it).  Straight-line predicated
+                // code for the first few leptons of each kind (a divergent loop costs more than the work it does).
+                const uint32_t out = lep_a + 8u * (unsigned)l0;      // (l0 <= MAX_LIST by the capacities)
                 {
-                    uint32_t a = a_mpt + 4u * (unsigned)km0;
-                    const uint32_t aend = a + 4u * (unsigned)nm;
+                    const uint32_t a = a_mpt + 4u * (unsigned)km0;
+                    constexpr int UNR_M = 5;
+#pragma unroll
+                    for (int k = 0; k < UNR_M; ++k)
+                        if (k < nm) {
+                            const float pt = lds_f32(a + 4u * k), eta = lds_f32(a + ms + 4u * k), phi = lds_f32(a + 2 * ms + 4u * k);
+                            sts_v2(out + 8u * k, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                        }
 #pragma unroll 1
-                    for (; a != aend; a += 4, out += 8) {
-                        const float pt = lds_f32(a), eta = lds_f32(a + ms), phi = lds_f32(a + 2 * ms);
-                        sts_v2(out, pt > P.lep_pt_min ? -eta : -CUDART_INF_F, -phi);
+                    for (int k = UNR_M; k < nm; ++k) {
+                        const float pt = lds_f32(a + 4u * k), eta = lds_f32(a + ms + 4u * k), phi = lds_f32(a + 2 * ms + 4u * k);
+                        sts_v2(out + 8u * k, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
                     }
                 }
                 if (HAS_EL) {
-                    uint32_t a = a_ept + 4u * (unsigned)kq0;
-                    const uint32_t aend = a + 4u * (unsigned)nq;
+                    const uint32_t a = a_ept + 4u * (unsigned)kq0;
+                    const uint32_t oe = out + 8u * (unsigned)nm;
+                    constexpr int UNR_E = 4;
+#pragma unroll
+                    for (int k = 0; k < UNR_E; ++k)
+                        if (k < nq) {
+                            const float pt = lds_f32(a + 4u * k), eta = lds_f32(a + es + 4u * k), phi = lds_f32(a + 2 * es + 4u * k);
+                            sts_v2(oe + 8u * k, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                        }
 #pragma unroll 1
-                    for (; a != aend; a += 4, out += 8) {
-                        const float pt = lds_f32(a), eta = lds_f32(a + es), phi = lds_f32(a + 2 * es);
-                        sts_v2(out, pt > P.lep_pt_min ? -eta : -CUDART_INF_F, -phi);
+                    for (int k = UNR_E; k < nq; ++k) {
+                        const float pt = lds_f32(a + 4u * k), eta = lds_f32(a + es + 4u * k), phi = lds_f32(a + 2 * es + 4u * k);
+                        sts_v2(oe + 8u * k, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
                     }
                 }
+                if (c & 1) sts_v2(out + 8u * (unsigned)c, CUDART_INF_F, 0.0f);     // pad entry
                 __syncwarp();       // bucket totals complete
                 const int4 t0 = lds_v4i(bk), t1 = lds_v4i(bk + 16);
                 int base = 0;
@@ -877,7 +898,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                 base += key > 4 ? t1.x : 0; base += key > 5 ? t1.y : 0; base += key > 6 ? t1.z : 0;
                 {
                     // per jet: byte offset in its column [10:0], byte offset [23:11] and byte length [31:24] of the list
-                    unsigned int word = (unsigned)(kj0 << 2) | ((unsigned)l0 << 14) | ((unsigned)c << 27);
+                    unsigned int word = (unsigned)(kj0 << 2) | ((unsigned)l0 << 14) | ((unsigned)npair << 28);
                     const uint32_t a0 = order_a + 4u * (unsigned)(base + pos);
                     uint32_t a = a0;
                     const uint32_t aend = a + 4u * (unsigned)(nj < TAIL_CUT ? nj : TAIL_CUT);
@@ -906,15 +927,11 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     uint32_t al = lep_a + ((word >> 11) & 0x1fffu);
                     const uint32_t alend = al + (word >> 24);
                     float dmin = CUDART_INF_F;
-                    if (word & (8u << 24)) {            // odd count: one lepton first, then pairs
-                        const float2 l = lds_v2(al);
-                        dmin = dr2_packed(make_float2(eta, phi), l);
-                        al += 8;
-                    }
 #pragma unroll 1
                     for (; al != alend; al += 16) {
-                        const float2 l = lds_v2(al), m = lds_v2(al + 8);
-                        dmin = fminf(dmin, fminf(dr2_packed(make_float2(eta, phi), l), dr2_packed(make_float2(eta, phi), m)));
+                        const float4 l = lds_v4(al);
+                        dmin = fminf(dmin, fminf(dr2_packed(make_float2(eta, phi), make_float2(l.x, l.y)),
+                                                 dr2_packed(make_float2(eta, phi), make_float2(l.z, l.w))));
                     }
                     const bool base_ok = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
                     if (!CALIB) {
@@ -929,7 +946,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                 __syncwarp();
                 if (P.out_jet_mask) {
                     // clean-jet mask, jets in their original order (coalesced bytes), from the verdicts just stored
-                    const long long lj0 = cur_lo_jets(P, cur_lo, lane) - P.jbase;
+                    const long long lj0 = __ldg(P.off[0] + e0) - P.jbase;
                     for (int j = lane; j < njt; j += 32) {
                         const float p = lds_f32(a_jpt + 4u * (unsigned)j);
                         if (!CALIB) {
@@ -1019,7 +1036,11 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         // the staging region is dead from here: start the next tile's copies under the finishing math
                         fence_proxy_async_smem();
                         __syncwarp();
-                        if (has_next && P.n_col > 0) fit = issue_tile(col, lane, nlo, nhi, bar);
+                        if (has_next && P.n_col > 0) {
+                            int nlo[3], ncnt[3];
+                            tile_counts(neo, nlo, ncnt);
+                            fit = issue_tile<HAS_EL>(P, region_a, lane, nlo, ncnt);
+                        }
                         released = true;
                     }
                     if (live)
@@ -1031,19 +1052,17 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         if (!released) {
             fence_proxy_async_smem();
             __syncwarp();
-            if (has_next && P.n_col > 0) fit = issue_tile(col, lane, nlo, nhi, bar);
+            if (has_next && P.n_col > 0) {
+                int nlo[3], ncnt[3];
+                tile_counts(neo, nlo, ncnt);
+                fit = issue_tile<HAS_EL>(P, smem_u32(R), lane, nlo, ncnt);
+            }
         }
         if (!staged && lane < ne) chain_event_global<CALIB>(P, smem_raw, e0 + lane);
         __syncwarp();
         eo = neo;
-        cur_lo = nlo;
         tile = tile_next;
-        tile_next += GW;
-        if (tile_next >= n_static && dyn) {
-            unsigned int raw = 0;
-            if (lane == 0) raw = atom_add_global_u32(P.tile_counter, 1u);
-            tile_next = n_static + (long long)__shfl_sync(0xffffffffu, raw, 0);
-        }
+        tile_next = take_tile();
 
         {   // the warp whose tile takes the CTA's event count across a multiple of flush_events flushes the histograms
             unsigned int c = 0;
@@ -1148,7 +1167,7 @@ static int chain_region_layout(ChainParams& P, const hepk_chain_desc* d, bool ca
     // the permutation is written after that and read until the region is released
     P.order_off = P.col_dst[4];
     if (o < (size_t)P.order_off + (size_t)cap_j * 4) o = (size_t)P.order_off + (size_t)cap_j * 4;
-    P.lep_off = take((size_t)(cap_m + cap_e + 4) * 8);
+    P.lep_off = take((size_t)(cap_m + cap_e + LIST_PAD) * 8);
     P.corr_off = take(calib ? (size_t)(cap_j + 8) * 4 : 0);
     P.bucket_off = take(2 * N_BUCKETS * 4);
     return (int)dev::align_up(o, 128);
@@ -1207,8 +1226,8 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (cap_j > MAX_JETS_TILE) cap_j = MAX_JETS_TILE;      // the jet's byte offset is packed in 11 bits
     if (cap_m < 4) cap_m = 4;
     if (has_el && cap_e < 4) cap_e = 4;
-    if (cap_m > 508) cap_m = 508;        // the list start (in bytes) is packed in 13 bits
-    if (cap_e > 508) cap_e = 508;        // 2 * 508 <= MAX_LIST, multiple of 4
+    if (cap_m > 492) cap_m = 492;        // the list start (in bytes) is packed in 13 bits
+    if (cap_e > 492) cap_e = 492;        // 2 * 492 + LIST_PAD <= MAX_LIST, multiple of 4
 
     const int smem_max = max_smem_optin();
     const int shared_bytes = (int)dev::chain_shared_layout(P, calib, nullptr, nullptr);
@@ -1240,11 +1259,11 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         if (P.col_ptr[c] && P.col_ptr[first] && P.col_mis[c] != P.col_mis[first]) P.n_col = 0;
     }
 
-    // CTA shape: as many warps per SM as shared memory allows (up to 16), in as few CTAs as possible so that
+    // CTA shape: as many warps per SM as shared memory allows (up to 20), in as few CTAs as possible so that
     // the privatised histograms are shared by many warps
     const int sm_total = smem_max + 1024;              // per SM; each CTA also pays 1 KB of system shared memory
     int best_ctas = 1, best_wpc = 1, best_total = 0;
-    const int max_warps_sm = d->tune_warps_per_sm > 0 ? d->tune_warps_per_sm : 16;
+    const int max_warps_sm = d->tune_warps_per_sm > 0 ? d->tune_warps_per_sm : 20;
     for (int ctas = 1; ctas <= 4; ++ctas) {
         if (d->tune_ctas_per_sm > 0 && ctas != d->tune_ctas_per_sm && !(ctas == 1 && d->tune_ctas_per_sm > 4)) continue;
         int budget = sm_total / ctas - 1024;
@@ -1262,7 +1281,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     P.wmax_bits = want_sumw ? (const unsigned int*)((const double*)workspace + n_sumw) : nullptr;
     P.tile_counter = want_sumw ? (unsigned int*)((double*)workspace + n_sumw) + 2 : nullptr;
 
-    // three register budgets: up to 16 warps per CTA (128 registers per thread), 20 (102) or 24 (85)
+    // two register budgets: up to 20 warps per CTA (96 registers per thread, no spills) or up to 24 (80)
     void (*kern)(ChainParams);
 #define HEPK_PICK(MAXT, FEAT)                                                                                        \
     (calib ? (has_el ? dev::chain_kernel<true, true, MAXT, FEAT> : dev::chain_kernel<true, false, MAXT, FEAT>)     \
@@ -1287,10 +1306,10 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (d->weights) feat_host |= dev::F_WEIGHTS;
     if (P.W > 1) feat_host |= dev::F_MULTIW;
     const bool common = (int)feat_host == FEAT_COMMON && !d->out_jet_mask && has_el;
-    if (wpc <= 16) kern = common ? (calib ? dev::chain_kernel<true, true, 512, FEAT_COMMON> : dev::chain_kernel<false, true, 512, FEAT_COMMON>)
-                                 : HEPK_PICK(512, -1);
-    else if (wpc <= 20) kern = HEPK_PICK(640, -1);
-    else kern = HEPK_PICK(768, -1);
+#define HEPK_PICK_COMMON(MAXT) (calib ? dev::chain_kernel<true, true, MAXT, FEAT_COMMON> : dev::chain_kernel<false, true, MAXT, FEAT_COMMON>)
+    if (wpc <= 20) kern = common ? HEPK_PICK_COMMON(640) : HEPK_PICK(640, -1);
+    else kern = common ? HEPK_PICK_COMMON(768) : HEPK_PICK(768, -1);
+#undef HEPK_PICK_COMMON
 #undef HEPK_PICK
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
