@@ -15,6 +15,9 @@
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 /* float32 constants of the dphi wrap (R6): PI_F = 0x40490FDB, TWO_PI_F = 0x40C90FDB. */
 static const float PI_F = 3.14159274101257324f;
@@ -306,6 +309,46 @@ int32_t hepo_fill_histogram(const float* data, const float* weights, int64_t n,
     return 0;
 }
 
+/* the same fill with the sum of squared weights per slot (the statistical
+ * uncertainty of a weighted bin); w*w in float64 from the float32 weight, one rounding at the end.
+ * weights == NULL: every weight is 1, so sumw2 == sumw == counts. */
+int32_t hepo_fill_histogram_w2(const float* data, const float* weights, int64_t n,
+                               const float* edges, int32_t nbins, float* sumw, float* sumw2, int64_t* counts)
+{
+    if (n < 0 || nbins < 1 || !edges || (n > 0 && !data)) return -1;
+    double* acc = (double*)calloc(2 * ((size_t)nbins + 2), sizeof(double));
+    if (!acc) return -1;
+    double* acc2 = acc + nbins + 2;
+    for (int64_t i = 0; i < n; ++i) {
+        int32_t s = hist_slot(data[i], edges, nbins);
+        double w = weights ? (double)weights[i] : 1.0;
+        acc[s] += w;
+        acc2[s] += w * w;
+        if (counts) counts[s] += 1;
+    }
+    for (int32_t s = 0; s < nbins + 2; ++s) {
+        if (sumw) sumw[s] = (float)((double)sumw[s] + acc[s]);
+        if (sumw2) sumw2[s] = (float)((double)sumw2[s] + acc2[s]);
+    }
+    free(acc);
+    return 0;
+}
+
+/* SURVEY.md 8(f-2), "event weight computation based on histogram lookups: pileup, lepton
+ * efficiency corrections": w_out[e] = w_in[e] * table[B(x[e])], B the clamped bin of hepo_lookup_binned (1-D),
+ * ONE float32 multiply (exact class).  w_in == NULL: w_in = 1. */
+int32_t hepo_event_weight_lookup(const float* w_in, const float* x, int64_t n,
+                                 const float* edges, int32_t nbins, const float* table, float* w_out)
+{
+    if (n < 0 || nbins < 1 || !edges || !table || (n > 0 && (!x || !w_out))) return -1;
+    for (int64_t e = 0; e < n; ++e) {
+        float f = table[find_bin_clamped(x[e], edges, nbins)];
+        float w = w_in ? w_in[e] : 1.0f;
+        w_out[e] = w * f;
+    }
+    return 0;
+}
+
 /* ------------------------------------------------------------------ c7: the fused chain, event by event
  * Steps follow the benchmark analysis list PAPER.md:L131-139 restricted to the hot path:
  * object selection (L132), jet-lepton dR matching (L133), jet corrections by histogram lookup
@@ -313,35 +356,35 @@ int32_t hepo_fill_histogram(const float* data, const float* weights, int64_t n,
  * weighted histograms (L139). */
 size_t hepo_chain_desc_size(void) { return sizeof(hepo_chain_desc); }
 
-int32_t hepo_analysis_chain(const hepo_chain_desc* d)
+/* slot prefix of the active observables; returns the slots per variant */
+static int64_t chain_hist_layout(const hepo_chain_desc* d, int64_t* obs_prefix)
 {
-    if (!d || d->n_events < 0 || d->n_variants < 1 || d->n_wvar < 1) return -1;
-    if (d->n_events > 0 && (!d->jets.offsets || !d->muons.offsets)) return -1;
-    if (!d->calib_table && d->n_variants != 1) return -1;
+    obs_prefix[0] = 0;
+    for (int o = 0; o < HEPO_N_OBS; ++o)
+        obs_prefix[o + 1] = obs_prefix[o] + (d->axis_edges[o] ? d->axis_nbins[o] + 2 : 0);
+    return obs_prefix[HEPO_N_OBS];
+}
+
+/* Events [e_begin, e_end) of the chain.  acc / acc2: float64 accumulators of sumw / sumw2 (NULL: not wanted),
+ * counts: int64 accumulators (NULL: not wanted), all in the layout of the descriptor's histogram arrays. */
+static int32_t chain_event_range(const hepo_chain_desc* d, int64_t e_begin, int64_t e_end,
+                                 double* acc, double* acc2, int64_t* counts)
+{
     const int64_t N = d->n_events;
     const int32_t V = d->n_variants, W = d->n_wvar;
     const int has_el = d->electrons.offsets != NULL;
     const float thr = d->dr_max * d->dr_max;
-
-    /* histogram layout */
     int64_t obs_prefix[HEPO_N_OBS + 1];
-    obs_prefix[0] = 0;
-    for (int o = 0; o < HEPO_N_OBS; ++o)
-        obs_prefix[o + 1] = obs_prefix[o] + (d->axis_edges[o] ? d->axis_nbins[o] + 2 : 0);
-    const int64_t slots_per_variant = obs_prefix[HEPO_N_OBS];
-    double* acc = NULL;
-    if (d->hist_sumw && slots_per_variant > 0) {
-        acc = (double*)calloc((size_t)(V * W * slots_per_variant), sizeof(double));
-        if (!acc) return -1;
-    }
+    const int64_t slots_per_variant = chain_hist_layout(d, obs_prefix);
 
     int64_t cap = 64;
     float* ptv = (float*)malloc((size_t)cap * sizeof(float));
     uint8_t* matched = (uint8_t*)malloc((size_t)cap);
     uint8_t* clean = (uint8_t*)malloc((size_t)cap);
     float* corr = (float*)malloc((size_t)cap * sizeof(float));
+    if (!ptv || !matched || !clean || !corr) { free(ptv); free(matched); free(clean); free(corr); return -1; }
 
-    for (int64_t iev = 0; iev < N; ++iev) {
+    for (int64_t iev = e_begin; iev < e_end; ++iev) {
         const int64_t j0 = d->jets.offsets[iev] - d->jets.content_base;
         const int64_t nj = d->jets.offsets[iev + 1] - d->jets.offsets[iev];
         if (nj > cap) {
@@ -372,6 +415,9 @@ int32_t hepo_analysis_chain(const hepo_chain_desc* d)
                 corr[k] = d->calib_table[(int64_t)bx * d->calib_neta + by];
             }
         }
+        /* event-weight factor from a 1-D lookup on a per-event column, variant independent */
+        float evw = 1.0f;
+        if (d->evw_table) evw = d->evw_table[find_bin_clamped(d->evw_x[iev], d->evw_edges, d->evw_nbins)];
         for (int32_t v = 0; v < V; ++v) {
             int32_t njet = 0, arg = -1;
             double ht = 0.0;
@@ -416,22 +462,108 @@ int32_t hepo_analysis_chain(const hepo_chain_desc* d)
                 if (!d->axis_edges[ob]) continue;
                 const int32_t nb = d->axis_nbins[ob];
                 const int32_t s = hist_slot(obs[ob], d->axis_edges[ob], nb);
-                if (d->hist_counts) d->hist_counts[(int64_t)v * slots_per_variant + obs_prefix[ob] + s] += 1;
-                if (acc)
+                if (counts) counts[(int64_t)v * slots_per_variant + obs_prefix[ob] + s] += 1;
+                if (acc || acc2)
                     for (int32_t w = 0; w < W; ++w) {
-                        double wt = d->weights ? (double)d->weights[(int64_t)w * N + iev] : 1.0;
-                        acc[((int64_t)v * slots_per_variant + obs_prefix[ob]) * W + (int64_t)w * (nb + 2) + s] += wt;
+                        float wf = d->weights ? d->weights[(int64_t)w * N + iev] : 1.0f;
+                        if (d->evw_table) wf = wf * evw;        /* float32 multiply (hepo_event_weight_lookup) */
+                        const double wt = (double)wf;
+                        const int64_t slot = ((int64_t)v * slots_per_variant + obs_prefix[ob]) * W + (int64_t)w * (nb + 2) + s;
+                        if (acc) acc[slot] += wt;
+                        if (acc2) acc2[slot] += wt * wt;
                     }
             }
         }
     }
-    if (acc) {
-        const int64_t total = (int64_t)V * W * slots_per_variant;
-        for (int64_t i = 0; i < total; ++i) d->hist_sumw[i] = (float)((double)d->hist_sumw[i] + acc[i]);
-        free(acc);
-    }
     free(ptv); free(matched); free(clean); free(corr);
     return 0;
+}
+
+static int chain_args_ok(const hepo_chain_desc* d)
+{
+    if (!d || d->n_events < 0 || d->n_variants < 1 || d->n_wvar < 1) return 0;
+    if (d->n_events > 0 && (!d->jets.offsets || !d->muons.offsets)) return 0;
+    if (!d->calib_table && d->n_variants != 1) return 0;
+    if (d->evw_table && (!d->evw_x || !d->evw_edges || d->evw_nbins < 1)) return 0;
+    return 1;
+}
+
+int32_t hepo_analysis_chain(const hepo_chain_desc* d)
+{
+    if (!chain_args_ok(d)) return -1;
+    int64_t obs_prefix[HEPO_N_OBS + 1];
+    const int64_t total = (int64_t)d->n_variants * d->n_wvar * chain_hist_layout(d, obs_prefix);
+    double *acc = NULL, *acc2 = NULL;
+    if (d->hist_sumw && total > 0) { acc = (double*)calloc((size_t)total, sizeof(double)); if (!acc) return -1; }
+    if (d->hist_sumw2 && total > 0) { acc2 = (double*)calloc((size_t)total, sizeof(double)); if (!acc2) { free(acc); return -1; } }
+    const int32_t rc = chain_event_range(d, 0, d->n_events, acc, acc2, d->hist_counts);
+    if (rc == 0) {
+        for (int64_t i = 0; acc && i < total; ++i) d->hist_sumw[i] = (float)((double)d->hist_sumw[i] + acc[i]);
+        for (int64_t i = 0; acc2 && i < total; ++i) d->hist_sumw2[i] = (float)((double)d->hist_sumw2[i] + acc2[i]);
+    }
+    free(acc); free(acc2);
+    return rc;
+}
+
+/* The same chain on all host cores (Listing 1's `prange` over events; Table I's thread columns):
+ * contiguous event blocks, one per thread, each through chain_event_range with PRIVATE histogram accumulators
+ * that are merged in thread order afterwards.  Per-event outputs are identical to the single-thread function's;
+ * counts are identical; sumw / sumw2 differ only in the order of the float64 additions.  A timing baseline
+ * (bench.py cpu_baseline); the single-thread function stays the checker. */
+int32_t hepo_omp_max_threads(void)
+{
+#ifdef _OPENMP
+    return (int32_t)omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+int32_t hepo_analysis_chain_omp(const hepo_chain_desc* d, int32_t n_threads)
+{
+    if (!chain_args_ok(d)) return -1;
+    if (n_threads < 1) n_threads = hepo_omp_max_threads();
+    int64_t obs_prefix[HEPO_N_OBS + 1];
+    const int64_t spv = chain_hist_layout(d, obs_prefix);
+    const int64_t total = (int64_t)d->n_variants * d->n_wvar * spv;
+    const int64_t ctotal = (int64_t)d->n_variants * spv;
+    const int want1 = d->hist_sumw && total > 0, want2 = d->hist_sumw2 && total > 0, wantc = d->hist_counts && ctotal > 0;
+    double* acc = want1 ? (double*)calloc((size_t)(total * n_threads), sizeof(double)) : NULL;
+    double* acc2 = want2 ? (double*)calloc((size_t)(total * n_threads), sizeof(double)) : NULL;
+    int64_t* cnt = wantc ? (int64_t*)calloc((size_t)(ctotal * n_threads), sizeof(int64_t)) : NULL;
+    if ((want1 && !acc) || (want2 && !acc2) || (wantc && !cnt)) { free(acc); free(acc2); free(cnt); return -1; }
+    int32_t rc = 0;
+    const int64_t N = d->n_events;
+#ifdef _OPENMP
+#pragma omp parallel for num_threads(n_threads) schedule(static, 1)
+#endif
+    for (int32_t t = 0; t < n_threads; ++t) {
+        const int64_t e0 = N * t / n_threads, e1 = N * (t + 1) / n_threads;
+        const int32_t r = chain_event_range(d, e0, e1, acc ? acc + total * t : NULL, acc2 ? acc2 + total * t : NULL,
+                                            cnt ? cnt + ctotal * t : NULL);
+        if (r != 0) {
+#ifdef _OPENMP
+#pragma omp critical
+#endif
+            rc = r;
+        }
+    }
+    if (rc == 0) {
+        for (int64_t i = 0; acc && i < total; ++i) {
+            double s = 0.0;
+            for (int32_t t = 0; t < n_threads; ++t) s += acc[total * t + i];
+            d->hist_sumw[i] = (float)((double)d->hist_sumw[i] + s);
+        }
+        for (int64_t i = 0; acc2 && i < total; ++i) {
+            double s = 0.0;
+            for (int32_t t = 0; t < n_threads; ++t) s += acc2[total * t + i];
+            d->hist_sumw2[i] = (float)((double)d->hist_sumw2[i] + s);
+        }
+        for (int64_t i = 0; cnt && i < ctotal; ++i)
+            for (int32_t t = 0; t < n_threads; ++t) d->hist_counts[i] += cnt[ctotal * t + i];
+    }
+    free(acc); free(acc2); free(cnt);
+    return rc;
 }
 
 /* ---- SURVEY.md 8(f-1) ---------------------------------------------------------------------------------- */
@@ -545,6 +677,31 @@ int32_t hepo_fill_histogram_2d(const float* x, const float* y, const float* weig
     }
     if (sumw)
         for (size_t s = 0; s < slots; ++s) sumw[s] = (float)((double)sumw[s] + acc[s]);
+    free(acc);
+    return 0;
+}
+
+/* the same with the sum of squared weights per slot (see hepo_fill_histogram_w2) */
+int32_t hepo_fill_histogram_2d_w2(const float* x, const float* y, const float* weights, int64_t n,
+                                  const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                                  float* sumw, float* sumw2, int64_t* counts)
+{
+    if (n < 0 || nx < 1 || ny < 1 || !edges_x || !edges_y || (n > 0 && (!x || !y))) return -1;
+    const size_t slots = ((size_t)nx + 2) * ((size_t)ny + 2);
+    double* acc = (double*)calloc(2 * slots, sizeof(double));
+    if (!acc) return -1;
+    double* acc2 = acc + slots;
+    for (int64_t i = 0; i < n; ++i) {
+        const size_t s = (size_t)hist_slot(x[i], edges_x, nx) * ((size_t)ny + 2) + (size_t)hist_slot(y[i], edges_y, ny);
+        const double w = weights ? (double)weights[i] : 1.0;
+        acc[s] += w;
+        acc2[s] += w * w;
+        if (counts) counts[s] += 1;
+    }
+    for (size_t s = 0; s < slots; ++s) {
+        if (sumw) sumw[s] = (float)((double)sumw[s] + acc[s]);
+        if (sumw2) sumw2[s] = (float)((double)sumw2[s] + acc2[s]);
+    }
     free(acc);
     return 0;
 }

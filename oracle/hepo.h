@@ -73,6 +73,18 @@ int32_t hepo_lookup_binned(const float* x, const float* y, int64_t n,
 int32_t hepo_fill_histogram(const float* data, const float* weights, int64_t n,
                             const float* edges, int32_t nbins, float* sumw, int64_t* counts);
 
+/* fill_histogram with the sum of squared weights: sumw2[slot] += w*w, float64
+ * accumulation of the float32 weight's square, rounded once; weights == NULL: w = 1 (sumw2 == sumw == counts).
+ * sumw, sumw2, counts each nullable, all accumulate. */
+int32_t hepo_fill_histogram_w2(const float* data, const float* weights, int64_t n,
+                               const float* edges, int32_t nbins, float* sumw, float* sumw2, int64_t* counts);
+
+/* Event weight from a histogram lookup ("event weight computation based on
+ * histogram lookups: pileup, lepton efficiency corrections"): w_out[e] = w_in[e] * table[B(x[e])], one float32
+ * multiply, B the clamped bin of hepo_lookup_binned; w_in == NULL: w_in = 1. */
+int32_t hepo_event_weight_lookup(const float* w_in, const float* x, int64_t n,
+                                 const float* edges, int32_t nbins, const float* table, float* w_out);
+
 /* ---- fused chain (PAPER.md:L129-139 for the analysis steps) ---- */
 enum { HEPO_OBS_NJET = 0, HEPO_OBS_HT, HEPO_OBS_MAXPT, HEPO_OBS_MINPT, HEPO_OBS_MJJ, HEPO_OBS_SUBPT, HEPO_N_OBS };
 
@@ -106,10 +118,26 @@ typedef struct {
     uint8_t* out_jet_mask;        /* [n_variants][jets.n_objects] clean-jet mask */
     /* histograms (accumulate): sumw [V][active obs o][n_wvar][nbins_o+2]; counts [V][active obs o][nbins_o+2] */
     float* hist_sumw; int64_t* hist_counts;
+    /* optional per-event weight factor from a 1-D lookup on a per-event column,
+     * factor[e] = evw_table[B(evw_x[e])] (clamped bin of hepo_lookup_binned), multiplied into every weight column
+     * with ONE float32 multiply before the fill (weights NULL: 1.0f * factor).  evw_table == NULL: none. */
+    const float* evw_x;           /* [n_events] */
+    const float* evw_edges;       /* [evw_nbins+1] */
+    int32_t evw_nbins;
+    const float* evw_table;       /* [evw_nbins] */
+    /* sum of squared (final) weights per slot, layout of hist_sumw, accumulates; NULL = not wanted */
+    float* hist_sumw2;
 } hepo_chain_desc;
 
 int32_t hepo_analysis_chain(const hepo_chain_desc* d);
 size_t  hepo_chain_desc_size(void);
+
+/* The same computation on n_threads host threads (<= 0: all; OpenMP `parallel for` over contiguous event blocks,
+ * PAPER.md:L66-68 `prange`), per-thread private histograms merged in thread order.  TIMING BASELINE for bench.py;
+ * hepo_analysis_chain stays the checker.  Per-event outputs and counts equal the single-thread results exactly,
+ * sumw / sumw2 up to the order of the float64 additions. */
+int32_t hepo_analysis_chain_omp(const hepo_chain_desc* d, int32_t n_threads);
+int32_t hepo_omp_max_threads(void);
 
 /* ---- the remaining generic kernels of the paper's list ------------------------------
  *
@@ -153,6 +181,9 @@ int32_t hepo_lookup_interp(const float* x, int64_t n, const float* xs, const flo
 int32_t hepo_fill_histogram_2d(const float* x, const float* y, const float* weights, int64_t n,
                                const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
                                float* sumw, int64_t* counts);
+int32_t hepo_fill_histogram_2d_w2(const float* x, const float* y, const float* weights, int64_t n,
+                                  const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                                  float* sumw, float* sumw2, int64_t* counts);
 
 /* ---- jet-triplet candidate -------------------------------------------------------------
  *

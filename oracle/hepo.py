@@ -161,6 +161,31 @@ def fill_histogram(data, weights, edges, sumw=None, counts=None):
     return sumw, counts
 
 
+def fill_histogram_w2(data, weights, edges, sumw=None, sumw2=None, counts=None):
+    """Returns (sumw, sumw2 float32[nbins+2], counts int64[nbins+2]); all accumulate into the arrays passed in."""
+    data, weights, edges = _f32(data), _f32(weights), _f32(edges)
+    nbins = edges.shape[0] - 1
+    if sumw is None:
+        sumw = np.zeros(nbins + 2, dtype=np.float32)
+    if sumw2 is None:
+        sumw2 = np.zeros(nbins + 2, dtype=np.float32)
+    if counts is None:
+        counts = np.zeros(nbins + 2, dtype=np.int64)
+    _check(lib().hepo_fill_histogram_w2(_p(data, np.float32), _p(weights, np.float32), C.c_int64(data.shape[0]),
+                                        _p(edges, np.float32), C.c_int32(nbins), _p(sumw, np.float32),
+                                        _p(sumw2, np.float32), _p(counts, np.int64)))
+    return sumw, sumw2, counts
+
+
+def event_weight_lookup(w_in, x, edges, table):
+    w_in, x, edges, table = _f32(w_in), _f32(x), _f32(edges), _f32(table)
+    out = np.empty(x.shape[0], dtype=np.float32)
+    _check(lib().hepo_event_weight_lookup(_p(w_in, np.float32), _p(x, np.float32), C.c_int64(x.shape[0]),
+                                          _p(edges, np.float32), C.c_int32(edges.shape[0] - 1), _p(table, np.float32),
+                                          _p(out, np.float32)))
+    return out
+
+
 def lookup_interp(x, xs, ys):
     x, xs, ys = _f32(x), _f32(xs), _f32(ys)
     out = np.empty(x.shape[0], dtype=np.float32)
@@ -181,6 +206,22 @@ def fill_histogram_2d(x, y, weights, edges_x, edges_y, sumw=None, counts=None):
                                         _p(edges_x, np.float32), C.c_int32(nx), _p(edges_y, np.float32), C.c_int32(ny),
                                         _p(sumw, np.float32), _p(counts, np.int64)))
     return sumw, counts
+
+
+def fill_histogram_2d_w2(x, y, weights, edges_x, edges_y, sumw=None, sumw2=None, counts=None):
+    """Returns (sumw, sumw2 float32[nx+2][ny+2], counts int64[nx+2][ny+2]); all accumulate."""
+    x, y, weights, edges_x, edges_y = _f32(x), _f32(y), _f32(weights), _f32(edges_x), _f32(edges_y)
+    nx, ny = edges_x.shape[0] - 1, edges_y.shape[0] - 1
+    if sumw is None:
+        sumw = np.zeros((nx + 2, ny + 2), dtype=np.float32)
+    if sumw2 is None:
+        sumw2 = np.zeros((nx + 2, ny + 2), dtype=np.float32)
+    if counts is None:
+        counts = np.zeros((nx + 2, ny + 2), dtype=np.int64)
+    _check(lib().hepo_fill_histogram_2d_w2(_p(x, np.float32), _p(y, np.float32), _p(weights, np.float32), C.c_int64(x.shape[0]),
+                                           _p(edges_x, np.float32), C.c_int32(nx), _p(edges_y, np.float32), C.c_int32(ny),
+                                           _p(sumw, np.float32), _p(sumw2, np.float32), _p(counts, np.int64)))
+    return sumw, sumw2, counts
 
 
 def triplet_mass(pt, eta, phi, mass, offsets, target, mask_rows=None, mask_content=None, content_base=0):
@@ -226,6 +267,8 @@ class ChainDesc(C.Structure):
         ("out_mjj", C.c_void_p), ("out_subpt", C.c_void_p),
         ("out_jet_mask", C.c_void_p),
         ("hist_sumw", C.c_void_p), ("hist_counts", C.c_void_p),
+        ("evw_x", C.c_void_p), ("evw_edges", C.c_void_p), ("evw_nbins", C.c_int32), ("evw_table", C.c_void_p),
+        ("hist_sumw2", C.c_void_p),
     ]
 
 
@@ -257,11 +300,18 @@ def hist_layout(hists, axes, n_variants, n_wvar):
     return prefix, tot
 
 
-def analysis_chain(wl, e0=0, e1=None, want_mask=True, hist_sumw=None, hist_counts=None):
+def max_threads():
+    return int(lib().hepo_omp_max_threads())
+
+
+def analysis_chain(wl, e0=0, e1=None, want_mask=True, hist_sumw=None, hist_counts=None, evw=None, want_sumw2=False,
+                   hist_sumw2=None, threads=1):
     """Run the oracle chain on events [e0, e1) of a hepgen.Workload.
 
     Returns a dict with per-event outputs [V][n], jet_mask [V][Mj] (whole collection; only rows of the
     event range are written), hist_sumw (flat float32) and hist_counts (flat int64), plus 'layout'.
+    evw: optional dict(x=float32[n_events], edges=float32[nb+1], table=float32[nb]) — the per-event weight factor
+    from a lookup; want_sumw2: also return hist_sumw2; threads != 1: the OpenMP timing leg (<= 0: all cores).
     """
     keep = []
     if e1 is None:
@@ -314,7 +364,20 @@ def analysis_chain(wl, e0=0, e1=None, want_mask=True, hist_sumw=None, hist_count
     if hist_counts is None:
         hist_counts = np.zeros(V * spv, np.int64)
     d.hist_sumw, d.hist_counts = hist_sumw.ctypes.data, hist_counts.ctypes.data
-    _check(lib().hepo_analysis_chain(C.byref(d)))
+    if evw is not None:
+        ex = np.ascontiguousarray(np.asarray(evw["x"], dtype=np.float32)[e0:e1])
+        ee, et = _f32(evw["edges"]), _f32(evw["table"])
+        keep += [ex, ee, et]
+        d.evw_x, d.evw_edges, d.evw_nbins, d.evw_table = ex.ctypes.data, ee.ctypes.data, ee.shape[0] - 1, et.ctypes.data
+    if want_sumw2 or hist_sumw2 is not None:
+        if hist_sumw2 is None:
+            hist_sumw2 = np.zeros(V * W * spv, np.float32)
+        d.hist_sumw2 = hist_sumw2.ctypes.data
+        out["hist_sumw2"] = hist_sumw2
+    if threads == 1:
+        _check(lib().hepo_analysis_chain(C.byref(d)))
+    else:
+        _check(lib().hepo_analysis_chain_omp(C.byref(d), C.c_int32(threads)))
     out["hist_sumw"], out["hist_counts"] = hist_sumw, hist_counts
     out["layout"] = dict(prefix=prefix, slots_per_variant=spv, n_variants=V, n_wvar=W)
     return out

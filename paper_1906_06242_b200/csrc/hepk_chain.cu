@@ -384,7 +384,9 @@ __device__ __forceinline__ void add_weight(const ChainParams& P, unsigned feat, 
 
 // Per event and variant: leading-pair mass, outputs, histograms.  Shared by the staged path and the per-event
 // path.  The leading jets' (eta, phi, mass) are passed in by value; i2 < 0 means fewer than two clean jets.
-__device__ __forceinline__ void finish_event(const ChainParams& P, const ChainShared& S, unsigned feat, long long ev, int v, float wt0,
+template <int NW>
+__device__ __forceinline__ void finish_event(const ChainParams& P, const ChainShared& S, unsigned feat, long long ev, int v,
+                                             const float (&wt)[NW],
                                              int cnt, float sum, float mn, float b1, float b2, int i1, int i2,
                                              float eta1, float phi1, float m1, float eta2, float phi2, float m2)
 {
@@ -423,9 +425,16 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     bin[HEPK_OBS_SUBPT] = obs_bin<HEPK_OBS_SUBPT>(P, S, feat, v, subpt);
     if (!(feat & F_SUMW)) return;
     const float wscale = lds_f32(smem_u32(S.wscale));
-    add_weight(P, feat, bin, 0, wt0, wscale);
+    add_weight(P, feat, bin, 0, wt[0], wscale);
     if ((feat & (F_WEIGHTS | F_MULTIW)) != (F_WEIGHTS | F_MULTIW)) return;
-    for (int w = 1; w < P.W; ++w) add_weight(P, feat, bin, w, __ldg(P.weights + (long long)w * P.n_events + ev), wscale);
+    if (NW > 1) {
+        // the event's weights were loaded once per tile and serve every variant and observable
+#pragma unroll
+        for (int w = 1; w < NW; ++w)
+            if (w < P.W) add_weight(P, feat, bin, w, wt[w], wscale);
+    } else {
+        for (int w = 1; w < P.W; ++w) add_weight(P, feat, bin, w, __ldg(P.weights + (long long)w * P.n_events + ev), wscale);
+    }
 }
 
 // Order-preserving map float -> unsigned (and back): a < b  <=>  ord_key(a) < ord_key(b); no finite value maps to 0.
@@ -567,7 +576,8 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, unsigned c
             e1 = P.jeta[x]; p1 = P.jphi[x]; m1 = P.jmass[x];
             e2 = P.jeta[y]; p2 = P.jphi[y]; m2 = P.jmass[y];
         }
-        finish_event(P, S, chain_features(P), ev, v, P.weights ? __ldg(P.weights + ev) : 1.0f, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
+        const float wt[1] = {P.weights ? __ldg(P.weights + ev) : 1.0f};
+        finish_event<1>(P, S, chain_features(P), ev, v, wt, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
     }
 }
 
@@ -663,7 +673,8 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
     return true;
 }
 
-template <bool CALIB, bool HAS_EL, int MAXT, int FEAT>
+// NW: weight columns of an event kept in registers (1, or HEPK_MAX_WVAR for launches with several columns)
+template <bool CALIB, bool HAS_EL, int MAXT, int FEAT, int NW = 1>
 __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ ChainParams P)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -812,8 +823,13 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         const long long rest = P.n_events - e0;
         const int ne = rest < TILE_EVENTS ? (int)rest : TILE_EVENTS;
         const bool has_next = tile_next < P.n_tiles;
-        float wt0 = 1.0f;                                                // weight column 0 of the lane's event, loaded early
-        if ((feat & (F_SUMW | F_WEIGHTS)) == (F_SUMW | F_WEIGHTS) && lane < ne) wt0 = __ldg(P.weights + e0 + lane);
+        float wt[NW];                                                    // weights of the lane's event, loaded early
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+            wt[w] = 1.0f;
+            if ((feat & (F_SUMW | F_WEIGHTS)) == (F_SUMW | F_WEIGHTS) && lane < ne && w < P.W)
+                wt[w] = __ldg(P.weights + (long long)w * P.n_events + e0 + lane);
+        }
         EventOffsets neo;
         neo.j0 = neo.j1 = neo.m0 = neo.m1 = neo.q0 = neo.q1 = 0;
         if (has_next) load_event_offsets<HAS_EL>(P, tile_next, lane, neo);
@@ -1044,7 +1060,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         released = true;
                     }
                     if (live)
-                        finish_event(P, S, feat, e0 + lane, v, wt0, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
+                        finish_event<NW>(P, S, feat, e0 + lane, v, wt, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
                 }
             }
             bsel ^= 1;
@@ -1307,7 +1323,12 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (P.W > 1) feat_host |= dev::F_MULTIW;
     const bool common = (int)feat_host == FEAT_COMMON && !d->out_jet_mask && has_el;
 #define HEPK_PICK_COMMON(MAXT) (calib ? dev::chain_kernel<true, true, MAXT, FEAT_COMMON> : dev::chain_kernel<false, true, MAXT, FEAT_COMMON>)
-    if (wpc <= 20) kern = common ? HEPK_PICK_COMMON(640) : HEPK_PICK(640, -1);
+    // several weight columns and few warps (large histograms): a build that keeps the event's weights in registers
+    const bool multiw = P.W > 1 && d->weights && wpc <= 12;
+    if (multiw)
+        kern = calib ? (has_el ? dev::chain_kernel<true, true, 384, -1, HEPK_MAX_WVAR> : dev::chain_kernel<true, false, 384, -1, HEPK_MAX_WVAR>)
+                     : (has_el ? dev::chain_kernel<false, true, 384, -1, HEPK_MAX_WVAR> : dev::chain_kernel<false, false, 384, -1, HEPK_MAX_WVAR>);
+    else if (wpc <= 20) kern = common ? HEPK_PICK_COMMON(640) : HEPK_PICK(640, -1);
     else kern = common ? HEPK_PICK_COMMON(768) : HEPK_PICK(768, -1);
 #undef HEPK_PICK_COMMON
 #undef HEPK_PICK
