@@ -205,17 +205,33 @@ typedef struct hepk_chain_desc {
      *   hist_sumw   float32 [n_variants][active o][n_wvar][nbins_o+2]
      *   hist_counts int64   [n_variants][active o][nbins_o+2] */
     float* hist_sumw; int64_t* hist_counts;
-    /* tuning / test hooks; 0 = automatic */
+    /* SURVEY.md 8(f-2), PAPER.md:L134 ("event weight computation based on histogram lookups: pileup, lepton
+     * efficiency corrections"): optional per-event weight factor f[e] = evw_table[B(evw_x[e])] (B: the clamped
+     * bin of hepk_lookup_binned, 1-D), multiplied into every weight column with ONE float32 multiply before the
+     * fill (weights == NULL: 1.0f * f).  evw_x: float32[n_events]; evw_edges: float32[evw_nbins+1] ascending;
+     * evw_table: float32[evw_nbins], NULL = no factor; evw_nbins <= 4096. */
+    const float* evw_x; const float* evw_edges; int32_t evw_nbins; const float* evw_table;
+    /* sum of squared (final) weights per slot (the uncertainty of a weighted bin), layout of
+     * hist_sumw, accumulates; NULL = not wanted.  Without weights and factor it equals the counts. */
+    float* hist_sumw2;
+    /* RESERVED for the library's own tests (staging capacities and CTA shape); leave 0 = automatic */
     int32_t tune_cap_jets;       /* shared-memory capacity (jets per staged 32-event tile) */
     int32_t tune_cap_leptons;    /* capacity per lepton collection */
     int32_t tune_ctas_per_sm;    /* persistent CTAs per SM */
     int32_t tune_warps_per_cta;  /* warps (each owning its own tiles and staging region) per CTA, at most 24 */
     int32_t tune_warps_per_sm;   /* resident warps per SM the launch aims for (default 20) */
+    int32_t tune_variants_per_pass; /* variants per kernel launch (default: all, fewer when the histograms crowd out the warps) */
 } hepk_chain_desc;
 
 /* `d` is a HOST pointer to a descriptor whose array pointers are DEVICE pointers.  `workspace` is a
- * device buffer of at least hepk_chain_workspace_bytes(d) bytes (float64 histogram accumulators),
- * private to this call until the stream reaches its end. */
+ * device buffer of at least hepk_chain_workspace_bytes(d) bytes (64-bit histogram accumulators; needed
+ * whenever a histogram output is asked for), private to this call until the stream reaches its end.
+ *
+ * Weighted bins (tolerance class): when all weight columns (times the lookup factor) are finite and span
+ * at most a factor 8 in magnitude, entries are accumulated in fixed point — each entry rounded once to
+ * a multiple of 2^-k >= 2^-20 max|w|, exact integer sums, order independent — which bounds the error of a
+ * bin by 7.7e-6 of its smallest entry times the entries it holds; otherwise bins are float32 partial sums
+ * of at most ~1000 entries merged in float64.  Either way |error| <= 1e-5 * sum|w_i| of the bin. */
 size_t  hepk_chain_workspace_bytes(const hepk_chain_desc* d);
 int32_t hepk_analysis_chain(const hepk_chain_desc* d, void* workspace, size_t workspace_bytes, void* stream);
 

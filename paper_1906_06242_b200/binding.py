@@ -50,8 +50,11 @@ class ChainDesc(C.Structure):
         ("out_mjj", C.c_void_p), ("out_subpt", C.c_void_p),
         ("out_jet_mask", C.c_void_p),
         ("hist_sumw", C.c_void_p), ("hist_counts", C.c_void_p),
+        ("evw_x", C.c_void_p), ("evw_edges", C.c_void_p), ("evw_nbins", C.c_int32), ("evw_table", C.c_void_p),
+        ("hist_sumw2", C.c_void_p),
         ("tune_cap_jets", C.c_int32), ("tune_cap_leptons", C.c_int32),
         ("tune_ctas_per_sm", C.c_int32), ("tune_warps_per_cta", C.c_int32), ("tune_warps_per_sm", C.c_int32),
+        ("tune_variants_per_pass", C.c_int32),
     ]
 
 
@@ -330,6 +333,7 @@ class ChainInputs:
     hists: tuple                            # names from OBSERVABLES
     axes: dict                              # name -> float32 device tensor of edges
     calib: dict | None = None               # pt_edges, eta_edges, table (device), scales (list of float)
+    evw: dict | None = None                 # event-weight lookup: x [n_events], edges [nb+1], table [nb] (device float32)
 
     @property
     def n_variants(self):
@@ -387,7 +391,7 @@ class ChainPlan:
     EVENT_OUTPUTS = ("njet", "argmax", "ht", "maxpt", "minpt", "mjj", "subpt")
 
     def __init__(self, inp: ChainInputs, want_event_outputs=True, want_mask=False, want_hists=True, want_counts=True,
-                 tune=None):
+                 want_sumw2=False, tune=None):
         """want_event_outputs: True (all seven), False (none) or a tuple of names from EVENT_OUTPUTS."""
         self.inp = inp
         dev = inp.jets.pt.device
@@ -435,6 +439,16 @@ class ChainPlan:
             if want_counts:
                 self.out["hist_counts"] = torch.zeros(V * self.spv, dtype=torch.int64, device=dev)
                 d.hist_counts = self.out["hist_counts"].data_ptr()
+            if want_sumw2:
+                self.out["hist_sumw2"] = torch.zeros(V * W * self.spv, dtype=torch.float32, device=dev)
+                d.hist_sumw2 = self.out["hist_sumw2"].data_ptr()
+        if inp.evw is not None:
+            for k in ("x", "edges", "table"):
+                t = inp.evw[k]
+                assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32, k
+            assert inp.evw["x"].numel() == N and inp.evw["table"].numel() == inp.evw["edges"].numel() - 1
+            d.evw_x, d.evw_edges = inp.evw["x"].data_ptr(), inp.evw["edges"].data_ptr()
+            d.evw_nbins, d.evw_table = inp.evw["table"].numel(), inp.evw["table"].data_ptr()
         for k, v in (tune or {}).items():
             setattr(d, "tune_" + k, int(v))
         self.desc = d
@@ -443,7 +457,7 @@ class ChainPlan:
         self.V, self.W = V, W
 
     def zero_hists(self):
-        for k in ("hist_sumw", "hist_counts"):
+        for k in ("hist_sumw", "hist_sumw2", "hist_counts"):
             if k in self.out:
                 self.out[k].zero_()
 
@@ -475,7 +489,9 @@ class HostChainPlan:
     All inputs and outputs are host tensors; the C library does the host->device copies, the kernels and the
     device->host copies.  `wl` needs the attributes of hepgen.Workload (numpy arrays)."""
 
-    def __init__(self, wl, batch_events, want_event_outputs=True, want_hists=True, want_counts=True, device="cuda"):
+    def __init__(self, wl, batch_events, want_event_outputs=True, want_hists=True, want_counts=True, want_sumw2=False,
+                 evw=None, device="cuda"):
+        """evw: optional dict(x, edges, table) of numpy float32 arrays (the event-weight lookup)."""
         pin = lambda a: torch.from_numpy(a).pin_memory()
         self.keep = []
         self.h2d_bytes = 0
@@ -540,6 +556,15 @@ class HostChainPlan:
                 self.out["hist_counts"] = torch.zeros(V * self.spv, dtype=torch.int64).pin_memory()
                 d.hist_counts = self.out["hist_counts"].data_ptr()
                 self.d2h_bytes += self.out["hist_counts"].numel() * 8
+            if want_sumw2:
+                self.out["hist_sumw2"] = torch.zeros(V * W * self.spv, dtype=torch.float32).pin_memory()
+                d.hist_sumw2 = self.out["hist_sumw2"].data_ptr()
+                self.d2h_bytes += self.out["hist_sumw2"].numel() * 4
+        if evw is not None:
+            ex, ee, et = (pin(evw[k]) for k in ("x", "edges", "table"))
+            self.keep += [ex, ee, et]
+            d.evw_x, d.evw_edges, d.evw_nbins, d.evw_table = ex.data_ptr(), ee.data_ptr(), et.numel(), et.data_ptr()
+            self.h2d_bytes += ex.numel() * 4
         self.desc, self.V, self.W = d, V, W
         self.batch_events = int(batch_events)
         nbytes = lib().hepk_chain_host_workspace_bytes(C.byref(d), C.c_int64(self.batch_events))
@@ -548,7 +573,7 @@ class HostChainPlan:
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=device)
 
     def zero_hists(self):
-        for k in ("hist_sumw", "hist_counts"):
+        for k in ("hist_sumw", "hist_sumw2", "hist_counts"):
             if k in self.out:
                 self.out[k].zero_()
 

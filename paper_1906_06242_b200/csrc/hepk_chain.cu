@@ -69,14 +69,27 @@ struct ChainParams {
     int* out_njet; int* out_argmax;
     float *out_ht, *out_maxpt, *out_minpt, *out_mjj, *out_subpt;
     unsigned char* out_jet_mask;
-    double* hist_acc;                    // workspace: [V][active o][W][nbins_o+2] float64, or nullptr
-    unsigned long long* hist_counts;     // [V][active o][nbins_o+2], or nullptr
+    // Histograms.  Privatised bins (shared memory) and their global accumulators (workspace) share one INTERNAL
+    // layout: word (v, o, slot, col) at ((v * spv + obs_prefix[o] + slot) * WS + col), columns: W x sumw, then
+    // 2W x sumw2 (if asked for), then the event count (if asked for); WS >= the number of columns.  All columns of a
+    // slot are neighbours, so one event's updates of a slot are immediate offsets from one address.  sumw2 takes two
+    // columns per weight (value and rounding remainder, see add_weights).
+    int WS, ncol, col_w2, col_cnt;       // col_w2 / col_cnt: first sumw2 column / count column, -1 = absent
+    long long* hist_acc;                 // workspace: n_words accumulators (int64 fixed point, or float64 bits), or nullptr
+    unsigned int* hist_hdr;              // workspace header (HDR_* words), or nullptr
+    float *hist_sumw, *hist_sumw2;       // the caller's arrays (chain_finalize_hist)
+    long long* hist_counts;
+    const float *evw_x, *evw_edges, *evw_table;   // per-event weight factor from a lookup (evw_table nullptr: none)
+    int evw_nbins;
     int order_off, lep_off, corr_off, bucket_off;   // byte offsets inside a warp's region
     int region_bytes, shared_bytes;      // per-warp region; CTA-shared part in front of the regions
-    int flush_events;                    // a CTA flushes its histograms to the global accumulators every this many events
-    const unsigned int* wmax_bits;       // [0] bits of max |weight| over the launch, [1] != 0: a weight is not finite
-    unsigned int* tile_counter;          // zeroed per launch: tiles beyond the first one of each warp are handed out dynamically (nullptr: static)
+    unsigned int* tile_counter;          // zeroed per launch: the last eighth of the tiles is handed out through it (nullptr: static)
 };
+
+// Workspace header words (uint32), written by chain_weight_range_kernel, read by the chain kernel and the finalize step.
+enum { HDR_WMAX = 0, HDR_BAD = 1, HDR_TILE = 2, HDR_WMIN = 3, HDR_TMAX = 4, HDR_TMIN = 5, HDR_WORDS = 16 };
+constexpr int SCAN_SLICES = 32;          // the bins are checked for overflow in this many slices, one per finished tile
+constexpr int FLUSH_AT = 1 << 29;        // a fixed-point bin is moved to its global accumulator when |bin| reaches this
 
 namespace dev {
 
@@ -85,10 +98,10 @@ struct ChainShared {
     float *edges, *axis_lo, *axis_inv;   // axis_inv == 0: the axis is not uniform enough for the arithmetic bin guess
     float *cal_pt_edges, *cal_eta_edges, *cal_table;
     float* cal_axis;                     // per calibration axis (pt, eta): [mode (0 search, 1 linear, 2 log2), lo, inv, unused]
-    float* h_sumw;                       // int32 fixed point (w * 2^k) when wscale[0] != 0, else float
-    unsigned int* h_cnt;
-    float* wscale;                       // [0] 2^k or 0, [1] 2^-k
-    unsigned int* since;                 // events filled since the last flush
+    unsigned int* h_bins;                // internal layout; sumw / sumw2 columns: int32 fixed point when wscale[0] != 0, else float
+    float* wscale;                       // [0] 2^k (0: float bins), [1] 2^k2 for squared weights
+    float *evw_edges, *evw_table;
+    unsigned int* scan;                  // ticket of the overflow scan
     unsigned int* next;                  // tiles of the CTA's own range handed out so far
 };
 
@@ -108,10 +121,11 @@ __host__ __device__ inline size_t chain_shared_layout(const ChainParams& P, bool
     r = take(calib ? (size_t)P.cal_npt * P.cal_neta * 4 : 0, 4); if (s) s->cal_table = (float*)(base + r);
     r = take(calib ? 32 : 0, 16); if (s) s->cal_axis = (float*)(base + r);
     const size_t spv = (size_t)P.obs_prefix[HEPK_N_OBS];
-    r = take(P.hist_acc ? spv * P.V * P.W * 4 : 0, 4); if (s) s->h_sumw = (float*)(base + r);
-    r = take(P.hist_counts ? spv * P.V * 4 : 0, 4); if (s) s->h_cnt = (unsigned int*)(base + r);
+    r = take(P.evw_table ? (size_t)(P.evw_nbins + 1) * 4 : 0, 4); if (s) s->evw_edges = (float*)(base + r);
+    r = take(P.evw_table ? (size_t)P.evw_nbins * 4 : 0, 4); if (s) s->evw_table = (float*)(base + r);
+    r = take(P.hist_acc ? spv * P.V * P.WS * 4 : 0, 16); if (s) s->h_bins = (unsigned int*)(base + r);
     r = take(8, 4); if (s) s->wscale = (float*)(base + r);
-    r = take(4, 4); if (s) s->since = (unsigned int*)(base + r);
+    r = take(4, 4); if (s) s->scan = (unsigned int*)(base + r);
     r = take(4, 4); if (s) s->next = (unsigned int*)(base + r);
     return align_up(o, 128);
 }
@@ -331,7 +345,8 @@ __device__ __forceinline__ float pair_mass_lean(float pt1, float eta1, float phi
 // What the launch asked for, as one register of flags (tested with one instruction instead of a pointer compare).
 enum : unsigned {
     F_NJET = 1u << 0, F_ARGMAX = 1u << 1, F_HT = 1u << 2, F_MAXPT = 1u << 3, F_MINPT = 1u << 4, F_MJJ = 1u << 5,
-    F_SUBPT = 1u << 6, F_OBS0 = 1u << 8 /* .. << 13 */, F_COUNTS = 1u << 16, F_SUMW = 1u << 17, F_WEIGHTS = 1u << 18, F_MULTIW = 1u << 19 /* more than one weight column */
+    F_SUBPT = 1u << 6, F_OBS0 = 1u << 8 /* .. << 13 */, F_COUNTS = 1u << 16, F_SUMW = 1u << 17, F_WEIGHTS = 1u << 18, F_MULTIW = 1u << 19 /* more than one weight column */,
+    F_SUMW2 = 1u << 20, F_EVW = 1u << 21
 };
 __device__ __forceinline__ unsigned chain_features(const ChainParams& P)
 {
@@ -346,39 +361,77 @@ __device__ __forceinline__ unsigned chain_features(const ChainParams& P)
 #pragma unroll
     for (int ob = 0; ob < HEPK_N_OBS; ++ob)
         if (P.axis_edges[ob]) f |= F_OBS0 << ob;
-    if (P.hist_counts) f |= F_COUNTS;
-    if (P.hist_acc) f |= F_SUMW;
+    if (P.col_cnt >= 0) f |= F_COUNTS;
+    if (P.hist_acc && P.hist_sumw) f |= F_SUMW;
+    if (P.col_w2 >= 0) f |= F_SUMW2;
     if (P.weights) f |= F_WEIGHTS;
     if (P.W > 1) f |= F_MULTIW;
+    if (P.evw_table) f |= F_EVW;
     return f;
 }
 
 // Slot of one observable: bumps its count and returns the shared-memory address of its bin in weight column 0
 // (0 when the observable is not histogrammed).  sumw layout [v][o][w][nbins_o + 2].
+// Shared-memory address of the slot row (all columns of one slot) of observable OB for value x; 0: not histogrammed.
 template <int OB>
-__device__ __forceinline__ uint32_t obs_bin(const ChainParams& P, const ChainShared& S, unsigned feat, int v, float x)
+__device__ __forceinline__ uint32_t obs_row(const ChainParams& P, const ChainShared& S, unsigned feat, int v, float x)
 {
     if (!(feat & (F_OBS0 << OB))) return 0u;
     const int nb = P.axis_nbins[OB];
     const int slot = slot_lean(x, smem_u32(S.edges) + 4u * (unsigned)P.edge_prefix[OB], nb, lds_f32(smem_u32(S.axis_lo) + 4u * OB),
                                lds_f32(smem_u32(S.axis_inv) + 4u * OB));
-    const int spv = P.obs_prefix[HEPK_N_OBS], pre = P.obs_prefix[OB];
-    if (feat & F_COUNTS) red_add_shared_u32(smem_u32(S.h_cnt) + 4u * (unsigned)(v * spv + pre + slot), 1u);
-    return smem_u32(S.h_sumw) + 4u * (unsigned)((v * spv + pre) * P.W + slot);
+    return smem_u32(S.h_bins) + 4u * (unsigned)((v * P.obs_prefix[HEPK_N_OBS] + P.obs_prefix[OB] + slot) * P.WS);
 }
 
-// One weight into the bins of the active observables.  Fixed point (wscale != 0): the weight is rounded once to
-// a multiple of 2^-k and added with the native integer shared-memory atomic; else float (a compare-and-swap loop).
-__device__ __forceinline__ void add_weight(const ChainParams& P, unsigned feat, const uint32_t (&bin)[HEPK_N_OBS], int w,
-                                           float wt, float wscale)
+// One value into column `col` of the slot rows of the active observables.  Fixed point (FIXED): q is the weight
+// rounded once to a multiple of 2^-k, added with the native integer shared-memory atomic; else the float weight
+// (a compare-and-swap loop in hardware).
+template <bool FIXED>
+__device__ __forceinline__ void add_column(unsigned feat, const uint32_t (&row)[HEPK_N_OBS], int col, int q, float wt)
 {
-    const int q = __float2int_rn(wt * wscale);
 #pragma unroll
     for (int ob = 0; ob < HEPK_N_OBS; ++ob) {
         if (!(feat & (F_OBS0 << ob))) continue;
-        const uint32_t a = bin[ob] + 4u * (unsigned)(w * (P.axis_nbins[ob] + 2));
-        if (wscale != 0.0f) red_add_shared_s32(a, q);
+        const uint32_t a = row[ob] + 4u * (unsigned)col;
+        if (FIXED) red_add_shared_s32(a, q);
         else red_add_shared_f32(a, wt);
+    }
+}
+
+// All weight columns of one event into its slot rows.
+template <bool FIXED, int NW>
+__device__ __forceinline__ void add_weights(const ChainParams& P, unsigned feat, const uint32_t (&row)[HEPK_N_OBS],
+                                            const float (&wt)[NW], long long ev, float evf, float sc, float sc2)
+{
+    const bool w2 = (feat & F_SUMW2) != 0, w1 = (feat & F_SUMW) != 0;
+    auto one = [&](int w, float x) {
+        if (w1) add_column<FIXED>(feat, row, w, FIXED ? __float2int_rn(x * sc) : 0, x);
+        if (w2) {
+            // squared weights span the square of the weights' range: two fixed-point columns per weight, the second
+            // holding the rounding remainder of the first at 2^20 times its scale (both exact integers below 2^19)
+            const float x2 = x * x, y = x2 * sc2;
+            const int qh = FIXED ? __float2int_rn(y) : 0;
+            add_column<FIXED>(feat, row, P.col_w2 + 2 * w, qh, x2);
+            if (FIXED) add_column<true>(feat, row, P.col_w2 + 2 * w + 1, __float2int_rn((y - (float)qh) * 1048576.0f), 0.0f);
+        }
+    };
+    one(0, wt[0]);
+    if ((feat & (F_WEIGHTS | F_MULTIW)) != (F_WEIGHTS | F_MULTIW)) return;
+    if (NW > 1) {
+        // the event's weights were loaded once per tile and serve every variant and observable
+#pragma unroll
+        for (int w = 1; w < NW; ++w)
+            if (w < P.W) one(w, wt[w]);
+    } else {
+        // eight loads in flight, then their fills (one memory latency per eight columns, not per column)
+        for (int w0 = 1; w0 < P.W; w0 += 8) {
+            float x[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) x[k] = w0 + k < P.W ? __ldg(P.weights + (long long)(w0 + k) * P.n_events + ev) : 0.0f;
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                if (w0 + k < P.W) one(w0 + k, (feat & F_EVW) ? __fmul_rn(x[k], evf) : x[k]);
+        }
     }
 }
 
@@ -386,7 +439,7 @@ __device__ __forceinline__ void add_weight(const ChainParams& P, unsigned feat, 
 // path.  The leading jets' (eta, phi, mass) are passed in by value; i2 < 0 means fewer than two clean jets.
 template <int NW>
 __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainShared& S, unsigned feat, long long ev, int v,
-                                             const float (&wt)[NW],
+                                             const float (&wt)[NW], float evf,
                                              int cnt, float sum, float mn, float b1, float b2, int i1, int i2,
                                              float eta1, float phi1, float m1, float eta2, float phi2, float m2)
 {
@@ -416,25 +469,22 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     if (feat & F_MJJ) P.out_mjj[o] = mjj;
     if (feat & F_SUBPT) P.out_subpt[o] = subpt;
     if (!hists) return;
-    uint32_t bin[HEPK_N_OBS];
-    bin[HEPK_OBS_NJET] = obs_bin<HEPK_OBS_NJET>(P, S, feat, v, (float)cnt);
-    bin[HEPK_OBS_HT] = obs_bin<HEPK_OBS_HT>(P, S, feat, v, sum);
-    bin[HEPK_OBS_MAXPT] = obs_bin<HEPK_OBS_MAXPT>(P, S, feat, v, b1);
-    bin[HEPK_OBS_MINPT] = obs_bin<HEPK_OBS_MINPT>(P, S, feat, v, mn);
-    bin[HEPK_OBS_MJJ] = obs_bin<HEPK_OBS_MJJ>(P, S, feat, v, mjj);
-    bin[HEPK_OBS_SUBPT] = obs_bin<HEPK_OBS_SUBPT>(P, S, feat, v, subpt);
-    if (!(feat & F_SUMW)) return;
-    const float wscale = lds_f32(smem_u32(S.wscale));
-    add_weight(P, feat, bin, 0, wt[0], wscale);
-    if ((feat & (F_WEIGHTS | F_MULTIW)) != (F_WEIGHTS | F_MULTIW)) return;
-    if (NW > 1) {
-        // the event's weights were loaded once per tile and serve every variant and observable
+    uint32_t row[HEPK_N_OBS];
+    row[HEPK_OBS_NJET] = obs_row<HEPK_OBS_NJET>(P, S, feat, v, (float)cnt);
+    row[HEPK_OBS_HT] = obs_row<HEPK_OBS_HT>(P, S, feat, v, sum);
+    row[HEPK_OBS_MAXPT] = obs_row<HEPK_OBS_MAXPT>(P, S, feat, v, b1);
+    row[HEPK_OBS_MINPT] = obs_row<HEPK_OBS_MINPT>(P, S, feat, v, mn);
+    row[HEPK_OBS_MJJ] = obs_row<HEPK_OBS_MJJ>(P, S, feat, v, mjj);
+    row[HEPK_OBS_SUBPT] = obs_row<HEPK_OBS_SUBPT>(P, S, feat, v, subpt);
+    if (feat & F_COUNTS) {
 #pragma unroll
-        for (int w = 1; w < NW; ++w)
-            if (w < P.W) add_weight(P, feat, bin, w, wt[w], wscale);
-    } else {
-        for (int w = 1; w < P.W; ++w) add_weight(P, feat, bin, w, __ldg(P.weights + (long long)w * P.n_events + ev), wscale);
+        for (int ob = 0; ob < HEPK_N_OBS; ++ob)
+            if (feat & (F_OBS0 << ob)) red_add_shared_u32(row[ob] + 4u * (unsigned)P.col_cnt, 1u);
     }
+    if (!(feat & (F_SUMW | F_SUMW2))) return;
+    const float2 sc = lds_v2(smem_u32(S.wscale));
+    if (sc.x != 0.0f) add_weights<true, NW>(P, feat, row, wt, ev, evf, sc.x, sc.y);
+    else add_weights<false, NW>(P, feat, row, wt, ev, evf, 0.0f, 0.0f);
 }
 
 // Order-preserving map float -> unsigned (and back): a < b  <=>  ord_key(a) < ord_key(b); no finite value maps to 0.
@@ -529,6 +579,50 @@ struct EventAcc {
     }
 };
 
+// Fixed-point scales of the weighted bins (R18) from the weight range in the workspace header: entries are
+// rint(w * 2^k) with |w| * 2^k < 2^19 (2^k2 likewise for w^2).  A bin is checked at least every ~1024 events of the
+// CTA plus the tiles in flight and moved out at 2^29, so it stays below 2^31.  The rounding error per entry is
+// <= 2^-20 max|w|, so the scheme is taken only when the weights span at most a factor 8 (error <= 7.7e-6 of the
+// smallest entry); otherwise sc = sc2 = 0: float bins.
+__device__ __forceinline__ void hist_scales(const ChainParams& P, float& sc, float& sc2)
+{
+    sc = sc2 = 0.0f;
+    if (!P.hist_hdr || P.hist_hdr[HDR_BAD] != 0u) return;
+    const float tmax = P.evw_table ? __uint_as_float(P.hist_hdr[HDR_TMAX]) : 1.0f;
+    const float tmin = P.evw_table ? __uint_as_float(P.hist_hdr[HDR_TMIN]) : 1.0f;
+    const float wm = __uint_as_float(P.hist_hdr[HDR_WMAX]) * tmax;
+    const float wn = __uint_as_float(P.hist_hdr[HDR_WMIN]) * tmin;
+    if (!(wm > 0.0f && wm < CUDART_INF_F && wn > 0.0f && wm <= 8.0f * wn)) return;
+    if (!(wm * wm < CUDART_INF_F && wn * wn > 0.0f)) return;
+    int e, e2;
+    frexpf(wm, &e);                                    // wm < 2^e
+    frexpf(wm * wm, &e2);
+    const int k = 19 - e, k2 = 19 - e2;
+    if (k <= -100 || k >= 100 || k2 <= -100 || k2 >= 100) return;
+    sc = ldexpf(1.0f, k);
+    sc2 = ldexpf(1.0f, k2);
+}
+
+// Per-event weight factor table[B(x)] (hepk_lookup_binned's clamped bin, 1-D) from the staged lookup.
+__device__ __forceinline__ float evw_factor(const ChainParams& P, const ChainShared& S, long long ev)
+{
+    const float x = __ldg(P.evw_x + ev);
+    const int n = P.evw_nbins;
+    const uint32_t ed = smem_u32(S.evw_edges);
+    int b;
+    if (x < lds_f32(ed)) b = 0;
+    else if (!(x < lds_f32(ed + 4u * (unsigned)n))) b = n - 1;
+    else {
+        int lo = 0, hi = n;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (x >= lds_f32(ed + 4u * (unsigned)mid)) lo = mid; else hi = mid;
+        }
+        b = lo;
+    }
+    return lds_f32(smem_u32(S.evw_table) + 4u * (unsigned)b);
+}
+
 // dR match of one jet against one lepton collection of event `ev`, straight from global memory.
 __device__ inline bool match_global(const ChainParams& P, float eta, float phi, const long long* off, long long base,
                                     const float* lpt, const float* leta, const float* lphi, long long ev)
@@ -576,38 +670,33 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, unsigned c
             e1 = P.jeta[x]; p1 = P.jphi[x]; m1 = P.jmass[x];
             e2 = P.jeta[y]; p2 = P.jphi[y]; m2 = P.jmass[y];
         }
-        const float wt[1] = {P.weights ? __ldg(P.weights + ev) : 1.0f};
-        finish_event<1>(P, S, chain_features(P), ev, v, wt, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
+        const float evf = P.evw_table ? evw_factor(P, S, ev) : 1.0f;
+        const float w0 = P.weights ? __ldg(P.weights + ev) : 1.0f;
+        const float wt[1] = {P.evw_table ? __fmul_rn(w0, evf) : w0};
+        finish_event<1>(P, S, chain_features(P), ev, v, wt, evf, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
     }
 }
 
-// Move the privatised histograms of the CTA into the global accumulators.  Safe against concurrent fills by
-// other warps: every bin is taken with an atomic exchange.
-__device__ __forceinline__ void flush_hist(const ChainParams& P, const ChainShared& S, int t, int nt)
+// Move privatised bins [i0, i1) of the CTA into the global accumulators (thread t of nt).  Safe against concurrent
+// fills by other warps: a bin is taken with an atomic exchange.  Fixed-point and count columns are exact integers,
+// so they only move when `all` is set or the bin is about to leave the int32 range (|bin| >= FLUSH_AT); float bins
+// move whenever they are non-zero (their rounding error grows with their content).
+__device__ __forceinline__ void flush_bins(const ChainParams& P, const ChainShared& S, int i0, int i1, int t, int nt, bool all)
 {
-    const int spv = P.obs_prefix[HEPK_N_OBS];
-    if (P.hist_acc) {
-        const int n = spv * P.V * P.W;
-        const bool fixed = S.wscale[0] != 0.0f;
-        const double inv = (double)S.wscale[1];
-        int* hi = (int*)S.h_sumw;
-        for (int i = t; i < n; i += nt) {
-            if (hi[i] == 0) continue;          // +0.0f and integer 0 share the bit pattern
-            if (fixed) {
-                const int x = atomicExch(hi + i, 0);
-                if (x) atomicAdd(P.hist_acc + i, (double)x * inv);
-            } else {
-                const float x = atomicExch(S.h_sumw + i, 0.0f);
-                if (x != 0.0f) atomicAdd(P.hist_acc + i, (double)x);
-            }
-        }
-    }
-    if (P.hist_counts) {
-        const int n = spv * P.V;
-        for (int i = t; i < n; i += nt) {
-            if (S.h_cnt[i] == 0u) continue;
-            const unsigned int c = atomicExch(S.h_cnt + i, 0u);
-            if (c) atomicAdd(P.hist_counts + i, (unsigned long long)c);
+    const bool fixed = S.wscale[0] != 0.0f;
+    int* bins = (int*)S.h_bins;
+    const int WS = P.WS, ccol = P.col_cnt;
+    for (int i = i0 + t; i < i1; i += nt) {
+        const int x = bins[i];
+        if (x == 0) continue;                         // +0.0f and integer 0 share the bit pattern
+        const bool is_int = fixed || (i % WS) == ccol;
+        if (is_int) {
+            if (!all && (unsigned)(x + FLUSH_AT) < 2u * (unsigned)FLUSH_AT) continue;      // |x| < FLUSH_AT
+            const int y = atomicExch(bins + i, 0);
+            if (y) atomicAdd((unsigned long long*)P.hist_acc + i, (unsigned long long)(long long)y);
+        } else {
+            const float y = atomicExch((float*)bins + i, 0.0f);
+            if (y != 0.0f) atomicAdd((double*)P.hist_acc + i, (double)y);
         }
     }
 }
@@ -705,22 +794,16 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     }
     {
         const int spv = P.obs_prefix[HEPK_N_OBS];
-        if (P.hist_acc) for (int i = tid; i < spv * P.V * P.W; i += nthr) S.h_sumw[i] = 0.0f;
-        if (P.hist_counts) for (int i = tid; i < spv * P.V; i += nthr) S.h_cnt[i] = 0u;
+        if (P.hist_acc) for (int i = tid; i < spv * P.V * P.WS; i += nthr) S.h_bins[i] = 0u;
+        if (P.evw_table) {
+            for (int i = tid; i <= P.evw_nbins; i += nthr) S.evw_edges[i] = P.evw_edges[i];
+            for (int i = tid; i < P.evw_nbins; i += nthr) S.evw_table[i] = P.evw_table[i];
+        }
         if (tid == 0) {
-            // fixed-point scale of the weighted bins: 4 * flush_events entries of max |w| * 2^k stay below 2^31
-            float sc = 0.0f, inv = 0.0f;
-            if (P.wmax_bits && P.wmax_bits[1] == 0u) {
-                const float wm = __uint_as_float(P.wmax_bits[0]);
-                if (wm > 0.0f && wm < CUDART_INF_F) {
-                    int e;
-                    frexpf(wm, &e);                                    // wm < 2^e
-                    const int k = 29 - (31 - __clz(P.flush_events)) - e;   // flush_events is a power of two
-                    if (k > -100 && k < 100) { sc = ldexpf(1.0f, k); inv = ldexpf(1.0f, -k); }
-                }
-            }
-            S.wscale[0] = sc; S.wscale[1] = inv;
-            *S.since = 0u;
+            float sc, sc2;
+            hist_scales(P, sc, sc2);
+            S.wscale[0] = sc; S.wscale[1] = sc2;
+            *S.scan = 0u;
             *S.next = 0u;
         }
     }
@@ -824,11 +907,14 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         const int ne = rest < TILE_EVENTS ? (int)rest : TILE_EVENTS;
         const bool has_next = tile_next < P.n_tiles;
         float wt[NW];                                                    // weights of the lane's event, loaded early
+        float evf = 1.0f;                                                // its weight factor from the lookup
+        if ((feat & F_EVW) && (feat & (F_SUMW | F_SUMW2)) && lane < ne) evf = evw_factor(P, S, e0 + lane);
 #pragma unroll
         for (int w = 0; w < NW; ++w) {
             wt[w] = 1.0f;
-            if ((feat & (F_SUMW | F_WEIGHTS)) == (F_SUMW | F_WEIGHTS) && lane < ne && w < P.W)
+            if ((feat & F_WEIGHTS) && (feat & (F_SUMW | F_SUMW2)) && lane < ne && w < P.W)
                 wt[w] = __ldg(P.weights + (long long)w * P.n_events + e0 + lane);
+            if (feat & F_EVW) wt[w] = __fmul_rn(wt[w], evf);             // one float32 multiply (exact class)
         }
         EventOffsets neo;
         neo.j0 = neo.j1 = neo.m0 = neo.m1 = neo.q0 = neo.q1 = 0;
@@ -1060,7 +1146,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         released = true;
                     }
                     if (live)
-                        finish_event<NW>(P, S, feat, e0 + lane, v, wt, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
+                        finish_event<NW>(P, S, feat, e0 + lane, v, wt, evf, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
                 }
             }
             bsel ^= 1;
@@ -1080,42 +1166,85 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         tile = tile_next;
         tile_next = take_tile();
 
-        {   // the warp whose tile takes the CTA's event count across a multiple of flush_events flushes the histograms
-            unsigned int c = 0;
-            if (lane == 0) c = atom_add_shared_u32(smem_u32(S.since), (unsigned)ne);
-            c = __shfl_sync(0xffffffffu, c, 0);
-            if ((c & ~(unsigned)(P.flush_events - 1)) != ((c + (unsigned)ne) & ~(unsigned)(P.flush_events - 1))) flush_hist(P, S, lane, 32);
+        if (P.hist_acc) {
+            // every finished tile checks one slice of the CTA's bins for values about to leave the int32 range
+            unsigned int t = 0;
+            if (lane == 0) t = atom_add_shared_u32(smem_u32(S.scan), 1u);
+            t = __shfl_sync(0xffffffffu, t, 0) % SCAN_SLICES;
+            const int n = P.obs_prefix[HEPK_N_OBS] * P.V * P.WS;
+            const int len = (n + SCAN_SLICES - 1) / SCAN_SLICES;
+            const int i0 = (int)t * len;
+            flush_bins(P, S, i0, i0 + len < n ? i0 + len : n, lane, 32, false);
         }
     }
     __syncthreads();
-    flush_hist(P, S, tid, nthr);
+    if (P.hist_acc) flush_bins(P, S, 0, P.obs_prefix[HEPK_N_OBS] * P.V * P.WS, tid, nthr, true);
 }
 
-// max |w| over the launch's weights (bits of a non-negative float order like unsigned integers) and a flag for
-// non-finite weights; out[0..1] zeroed by the caller.  w == nullptr: every weight is 1.
-__global__ void chain_wmax_kernel(const float* __restrict__ w, long long n, unsigned int* __restrict__ out)
+// Range of the launch's weights: max |w|, min non-zero |w| (bits of a non-negative float order like unsigned
+// integers) and a flag for non-finite values, into the workspace header; the same for the event-weight table.
+// hdr[HDR_WMAX] = hdr[HDR_TMAX] = 0, hdr[HDR_WMIN] = hdr[HDR_TMIN] = +inf bits, hdr[HDR_BAD] = 0 set by the caller.
+// w == nullptr: every weight is 1.
+__global__ void chain_weight_range_kernel(const float* __restrict__ w, long long n, const float* __restrict__ table, int nt,
+                                          unsigned int* __restrict__ hdr)
 {
-    if (!w) {
-        if (blockIdx.x == 0 && threadIdx.x == 0) out[0] = __float_as_uint(1.0f);
+    auto fold = [&](const float* p, long long cnt, int imax, int imin) {
+        float m = 0.0f, mn = CUDART_INF_F;
+        bool bad = false;
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += (long long)gridDim.x * blockDim.x) {
+            const float a = fabsf(p[i]);
+            bad = bad || !(a < CUDART_INF_F);
+            m = fmaxf(m, a);
+            if (a > 0.0f) mn = fminf(mn, a);
+        }
+        const unsigned int b = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
+        const unsigned int c = __reduce_min_sync(0xffffffffu, __float_as_uint(mn));
+        if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(hdr + HDR_BAD, 1u);
+        if ((threadIdx.x & 31) == 0) {
+            if (b) atomicMax(hdr + imax, b);
+            atomicMin(hdr + imin, c);
+        }
+    };
+    if (w) fold(w, n, HDR_WMAX, HDR_WMIN);
+    else if (blockIdx.x == 0 && threadIdx.x == 0) hdr[HDR_WMAX] = hdr[HDR_WMIN] = __float_as_uint(1.0f);
+    if (table) fold(table, nt, HDR_TMAX, HDR_TMIN);
+}
+
+// The caller's arrays from the accumulators: word (v, o, slot, col) of the internal layout goes to
+// sumw / sumw2 [v][o][w][slot] (float32(float64(old) + sum)) or counts [v][o][slot] (+=).
+__global__ void chain_finalize_hist(const __grid_constant__ ChainParams P)
+{
+    float sc, sc2;
+    hist_scales(P, sc, sc2);
+    const int spv = P.obs_prefix[HEPK_N_OBS];
+    const long long n = (long long)spv * P.V * P.WS;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int col = (int)(i % P.WS);
+    const long long r = i / P.WS;                   // (v, o, slot) as v * spv + prefix[o] + slot
+    const int v = (int)(r / spv), q = (int)(r % spv);
+    int o = 0;
+#pragma unroll
+    for (int k = 1; k < HEPK_N_OBS; ++k)
+        if (P.axis_edges[k] && q >= P.obs_prefix[k]) o = k;
+    while (!P.axis_edges[o]) ++o;                   // the first active observable has prefix 0
+    const int slot = q - P.obs_prefix[o], nb2 = P.axis_nbins[o] + 2;
+    if (col == P.col_cnt) {
+        P.hist_counts[r] += P.hist_acc[i];
         return;
     }
-    float m = 0.0f;
-    bool bad = false;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const float a = fabsf(w[i]);
-        bad = bad || !(a < CUDART_INF_F);
-        m = fmaxf(m, a);
-    }
-    const unsigned int b = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
-    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(out + 1, 1u);
-    if ((threadIdx.x & 31) == 0 && b) atomicMax(out, b);
-}
-
-// sumw[i] = float32(float64(sumw[i]) + acc[i])
-__global__ void chain_finalize_hist(float* __restrict__ sumw, const double* __restrict__ acc, int n)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) sumw[i] = (float)((double)sumw[i] + acc[i]);
+    if (col >= P.ncol) return;                      // padding column
+    const bool sq = P.col_w2 >= 0 && col >= P.col_w2;
+    if (sq && ((col - P.col_w2) & 1)) return;       // remainder column: handled with its value column
+    if (!sq && !P.hist_sumw) return;                // sumw columns exist but only sumw2 was asked for
+    const int w = sq ? (col - P.col_w2) >> 1 : col;
+    float* dst = (sq ? P.hist_sumw2 : P.hist_sumw) + ((long long)v * spv + P.obs_prefix[o]) * P.W + (long long)w * nb2 + slot;
+    const float s = sq ? sc2 : sc;
+    double add;
+    if (s == 0.0f) add = __longlong_as_double(P.hist_acc[i]);
+    else if (sq) add = ((double)P.hist_acc[i] + (double)P.hist_acc[i + 1] * (1.0 / 1048576.0)) / (double)s;
+    else add = (double)P.hist_acc[i] / (double)s;
+    *dst = (float)((double)*dst + add);
 }
 
 }  // namespace dev
@@ -1143,6 +1272,10 @@ static int32_t chain_validate(const hepk_chain_desc* d)
     }
     for (int o = 0; o < HEPK_N_OBS; ++o)
         if (d->axis_edges[o]) HEPK_REQUIRE(d->axis_nbins[o] >= 1, "histogram axis has no bins");
+    if (d->evw_table) {
+        HEPK_REQUIRE(d->evw_x && d->evw_edges, "event-weight lookup: x or edges is NULL");
+        HEPK_REQUIRE(d->evw_nbins >= 1 && d->evw_nbins <= 4096, "event-weight lookup: 1..4096 bins");
+    }
     return HEPK_OK;
 }
 
@@ -1155,6 +1288,29 @@ static long long hist_slots_per_variant(const hepk_chain_desc* d)
 }
 
 static int round_up4(long long x) { return (int)((x + 3) / 4 * 4); }
+
+static const unsigned int g_inf_bits = 0x7f800000u;      // +inf: start value of the "minimum |w|" header words
+
+// Internal histogram layout (ChainParams): columns of a slot row and the padded row length.
+struct HistLayout { int ncol, ws, col_w2, col_cnt; long long n_words; };
+static HistLayout hist_layout(const hepk_chain_desc* d)
+{
+    HistLayout h;
+    const long long sp = hist_slots_per_variant(d);
+    const int W = d->n_wvar;
+    const bool w1 = d->hist_sumw != nullptr, w2 = d->hist_sumw2 != nullptr, cn = d->hist_counts != nullptr;
+    h.ncol = 0; h.col_w2 = -1; h.col_cnt = -1;
+    if (sp > 0 && (w1 || w2 || cn)) {
+        h.ncol = (w1 || w2) ? W : 0;         // sumw columns are kept (unused) when only sumw2 is asked for
+        if (w2) { h.col_w2 = h.ncol; h.ncol += 2 * W; }        // value and rounding-remainder column per weight
+        if (cn) { h.col_cnt = h.ncol; h.ncol += 1; }
+    }
+    // an odd row length spreads the rows of a column over all shared-memory banks; pad when it costs little
+    h.ws = h.ncol;
+    if (h.ncol > 0 && (h.ncol & 1) == 0 && sp * d->n_variants * (h.ncol + 1) * 4 <= 32 * 1024) h.ws = h.ncol + 1;
+    h.n_words = sp * d->n_variants * h.ws;
+    return h;
+}
 
 // Fill the staged-column table and the per-warp region layout for the given capacities; returns the region size.
 static int chain_region_layout(ChainParams& P, const hepk_chain_desc* d, bool calib, int cap_j, int cap_m, int cap_e)
@@ -1189,8 +1345,10 @@ static int chain_region_layout(ChainParams& P, const hepk_chain_desc* d, bool ca
     return (int)dev::align_up(o, 128);
 }
 
-static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStream_t st)
+// plan_warps != nullptr: only work out the CTA shape (warps per SM; 0 = does not fit) and return.
+static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStream_t st, int* plan_warps)
 {
+    if (plan_warps) *plan_warps = 0;
     ChainParams P;
     memset(&P, 0, sizeof(P));
     P.n_events = d->n_events;
@@ -1221,10 +1379,16 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     P.obs_prefix[HEPK_N_OBS] = sp; P.edge_prefix[HEPK_N_OBS] = ep;
     P.out_njet = d->out_njet; P.out_argmax = d->out_argmax; P.out_ht = d->out_ht; P.out_maxpt = d->out_maxpt;
     P.out_minpt = d->out_minpt; P.out_mjj = d->out_mjj; P.out_subpt = d->out_subpt; P.out_jet_mask = d->out_jet_mask;
-    const long long n_sumw = (long long)sp * P.V * P.W;
-    const bool want_sumw = d->hist_sumw && sp > 0, want_cnt = d->hist_counts && sp > 0;
-    P.hist_acc = want_sumw ? (double*)workspace : nullptr;
-    P.hist_counts = want_cnt ? (unsigned long long*)d->hist_counts : nullptr;
+    const HistLayout hl = hist_layout(d);
+    const bool want_hist = hl.ncol > 0;
+    P.WS = hl.ws; P.ncol = hl.ncol; P.col_w2 = hl.col_w2; P.col_cnt = hl.col_cnt;
+    const long long n_words = hl.n_words;
+    P.hist_hdr = want_hist ? (unsigned int*)workspace : nullptr;
+    P.hist_acc = want_hist ? (long long*)((char*)workspace + HDR_WORDS * 4) : nullptr;
+    P.hist_sumw = want_hist ? d->hist_sumw : nullptr;
+    P.hist_sumw2 = want_hist ? d->hist_sumw2 : nullptr;
+    P.hist_counts = want_hist ? (long long*)d->hist_counts : nullptr;
+    P.evw_x = d->evw_x; P.evw_edges = d->evw_edges; P.evw_table = d->evw_table; P.evw_nbins = d->evw_nbins;
 
     // staging capacities per 32-event tile from the mean multiplicities: mean + ~4 sigma of a Poisson-like
     // tile total (a tile that does not fit takes the per-event path)
@@ -1248,6 +1412,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     const int smem_max = max_smem_optin();
     const int shared_bytes = (int)dev::chain_shared_layout(P, calib, nullptr, nullptr);
     if (shared_bytes + 1024 > smem_max) {
+        if (plan_warps) return HEPK_OK;
         set_error("hepk_analysis_chain: histograms need %d bytes of shared memory (max %d)", shared_bytes, smem_max);
         return HEPK_ERR_UNSUPPORTED;
     }
@@ -1262,6 +1427,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         region = chain_region_layout(P, d, calib, cap_j, cap_m, cap_e);
     }
     if (shared_bytes + region > smem_max) {
+        if (plan_warps) return HEPK_OK;
         set_error("hepk_analysis_chain: %d + %d bytes of shared memory needed (max %d)", shared_bytes, region, smem_max);
         return HEPK_ERR_UNSUPPORTED;
     }
@@ -1292,10 +1458,12 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         if (wpc * ctas > best_total) { best_total = wpc * ctas; best_ctas = ctas; best_wpc = wpc; }
     }
     const int wpc = best_wpc;
+    if (plan_warps) {
+        *plan_warps = best_total;
+        return HEPK_OK;
+    }
     const size_t smem = (size_t)shared_bytes + (size_t)wpc * region;
-    P.flush_events = 1024;
-    P.wmax_bits = want_sumw ? (const unsigned int*)((const double*)workspace + n_sumw) : nullptr;
-    P.tile_counter = want_sumw ? (unsigned int*)((double*)workspace + n_sumw) + 2 : nullptr;
+    P.tile_counter = want_hist ? P.hist_hdr + HDR_TILE : nullptr;
 
     // two register budgets: up to 20 warps per CTA (96 registers per thread, no spills) or up to 24 (80)
     void (*kern)(ChainParams);
@@ -1317,17 +1485,19 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (d->out_subpt) feat_host |= dev::F_SUBPT;
     for (int o = 0; o < HEPK_N_OBS; ++o)
         if (d->axis_edges[o]) feat_host |= dev::F_OBS0 << o;
-    if (P.hist_counts) feat_host |= dev::F_COUNTS;
-    if (P.hist_acc) feat_host |= dev::F_SUMW;
+    if (P.col_cnt >= 0) feat_host |= dev::F_COUNTS;
+    if (P.hist_acc && P.hist_sumw) feat_host |= dev::F_SUMW;
+    if (P.col_w2 >= 0) feat_host |= dev::F_SUMW2;
+    if (P.evw_table) feat_host |= dev::F_EVW;
     if (d->weights) feat_host |= dev::F_WEIGHTS;
     if (P.W > 1) feat_host |= dev::F_MULTIW;
     const bool common = (int)feat_host == FEAT_COMMON && !d->out_jet_mask && has_el;
 #define HEPK_PICK_COMMON(MAXT) (calib ? dev::chain_kernel<true, true, MAXT, FEAT_COMMON> : dev::chain_kernel<false, true, MAXT, FEAT_COMMON>)
     // several weight columns and few warps (large histograms): a build that keeps the event's weights in registers
-    const bool multiw = P.W > 1 && d->weights && wpc <= 12;
+    const bool multiw = P.W > 1 && d->weights && wpc <= 16;
     if (multiw)
-        kern = calib ? (has_el ? dev::chain_kernel<true, true, 384, -1, HEPK_MAX_WVAR> : dev::chain_kernel<true, false, 384, -1, HEPK_MAX_WVAR>)
-                     : (has_el ? dev::chain_kernel<false, true, 384, -1, HEPK_MAX_WVAR> : dev::chain_kernel<false, false, 384, -1, HEPK_MAX_WVAR>);
+        kern = calib ? (has_el ? dev::chain_kernel<true, true, 512, -1, HEPK_MAX_WVAR> : dev::chain_kernel<true, false, 512, -1, HEPK_MAX_WVAR>)
+                     : (has_el ? dev::chain_kernel<false, true, 512, -1, HEPK_MAX_WVAR> : dev::chain_kernel<false, false, 512, -1, HEPK_MAX_WVAR>);
     else if (wpc <= 20) kern = common ? HEPK_PICK_COMMON(640) : HEPK_PICK(640, -1);
     else kern = common ? HEPK_PICK_COMMON(768) : HEPK_PICK(768, -1);
 #undef HEPK_PICK_COMMON
@@ -1342,21 +1512,23 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (grid > need) grid = need;
     if (grid < 1) grid = 1;
 
-    if (want_sumw) {
-        HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)n_sumw * sizeof(double) + 16, st));
+    if (want_hist) {
+        HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, HDR_WORDS * 4 + (size_t)n_words * 8, st));
+        HEPK_CUDA_TRY(cudaMemcpyAsync((unsigned int*)workspace + HDR_WMIN, &g_inf_bits, 4, cudaMemcpyHostToDevice, st));
+        HEPK_CUDA_TRY(cudaMemcpyAsync((unsigned int*)workspace + HDR_TMIN, &g_inf_bits, 4, cudaMemcpyHostToDevice, st));
         const long long nw = (long long)P.W * P.n_events;
         long long blocks = (nw + 256 * 8 - 1) / (256 * 8);
         if (blocks > 4 * sm_count()) blocks = 4 * sm_count();
         if (blocks < 1) blocks = 1;
-        dev::chain_wmax_kernel<<<(unsigned)blocks, 256, 0, st>>>(d->weights, nw, (unsigned int*)((double*)workspace + n_sumw));
+        dev::chain_weight_range_kernel<<<(unsigned)blocks, 256, 0, st>>>(d->weights, nw, d->evw_table, d->evw_nbins, P.hist_hdr);
         HEPK_CUDA_TRY(cudaGetLastError());
     }
     profile_mark(st, 0);
     kern<<<(unsigned)grid, wpc * 32, smem, st>>>(P);
     profile_mark(st, 1);
     HEPK_CUDA_TRY(cudaGetLastError());
-    if (want_sumw) {
-        dev::chain_finalize_hist<<<(unsigned)((n_sumw + 255) / 256), 256, 0, st>>>(d->hist_sumw, (const double*)workspace, (int)n_sumw);
+    if (want_hist) {
+        dev::chain_finalize_hist<<<(unsigned)((n_words + 255) / 256), 256, 0, st>>>(P);
         HEPK_CUDA_TRY(cudaGetLastError());
     }
     return HEPK_OK;
@@ -1367,8 +1539,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
 extern "C" size_t hepk_chain_workspace_bytes(const hepk_chain_desc* d)
 {
     if (!d || d->n_variants < 1 || d->n_wvar < 1) return 0;
-    const long long n = hepk::hist_slots_per_variant(d) * d->n_variants * d->n_wvar;
-    return (size_t)(n > 0 ? n : 1) * sizeof(double) + 16;      // float64 accumulators + max |weight| slot
+    return hepk::HDR_WORDS * 4 + (size_t)hepk::hist_layout(d).n_words * 8 + 8;      // header + 64-bit accumulators
 }
 
 extern "C" int32_t hepk_analysis_chain(const hepk_chain_desc* d, void* workspace, size_t workspace_bytes, void* stream)
@@ -1377,9 +1548,49 @@ extern "C" int32_t hepk_analysis_chain(const hepk_chain_desc* d, void* workspace
     const int32_t rc = chain_validate(d);
     if (rc != HEPK_OK) return rc;
     if (d->n_events == 0) return HEPK_OK;
-    if (d->hist_sumw && hist_slots_per_variant(d) > 0) {
+    if (hist_layout(d).ncol > 0) {
         HEPK_REQUIRE(workspace != nullptr, "workspace is NULL");
         HEPK_REQUIRE(workspace_bytes >= hepk_chain_workspace_bytes(d), "workspace too small");
     }
-    return chain_launch(d, workspace, (cudaStream_t)stream);
+    // Variants are independent given the variant-independent first half of the chain, and the privatised histograms
+    // of all variants share the SM's shared memory with the warps' staging regions.  When they leave room for fewer
+    // than 12 warps (large histogram sets), or do not fit at all, the variants are run in groups, one launch per
+    // group: the first half is recomputed per group, which costs less than running at a fraction of the occupancy.
+    const int V = d->n_variants;
+    int group = V;
+    if (d->tune_variants_per_pass > 0) group = d->tune_variants_per_pass < V ? d->tune_variants_per_pass : V;
+    else if (V > 1 && hist_layout(d).ncol > 0) {
+        int best_g = 0, best_w = 0;
+        for (int g = V; g >= 1; --g) {
+            hepk_chain_desc t = *d;
+            t.n_variants = g;
+            int w = 0;
+            if (chain_launch(&t, workspace, nullptr, &w) != HEPK_OK) w = 0;
+            if (w >= 12) { best_g = g; best_w = w; break; }
+            if (w > best_w) { best_g = g; best_w = w; }
+        }
+        if (best_g == 0) best_g = V;         // nothing fits: let the launch report the error
+        group = best_g;
+    }
+    if (group >= V) return chain_launch(d, workspace, (cudaStream_t)stream, nullptr);
+    const long long spv = hist_slots_per_variant(d), N = d->n_events, W = d->n_wvar;
+    for (int v0 = 0; v0 < V; v0 += group) {
+        hepk_chain_desc t = *d;
+        t.n_variants = v0 + group <= V ? group : V - v0;
+        for (int v = 0; v < t.n_variants; ++v) t.calib_scales[v] = d->calib_scales[v0 + v];
+        if (t.out_njet) t.out_njet += v0 * N;
+        if (t.out_argmax) t.out_argmax += v0 * N;
+        if (t.out_ht) t.out_ht += v0 * N;
+        if (t.out_maxpt) t.out_maxpt += v0 * N;
+        if (t.out_minpt) t.out_minpt += v0 * N;
+        if (t.out_mjj) t.out_mjj += v0 * N;
+        if (t.out_subpt) t.out_subpt += v0 * N;
+        if (t.out_jet_mask) t.out_jet_mask += v0 * d->jets.n_objects;
+        if (t.hist_sumw) t.hist_sumw += v0 * spv * W;
+        if (t.hist_sumw2) t.hist_sumw2 += v0 * spv * W;
+        if (t.hist_counts) t.hist_counts += v0 * spv;
+        const int32_t r = chain_launch(&t, workspace, (cudaStream_t)stream, nullptr);
+        if (r != HEPK_OK) return r;
+    }
+    return HEPK_OK;
 }

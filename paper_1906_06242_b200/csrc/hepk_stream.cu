@@ -14,17 +14,18 @@ namespace hepk {
 struct SlotLayout {
     size_t joff, moff, eoff;
     size_t jcol[4], mcol[3], ecol[3];
-    size_t weights;
+    size_t weights, evw_x;
     size_t out_i[2], out_f[5], out_mask;
-    size_t hist_sumw, hist_counts, chain_ws;
+    size_t hist_sumw, hist_sumw2, hist_counts, chain_ws;
     size_t bytes;
 };
 
 struct HostPlan {
     long long B, n_batches, maxJ, maxM, maxE;
-    long long spv, n_sumw, n_cnt;
-    size_t shared_bytes;          // calib + axis edges
-    size_t cal_pt, cal_eta, cal_tab, axis[HEPK_N_OBS];
+    long long spv, n_sumw, n_sumw2, n_cnt;
+    size_t chain_ws_bytes;
+    size_t shared_bytes;          // calib + axis edges + event-weight lookup
+    size_t cal_pt, cal_eta, cal_tab, axis[HEPK_N_OBS], evw_edges, evw_table;
     SlotLayout slot;
 };
 
@@ -53,7 +54,9 @@ static bool make_plan(const hepk_chain_desc* d, long long B, HostPlan* p)
         if (d->axis_edges[o]) spv += d->axis_nbins[o] + 2;
     p->spv = spv;
     p->n_sumw = d->hist_sumw ? spv * d->n_variants * d->n_wvar : 0;
+    p->n_sumw2 = d->hist_sumw2 ? spv * d->n_variants * d->n_wvar : 0;
     p->n_cnt = d->hist_counts ? spv * d->n_variants : 0;
+    p->chain_ws_bytes = hepk_chain_workspace_bytes(d);      // depends on which histogram outputs are non-NULL only
 
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o += up256(bytes); return r; };
@@ -64,6 +67,10 @@ static bool make_plan(const hepk_chain_desc* d, long long B, HostPlan* p)
     }
     for (int ob = 0; ob < HEPK_N_OBS; ++ob)
         if (d->axis_edges[ob]) p->axis[ob] = take((size_t)(d->axis_nbins[ob] + 1) * 4);
+    if (d->evw_table) {
+        p->evw_edges = take((size_t)(d->evw_nbins + 1) * 4);
+        p->evw_table = take((size_t)d->evw_nbins * 4);
+    }
     p->shared_bytes = o;
 
     SlotLayout& s = p->slot;
@@ -76,24 +83,30 @@ static bool make_plan(const hepk_chain_desc* d, long long B, HostPlan* p)
     for (int c = 0; c < 3; ++c) s.mcol[c] = take((size_t)p->maxM * 4);
     for (int c = 0; c < 3; ++c) s.ecol[c] = take((size_t)p->maxE * 4);
     s.weights = take(d->weights ? (size_t)W * B * 4 : 0);
+    s.evw_x = take(d->evw_table ? (size_t)B * 4 : 0);
     for (int c = 0; c < 2; ++c) s.out_i[c] = take((size_t)V * B * 4);
     for (int c = 0; c < 5; ++c) s.out_f[c] = take((size_t)V * B * 4);
     s.out_mask = take(d->out_jet_mask ? (size_t)V * p->maxJ : 0);
     s.hist_sumw = take((size_t)p->n_sumw * 4);
+    s.hist_sumw2 = take((size_t)p->n_sumw2 * 4);
     s.hist_counts = take((size_t)p->n_cnt * 8);
-    s.chain_ws = take((size_t)(p->n_sumw > 0 ? p->n_sumw : 1) * 8 + 16);
+    s.chain_ws = take(p->chain_ws_bytes);
     s.bytes = o;
     return true;
 }
 
-static cudaStream_t g_streams[2] = {nullptr, nullptr};
-
-static int32_t ensure_streams()
-{
-    for (int i = 0; i < 2; ++i)
-        if (!g_streams[i]) HEPK_CUDA_TRY(cudaStreamCreateWithFlags(&g_streams[i], cudaStreamNonBlocking));
-    return HEPK_OK;
-}
+// Two copy/compute streams owned by ONE call (created on the current device, destroyed before it returns), so
+// concurrent calls from several host threads or on several devices share nothing.
+struct CallStreams {
+    cudaStream_t s[2] = {nullptr, nullptr};
+    bool own = false;
+    ~CallStreams()
+    {
+        if (!own) return;
+        for (int i = 0; i < 2; ++i)
+            if (s[i]) { cudaStreamSynchronize(s[i]); cudaStreamDestroy(s[i]); }   // drains work in flight on an error return
+    }
+};
 
 }  // namespace hepk
 
@@ -125,13 +138,16 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
     HEPK_REQUIRE(((uintptr_t)workspace & 255) == 0, "workspace must be 256-byte aligned");
 
     cudaStream_t user = (cudaStream_t)stream;
+    CallStreams cs;
     cudaStream_t st[2] = {user, user};
     if (overlap) {
-        int32_t rc = ensure_streams();
-        if (rc != HEPK_OK) return rc;
-        st[0] = g_streams[0]; st[1] = g_streams[1];
+        cs.own = true;
+        for (int i = 0; i < 2; ++i) HEPK_CUDA_TRY(cudaStreamCreateWithFlags(&cs.s[i], cudaStreamNonBlocking));
+        st[0] = cs.s[0]; st[1] = cs.s[1];
         HEPK_CUDA_TRY(cudaStreamSynchronize(user));     // earlier work of the caller's stream is complete
     }
+    // on an error return after work was enqueued on the caller's stream, wait for it before handing the buffers back
+    struct Drain { cudaStream_t q; bool armed; ~Drain() { if (armed) cudaStreamSynchronize(q); } } drain{user, true};
     unsigned char* base = (unsigned char*)workspace;
     unsigned char* slot_base[2] = {base + p.shared_bytes, base + p.shared_bytes + p.slot.bytes};
     const bool has_el = d->electrons.offsets != nullptr;
@@ -153,8 +169,16 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
             HEPK_CUDA_TRY(cudaMemcpyAsync(base + p.axis[ob], d->axis_edges[ob], (size_t)(d->axis_nbins[ob] + 1) * 4, cudaMemcpyHostToDevice, st[0]));
             tmpl.axis_edges[ob] = (const float*)(base + p.axis[ob]);
         }
+    if (d->evw_table) {
+        HEPK_REQUIRE(d->evw_x && d->evw_edges && d->evw_nbins >= 1, "event-weight lookup: x, edges or bins missing");
+        HEPK_CUDA_TRY(cudaMemcpyAsync(base + p.evw_edges, d->evw_edges, (size_t)(d->evw_nbins + 1) * 4, cudaMemcpyHostToDevice, st[0]));
+        HEPK_CUDA_TRY(cudaMemcpyAsync(base + p.evw_table, d->evw_table, (size_t)d->evw_nbins * 4, cudaMemcpyHostToDevice, st[0]));
+        tmpl.evw_edges = (const float*)(base + p.evw_edges);
+        tmpl.evw_table = (const float*)(base + p.evw_table);
+    }
     for (int s = 0; s < n_slots; ++s) {
         if (p.n_sumw) HEPK_CUDA_TRY(cudaMemsetAsync(slot_base[s] + p.slot.hist_sumw, 0, (size_t)p.n_sumw * 4, st[0]));
+        if (p.n_sumw2) HEPK_CUDA_TRY(cudaMemsetAsync(slot_base[s] + p.slot.hist_sumw2, 0, (size_t)p.n_sumw2 * 4, st[0]));
         if (p.n_cnt) HEPK_CUDA_TRY(cudaMemsetAsync(slot_base[s] + p.slot.hist_counts, 0, (size_t)p.n_cnt * 8, st[0]));
     }
     if (overlap) HEPK_CUDA_TRY(cudaStreamSynchronize(st[0]));   // tables visible to both streams
@@ -197,26 +221,32 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
                                               (size_t)nb * 4, cudaMemcpyHostToDevice, q));
             bd.weights = (const float*)(sb + p.slot.weights);
         }
+        if (d->evw_table) {
+            HEPK_CUDA_TRY(cudaMemcpyAsync(sb + p.slot.evw_x, d->evw_x + e0, (size_t)nb * 4, cudaMemcpyHostToDevice, q));
+            bd.evw_x = (const float*)(sb + p.slot.evw_x);
+        }
         int** out_i_dev[2] = {&bd.out_njet, &bd.out_argmax};
         float** out_f_dev[5] = {&bd.out_ht, &bd.out_maxpt, &bd.out_minpt, &bd.out_mjj, &bd.out_subpt};
         for (int c = 0; c < 2; ++c) *out_i_dev[c] = out_i_host[c] ? (int*)(sb + p.slot.out_i[c]) : nullptr;
         for (int c = 0; c < 5; ++c) *out_f_dev[c] = out_f_host[c] ? (float*)(sb + p.slot.out_f[c]) : nullptr;
         bd.out_jet_mask = d->out_jet_mask ? (uint8_t*)(sb + p.slot.out_mask) : nullptr;
         bd.hist_sumw = p.n_sumw ? (float*)(sb + p.slot.hist_sumw) : nullptr;
+        bd.hist_sumw2 = p.n_sumw2 ? (float*)(sb + p.slot.hist_sumw2) : nullptr;
         bd.hist_counts = p.n_cnt ? (int64_t*)(sb + p.slot.hist_counts) : nullptr;
 
-        const int32_t rc = hepk_analysis_chain(&bd, sb + p.slot.chain_ws, (size_t)(p.n_sumw > 0 ? p.n_sumw : 1) * 8 + 16, q);
+        const int32_t rc = hepk_analysis_chain(&bd, sb + p.slot.chain_ws, p.chain_ws_bytes, q);
         if (rc != HEPK_OK) return rc;
 
+        // per-event outputs: device [V][nb] -> host [V][N] at column e0, ONE strided copy per output and batch
+        for (int c = 0; c < 2; ++c)
+            if (out_i_host[c])
+                HEPK_CUDA_TRY(cudaMemcpy2DAsync(out_i_host[c] + e0, (size_t)N * 4, sb + p.slot.out_i[c], (size_t)nb * 4,
+                                                (size_t)nb * 4, (size_t)V, cudaMemcpyDeviceToHost, q));
+        for (int c = 0; c < 5; ++c)
+            if (out_f_host[c])
+                HEPK_CUDA_TRY(cudaMemcpy2DAsync(out_f_host[c] + e0, (size_t)N * 4, sb + p.slot.out_f[c], (size_t)nb * 4,
+                                                (size_t)nb * 4, (size_t)V, cudaMemcpyDeviceToHost, q));
         for (int v = 0; v < V; ++v) {
-            for (int c = 0; c < 2; ++c)
-                if (out_i_host[c])
-                    HEPK_CUDA_TRY(cudaMemcpyAsync(out_i_host[c] + (size_t)v * N + e0, sb + p.slot.out_i[c] + (size_t)v * nb * 4,
-                                                  (size_t)nb * 4, cudaMemcpyDeviceToHost, q));
-            for (int c = 0; c < 5; ++c)
-                if (out_f_host[c])
-                    HEPK_CUDA_TRY(cudaMemcpyAsync(out_f_host[c] + (size_t)v * N + e0, sb + p.slot.out_f[c] + (size_t)v * nb * 4,
-                                                  (size_t)nb * 4, cudaMemcpyDeviceToHost, q));
             if (d->out_jet_mask && bd.jets.n_objects > 0)
                 HEPK_CUDA_TRY(cudaMemcpyAsync(d->out_jet_mask + (size_t)v * d->jets.n_objects + (bd.jets.content_base - d->jets.content_base),
                                               sb + p.slot.out_mask + (size_t)v * bd.jets.n_objects, (size_t)bd.jets.n_objects,
@@ -224,14 +254,19 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
         }
     }
     // histograms: one copy back per buffer set, added on the host in float64
-    std::vector<float> hs((size_t)p.n_sumw);
+    const long long n_max = p.n_sumw > p.n_sumw2 ? p.n_sumw : p.n_sumw2;
+    std::vector<float> hs((size_t)n_max);
     std::vector<long long> hc((size_t)p.n_cnt);
-    std::vector<double> acc((size_t)p.n_sumw, 0.0);
+    std::vector<double> acc((size_t)p.n_sumw, 0.0), acc2((size_t)p.n_sumw2, 0.0);
     for (int s = 0; s < n_slots; ++s) {
         HEPK_CUDA_TRY(cudaStreamSynchronize(st[s]));
         if (p.n_sumw) {
             HEPK_CUDA_TRY(cudaMemcpy(hs.data(), slot_base[s] + p.slot.hist_sumw, (size_t)p.n_sumw * 4, cudaMemcpyDeviceToHost));
             for (long long i = 0; i < p.n_sumw; ++i) acc[i] += (double)hs[i];
+        }
+        if (p.n_sumw2) {
+            HEPK_CUDA_TRY(cudaMemcpy(hs.data(), slot_base[s] + p.slot.hist_sumw2, (size_t)p.n_sumw2 * 4, cudaMemcpyDeviceToHost));
+            for (long long i = 0; i < p.n_sumw2; ++i) acc2[i] += (double)hs[i];
         }
         if (p.n_cnt) {
             HEPK_CUDA_TRY(cudaMemcpy(hc.data(), slot_base[s] + p.slot.hist_counts, (size_t)p.n_cnt * 8, cudaMemcpyDeviceToHost));
@@ -239,5 +274,7 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
         }
     }
     for (long long i = 0; i < p.n_sumw; ++i) d->hist_sumw[i] = (float)((double)d->hist_sumw[i] + acc[i]);
+    for (long long i = 0; i < p.n_sumw2; ++i) d->hist_sumw2[i] = (float)((double)d->hist_sumw2[i] + acc2[i]);
+    drain.armed = false;
     return HEPK_OK;
 }

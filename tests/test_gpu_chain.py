@@ -315,3 +315,87 @@ def test_chain_full_size_config2_sampled(hk):
         sw, ct = plan.hist_view(name)
         assert to_np(ct).sum() == N
         assert abs(to_np(sw).astype(np.float64).sum() - tot) <= 1e-5 * tot
+
+
+# ---------------------------------------------------------------------------------------------- SURVEY.md 8(f-2)
+def _evw_np(wl, seed=5):
+    rng = np.random.default_rng(seed)
+    return dict(x=rng.uniform(-3, 65, wl.n_events).astype(np.float32), edges=np.linspace(0, 60, 31).astype(np.float32),
+                table=rng.uniform(0.6, 1.4, 30).astype(np.float32))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,n", [(1, 200_003), (2, 100_001), (4, 20_001)])
+def test_chain_event_weight_lookup_and_sumw2(hk, cfg, n):
+    """hepk_chain_desc.evw_* and hist_sumw2 against the oracle."""
+    wl = hepgen.generate(cfg, n_events=n)
+    evw = _evw_np(wl)
+    ref = hepo.analysis_chain(wl, want_mask=False, evw=evw, want_sumw2=True)
+    inp = hk.upload(wl)
+    inp.evw = {k: torch.from_numpy(v).cuda() for k, v in evw.items()}
+    out, plan = hk.analysis_chain(inp, want_sumw2=True)
+    torch.cuda.synchronize()
+    assert_exact(to_np(out["hist_counts"]), ref["hist_counts"], "counts")
+    assert_tol(to_np(out["hist_sumw"]), ref["hist_sumw"], "sumw with lookup factor")
+    assert_tol(to_np(out["hist_sumw2"]), ref["hist_sumw2"], "sumw2 with lookup factor")
+    assert_exact(to_np(out["njet"]), ref["njet"])
+    # sumw2 alone, without weights and factor: equals the counts
+    inp2 = hk.upload(wl)
+    inp2.weights = None
+    out2, _ = hk.analysis_chain(inp2, want_event_outputs=False, want_sumw2=True)
+    torch.cuda.synchronize()
+    V, W = 1 if wl.calib is None else len(wl.calib["scales"]), 1
+    assert_exact(to_np(out2["hist_sumw2"]), to_np(out2["hist_counts"]).astype(np.float32), "sumw2 == counts for unit weights")
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kind", ["outlier", "mixed_sign", "one_bin", "tiny_and_huge"])
+def test_chain_weight_dynamic_range(hk, kind):
+    """Weighted bins with a dynamic range inside one launch: the fixed-point bins are only used when the
+    weights span at most a factor 8; every case must stay within the tolerance of the float64 oracle."""
+    wl = hepgen.generate(2, n_events=150_001)
+    rng = np.random.default_rng(11)
+    w = wl.weights.copy()
+    if kind == "outlier":
+        w[0, 12345] = 2000.0                                   # one large generator weight sets max|w|
+    elif kind == "mixed_sign":
+        w[0] *= rng.choice(np.float32([-1.0, 1.0]), w.shape[1], p=[0.1, 0.9])
+    elif kind == "one_bin":
+        wl.jets.pt[:] = 25.0                                   # no clean jets: every event lands in the first HT bin
+    elif kind == "tiny_and_huge":
+        w[0] *= np.float32(10.0) ** rng.integers(-3, 4, w.shape[1]).astype(np.float32)
+    wl.weights = np.ascontiguousarray(w, dtype=np.float32)
+    ref = hepo.analysis_chain(wl, want_mask=False, want_sumw2=True)
+    out, _ = hk.analysis_chain(hk.upload(wl), want_event_outputs=False, want_sumw2=True)
+    torch.cuda.synchronize()
+    assert_exact(to_np(out["hist_counts"]), ref["hist_counts"])
+    if kind == "mixed_sign":
+        # cancelling sums: the bound is relative to sum |w| of the bin (include/hepk.h), checked against sumw2-free abs sums
+        absref = hepo.analysis_chain(_with_weights(wl, np.abs(wl.weights)), want_mask=False)["hist_sumw"]
+        err = np.abs(to_np(out["hist_sumw"]).astype(np.float64) - ref["hist_sumw"])
+        assert (err <= 1e-5 * np.abs(absref) + 1e-6).all(), err.max()
+    else:
+        assert_tol(to_np(out["hist_sumw"]), ref["hist_sumw"], f"sumw ({kind})")
+    assert_tol(to_np(out["hist_sumw2"]), ref["hist_sumw2"], f"sumw2 ({kind})")
+
+
+def _with_weights(wl, w):
+    import copy
+    c = copy.copy(wl)
+    c.weights = np.ascontiguousarray(w, dtype=np.float32)
+    return c
+
+
+@pytest.mark.gpu
+def test_chain_host_event_weight_and_sumw2(hk):
+    wl = hepgen.generate(3, n_events=60_001)
+    evw = _evw_np(wl)
+    ref = hepo.analysis_chain(wl, want_mask=False, evw=evw, want_sumw2=True)
+    hp = hk.HostChainPlan(wl, batch_events=17_000, want_sumw2=True, evw=evw)
+    out = hp.run(overlap=True)
+    assert_exact(out["hist_counts"].numpy(), ref["hist_counts"])
+    assert_tol(out["hist_sumw"].numpy(), ref["hist_sumw"], "host path sumw")
+    assert_tol(out["hist_sumw2"].numpy(), ref["hist_sumw2"], "host path sumw2")
+    for k in ("njet", "argmax", "maxpt"):
+        assert_exact(out[k].numpy(), ref[k], k)
+    assert_tol(out["ht"].numpy(), ref["ht"], "ht")
