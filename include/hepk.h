@@ -146,7 +146,9 @@ int32_t hepk_lookup_binned(const float* x, const float* y, int64_t n,
  *   edges[b] <= x < edges[b+1].   sumw[slot] += w (w = 1 if weights == NULL); counts[slot] += 1.
  * data, weights: float32[n]; edges: float32[nbins+1] ascending; sumw: float32[nbins+2] or NULL;
  * counts: int64[nbins+2] or NULL.  Both outputs accumulate.  Bins are privatised per CTA in shared
- * memory and merged with global atomics; nbins+2 <= 16384, else HEPK_ERR_UNSUPPORTED. */
+ * memory (float32 partial sums) and merged into the caller's float32 array with float atomics, so sumw
+ * depends on the merge order in its last bits; hepk_fill_histogram_w2 (below) takes a workspace and merges
+ * in 64 bits.  nbins+2 <= 16384, else HEPK_ERR_UNSUPPORTED. */
 int32_t hepk_fill_histogram(const float* data, const float* weights, int64_t n,
                             const float* edges, int32_t nbins,
                             float* sumw, int64_t* counts, void* stream);
@@ -214,6 +216,10 @@ typedef struct hepk_chain_desc {
     /* sum of squared (final) weights per slot (the uncertainty of a weighted bin), layout of
      * hist_sumw, accumulates; NULL = not wanted.  Without weights and factor it equals the counts. */
     float* hist_sumw2;
+    /* Row strides, in events, of `weights` ([n_wvar] rows) and of every per-event output array ([n_variants] rows);
+     * 0 = n_events (contiguous rows).  A shard of a larger workload (PAPER.md:L166 multi-GPU) passes
+     * pointers to its first event inside the whole arrays and the whole workload's event count here. */
+    int64_t weights_stride; int64_t out_stride;
     /* RESERVED for the library's own tests (staging capacities and CTA shape); leave 0 = automatic */
     int32_t tune_cap_jets;       /* shared-memory capacity (jets per staged 32-event tile) */
     int32_t tune_cap_leptons;    /* capacity per lepton collection */
@@ -301,6 +307,33 @@ size_t  hepk_hist2d_workspace_bytes(int32_t nx, int32_t ny);
 int32_t hepk_fill_histogram_2d(const float* x, const float* y, const float* weights, int64_t n,
                                const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
                                float* sumw, int64_t* counts, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Weighted fills with the sum of squared weights (PAPER.md:L109 `fill_histogram`; the squared sum is the statistical
+ * uncertainty of a weighted bin), one and two dimensions.  Slots and conventions of hepk_fill_histogram /
+ * hepk_fill_histogram_2d; additionally sumw2[slot] += w*w (w = 1 if weights == NULL, so sumw2 == counts).
+ * sumw, sumw2: float32, counts: int64, each nullable, all accumulate.  `workspace`: device buffer of at least
+ * hepk_hist_workspace_bytes(nx, ny) bytes (ny = 0 for one dimension; 64-bit accumulators), private to the call
+ * until the stream reaches its end.  Tolerance class, same guarantee as the chain's weighted bins: fixed-point
+ * bins (exact integer sums) for small histograms whose weights are finite and within a factor 8 of each other,
+ * float32 partial sums of at most 32768 entries merged in float64 otherwise.  nbins+2 (resp. (nx+2)*(ny+2))
+ * <= 16384 and rows x columns must fit 200 KB of shared memory, else HEPK_ERR_UNSUPPORTED. */
+size_t  hepk_hist_workspace_bytes(int32_t nx, int32_t ny);
+int32_t hepk_fill_histogram_w2(const float* data, const float* weights, int64_t n, const float* edges, int32_t nbins,
+                               float* sumw, float* sumw2, int64_t* counts, void* workspace, size_t workspace_bytes,
+                               void* stream);
+int32_t hepk_fill_histogram_2d_w2(const float* x, const float* y, const float* weights, int64_t n,
+                                  const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                                  float* sumw, float* sumw2, int64_t* counts, void* workspace, size_t workspace_bytes,
+                                  void* stream);
+
+/* Event weight from a histogram lookup ("event weight computation based on histogram lookups:
+ * pileup, lepton efficiency corrections"):
+ *   w_out[e] = w_in[e] * table[B(x[e])]     one float32 multiply (exact class); w_in == NULL: w_in = 1
+ * B: the clamped bin of hepk_lookup_binned on edges[nbins+1].  x, w_in, w_out: float32[n] (w_out may alias w_in);
+ * table: float32[nbins].  2*nbins+1 floats must fit 200 KB of shared memory, else HEPK_ERR_UNSUPPORTED.
+ * The fused chain applies the same factor through hepk_chain_desc.evw_*. */
+int32_t hepk_event_weight_lookup(const float* w_in, const float* x, int64_t n, const float* edges, int32_t nbins,
+                                 const float* table, float* w_out, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
  * Jet-triplet candidate ("top quark candidate from jet triplet with invariant

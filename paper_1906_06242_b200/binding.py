@@ -52,6 +52,7 @@ class ChainDesc(C.Structure):
         ("hist_sumw", C.c_void_p), ("hist_counts", C.c_void_p),
         ("evw_x", C.c_void_p), ("evw_edges", C.c_void_p), ("evw_nbins", C.c_int32), ("evw_table", C.c_void_p),
         ("hist_sumw2", C.c_void_p),
+        ("weights_stride", C.c_int64), ("out_stride", C.c_int64),
         ("tune_cap_jets", C.c_int32), ("tune_cap_leptons", C.c_int32),
         ("tune_ctas_per_sm", C.c_int32), ("tune_warps_per_cta", C.c_int32), ("tune_warps_per_sm", C.c_int32),
         ("tune_variants_per_pass", C.c_int32),
@@ -263,6 +264,59 @@ def fill_histogram_2d(x, y, weights, edges_x, edges_y, sumw=None, counts=None, w
     return sumw, counts
 
 
+def _hist_ws(nx, ny, dev):
+    L = lib()
+    L.hepk_hist_workspace_bytes.restype = C.c_size_t
+    return torch.empty(max(int(L.hepk_hist_workspace_bytes(C.c_int32(nx), C.c_int32(ny))), 8), dtype=torch.uint8, device=dev)
+
+
+def fill_histogram_w2(data, weights, edges, sumw=None, sumw2=None, counts=None, want=("sumw", "sumw2", "counts"), stream=None):
+    """Returns (sumw, sumw2 float32[nbins+2], counts int64[nbins+2]); arrays not in `want` and not given are None."""
+    nbins = edges.numel() - 1
+    dev = edges.device
+    if sumw is None and "sumw" in want:
+        sumw = torch.zeros(nbins + 2, dtype=torch.float32, device=dev)
+    if sumw2 is None and "sumw2" in want:
+        sumw2 = torch.zeros(nbins + 2, dtype=torch.float32, device=dev)
+    if counts is None and "counts" in want:
+        counts = torch.zeros(nbins + 2, dtype=torch.int64, device=dev)
+    ws = _hist_ws(nbins, 0, dev)
+    _check(lib().hepk_fill_histogram_w2(_ptr(data, torch.float32), _ptr(weights, torch.float32), C.c_int64(data.numel()),
+                                        _ptr(edges, torch.float32), C.c_int32(nbins), _ptr(sumw, torch.float32),
+                                        _ptr(sumw2, torch.float32), _ptr(counts, torch.int64), C.c_void_p(ws.data_ptr()),
+                                        C.c_size_t(ws.numel()), _stream(stream)), "fill_histogram_w2")
+    return sumw, sumw2, counts
+
+
+def fill_histogram_2d_w2(x, y, weights, edges_x, edges_y, sumw=None, sumw2=None, counts=None,
+                         want=("sumw", "sumw2", "counts"), stream=None):
+    nx, ny = edges_x.numel() - 1, edges_y.numel() - 1
+    dev = x.device
+    if sumw is None and "sumw" in want:
+        sumw = torch.zeros((nx + 2, ny + 2), dtype=torch.float32, device=dev)
+    if sumw2 is None and "sumw2" in want:
+        sumw2 = torch.zeros((nx + 2, ny + 2), dtype=torch.float32, device=dev)
+    if counts is None and "counts" in want:
+        counts = torch.zeros((nx + 2, ny + 2), dtype=torch.int64, device=dev)
+    ws = _hist_ws(nx, ny, dev)
+    _check(lib().hepk_fill_histogram_2d_w2(_ptr(x, torch.float32), _ptr(y, torch.float32), _ptr(weights, torch.float32),
+                                           C.c_int64(x.numel()), _ptr(edges_x, torch.float32), C.c_int32(nx),
+                                           _ptr(edges_y, torch.float32), C.c_int32(ny), _ptr(sumw, torch.float32),
+                                           _ptr(sumw2, torch.float32), _ptr(counts, torch.int64), C.c_void_p(ws.data_ptr()),
+                                           C.c_size_t(ws.numel()), _stream(stream)), "fill_histogram_2d_w2")
+    return sumw, sumw2, counts
+
+
+def event_weight_lookup(w_in, x, edges, table, out=None, stream=None):
+    n = x.numel()
+    if out is None:
+        out = torch.empty(n, dtype=torch.float32, device=x.device)
+    _check(lib().hepk_event_weight_lookup(_ptr(w_in, torch.float32), _ptr(x, torch.float32), C.c_int64(n),
+                                          _ptr(edges, torch.float32), C.c_int32(edges.numel() - 1), _ptr(table, torch.float32),
+                                          _ptr(out, torch.float32), _stream(stream)), "event_weight_lookup")
+    return out
+
+
 def triplet_mass(pt, eta, phi, mass, offsets, target, mask_rows=None, mask_content=None, content_base=0, want_indices=True,
                  stream=None):
     """Returns (mass float32[n_events], indices int32[n_events][3] or None)."""
@@ -381,7 +435,7 @@ def _fill_collection(s, c):
     s.pt, s.eta, s.phi = c.pt.data_ptr(), c.eta.data_ptr(), c.phi.data_ptr()
     s.mass = c.mass.data_ptr() if c.mass is not None else None
     for t in (c.offsets, c.pt, c.eta, c.phi):
-        assert t.is_cuda and t.is_contiguous()
+        assert t.is_cuda and (t.numel() <= 1 or t.stride(0) == 1)
     assert c.offsets.dtype == torch.int64 and c.pt.dtype == torch.float32
 
 
@@ -391,8 +445,10 @@ class ChainPlan:
     EVENT_OUTPUTS = ("njet", "argmax", "ht", "maxpt", "minpt", "mjj", "subpt")
 
     def __init__(self, inp: ChainInputs, want_event_outputs=True, want_mask=False, want_hists=True, want_counts=True,
-                 want_sumw2=False, tune=None):
-        """want_event_outputs: True (all seven), False (none) or a tuple of names from EVENT_OUTPUTS."""
+                 want_sumw2=False, tune=None, out_into=None, out_col=0):
+        """want_event_outputs: True (all seven), False (none) or a tuple of names from EVENT_OUTPUTS.
+        out_into: dict name -> tensor [V][N_total] of a larger workload; this plan (a shard of it) then writes its
+        per-event outputs at columns [out_col, out_col + n_events) of those arrays instead of allocating its own."""
         self.inp = inp
         dev = inp.jets.pt.device
         N, V, W = inp.n_events, inp.n_variants, inp.n_wvar
@@ -415,16 +471,25 @@ class ChainPlan:
                 d.calib_scales[i] = s
         d.n_variants, d.n_wvar = V, W
         if inp.weights is not None:
-            assert inp.weights.dtype == torch.float32 and inp.weights.is_contiguous() and inp.weights.shape == (W, N)
-            d.weights = inp.weights.data_ptr()
+            wt = inp.weights                   # [W][N], rows contiguous; a column slice of a larger array is fine
+            assert wt.dtype == torch.float32 and wt.shape == (W, N) and (N <= 1 or wt.stride(1) == 1)
+            d.weights = wt.data_ptr()
+            d.weights_stride = wt.stride(0) if W > 1 else 0
         self.out = {}
         if want_event_outputs:
             names = self.EVENT_OUTPUTS if want_event_outputs is True else tuple(want_event_outputs)
             for k in names:
                 assert k in self.EVENT_OUTPUTS, k
                 dt = torch.int32 if k in ("njet", "argmax") else torch.float32
-                self.out[k] = torch.empty((V, N), dtype=dt, device=dev)
-                setattr(d, "out_" + k, self.out[k].data_ptr())
+                if out_into is not None:
+                    whole = out_into[k]
+                    assert whole.dtype == dt and whole.is_contiguous() and whole.shape[0] == V
+                    self.out[k] = whole[:, out_col: out_col + N]
+                    d.out_stride = whole.shape[1]
+                    setattr(d, "out_" + k, whole.data_ptr() + 4 * out_col)
+                else:
+                    self.out[k] = torch.empty((V, N), dtype=dt, device=dev)
+                    setattr(d, "out_" + k, self.out[k].data_ptr())
         if want_mask:
             self.out["jet_mask"] = torch.zeros((V, inp.jets.pt.numel()), dtype=torch.uint8, device=dev)
             d.out_jet_mask = self.out["jet_mask"].data_ptr()
@@ -447,6 +512,7 @@ class ChainPlan:
                 t = inp.evw[k]
                 assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32, k
             assert inp.evw["x"].numel() == N and inp.evw["table"].numel() == inp.evw["edges"].numel() - 1
+            self._keep = inp.evw
             d.evw_x, d.evw_edges = inp.evw["x"].data_ptr(), inp.evw["edges"].data_ptr()
             d.evw_nbins, d.evw_table = inp.evw["table"].numel(), inp.evw["table"].data_ptr()
         for k, v in (tune or {}).items():
@@ -460,6 +526,10 @@ class ChainPlan:
         for k in ("hist_sumw", "hist_sumw2", "hist_counts"):
             if k in self.out:
                 self.out[k].zero_()
+
+    def zero_hists_on(self, stream):
+        with torch.cuda.stream(stream):
+            self.zero_hists()
 
     def run(self, stream=None):
         _check(lib().hepk_analysis_chain(C.byref(self.desc), C.c_void_p(self.workspace.data_ptr()),

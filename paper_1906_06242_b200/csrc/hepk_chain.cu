@@ -40,6 +40,7 @@ constexpr int N_BUCKETS = 8;        // jets are ordered by min(selected leptons 
 struct ChainParams {
     long long n_events;
     long long n_tiles;
+    long long w_stride, out_stride;   // row strides (in events) of the weights and of the per-event outputs
     // staged columns (see NCOL)
     const char* col_ptr[NCOL];      // element 0 of the column
     long long col_base[NCOL];       // content_base of the collection
@@ -427,7 +428,7 @@ __device__ __forceinline__ void add_weights(const ChainParams& P, unsigned feat,
         for (int w0 = 1; w0 < P.W; w0 += 8) {
             float x[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) x[k] = w0 + k < P.W ? __ldg(P.weights + (long long)(w0 + k) * P.n_events + ev) : 0.0f;
+            for (int k = 0; k < 8; ++k) x[k] = w0 + k < P.W ? __ldg(P.weights + (long long)(w0 + k) * P.w_stride + ev) : 0.0f;
 #pragma unroll
             for (int k = 0; k < 8; ++k)
                 if (w0 + k < P.W) one(w0 + k, (feat & F_EVW) ? __fmul_rn(x[k], evf) : x[k]);
@@ -460,7 +461,7 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
             if (near_lo || near_hi) mjj = pair_mass_f64(b1, eta1, phi1, m1, b2, eta2, phi2, m2);
         }
     }
-    const long long o = (long long)v * P.n_events + ev;
+    const long long o = (long long)v * P.out_stride + ev;
     if (feat & F_NJET) P.out_njet[o] = cnt;
     if (feat & F_ARGMAX) P.out_argmax[o] = i1;
     if (feat & F_HT) P.out_ht[o] = sum;
@@ -913,7 +914,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         for (int w = 0; w < NW; ++w) {
             wt[w] = 1.0f;
             if ((feat & F_WEIGHTS) && (feat & (F_SUMW | F_SUMW2)) && lane < ne && w < P.W)
-                wt[w] = __ldg(P.weights + (long long)w * P.n_events + e0 + lane);
+                wt[w] = __ldg(P.weights + (long long)w * P.w_stride + e0 + lane);
             if (feat & F_EVW) wt[w] = __fmul_rn(wt[w], evf);             // one float32 multiply (exact class)
         }
         EventOffsets neo;
@@ -1185,14 +1186,15 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
 // integers) and a flag for non-finite values, into the workspace header; the same for the event-weight table.
 // hdr[HDR_WMAX] = hdr[HDR_TMAX] = 0, hdr[HDR_WMIN] = hdr[HDR_TMIN] = +inf bits, hdr[HDR_BAD] = 0 set by the caller.
 // w == nullptr: every weight is 1.
-__global__ void chain_weight_range_kernel(const float* __restrict__ w, long long n, const float* __restrict__ table, int nt,
-                                          unsigned int* __restrict__ hdr)
+__global__ void chain_weight_range_kernel(const float* __restrict__ w, long long n, long long stride, int rows,
+                                          const float* __restrict__ table, int nt, unsigned int* __restrict__ hdr)
 {
-    auto fold = [&](const float* p, long long cnt, int imax, int imin) {
+    // p: `nrow` rows of `cnt` values, `rs` apart
+    auto fold = [&](const float* p, long long cnt, long long rs, int nrow, int imax, int imin) {
         float m = 0.0f, mn = CUDART_INF_F;
         bool bad = false;
-        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += (long long)gridDim.x * blockDim.x) {
-            const float a = fabsf(p[i]);
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt * nrow; i += (long long)gridDim.x * blockDim.x) {
+            const float a = fabsf(p[(i / cnt) * rs + i % cnt]);
             bad = bad || !(a < CUDART_INF_F);
             m = fmaxf(m, a);
             if (a > 0.0f) mn = fminf(mn, a);
@@ -1205,9 +1207,9 @@ __global__ void chain_weight_range_kernel(const float* __restrict__ w, long long
             atomicMin(hdr + imin, c);
         }
     };
-    if (w) fold(w, n, HDR_WMAX, HDR_WMIN);
+    if (w) fold(w, n, stride, rows, HDR_WMAX, HDR_WMIN);
     else if (blockIdx.x == 0 && threadIdx.x == 0) hdr[HDR_WMAX] = hdr[HDR_WMIN] = __float_as_uint(1.0f);
-    if (table) fold(table, nt, HDR_TMAX, HDR_TMIN);
+    if (table) fold(table, nt, nt, 1, HDR_TMAX, HDR_TMIN);
 }
 
 // The caller's arrays from the accumulators: word (v, o, slot, col) of the internal layout goes to
@@ -1353,6 +1355,8 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     memset(&P, 0, sizeof(P));
     P.n_events = d->n_events;
     P.n_tiles = (d->n_events + TILE_EVENTS - 1) / TILE_EVENTS;
+    P.w_stride = d->weights_stride > 0 ? d->weights_stride : d->n_events;
+    P.out_stride = d->out_stride > 0 ? d->out_stride : d->n_events;
     P.off[0] = (const long long*)d->jets.offsets;
     P.off[1] = (const long long*)d->muons.offsets;
     P.off[2] = (const long long*)d->electrons.offsets;
@@ -1520,7 +1524,8 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         long long blocks = (nw + 256 * 8 - 1) / (256 * 8);
         if (blocks > 4 * sm_count()) blocks = 4 * sm_count();
         if (blocks < 1) blocks = 1;
-        dev::chain_weight_range_kernel<<<(unsigned)blocks, 256, 0, st>>>(d->weights, nw, d->evw_table, d->evw_nbins, P.hist_hdr);
+        dev::chain_weight_range_kernel<<<(unsigned)blocks, 256, 0, st>>>(d->weights, P.n_events, P.w_stride, P.W, d->evw_table,
+                                                                         d->evw_nbins, P.hist_hdr);
         HEPK_CUDA_TRY(cudaGetLastError());
     }
     profile_mark(st, 0);
@@ -1573,7 +1578,7 @@ extern "C" int32_t hepk_analysis_chain(const hepk_chain_desc* d, void* workspace
         group = best_g;
     }
     if (group >= V) return chain_launch(d, workspace, (cudaStream_t)stream, nullptr);
-    const long long spv = hist_slots_per_variant(d), N = d->n_events, W = d->n_wvar;
+    const long long spv = hist_slots_per_variant(d), N = d->out_stride > 0 ? d->out_stride : d->n_events, W = d->n_wvar;
     for (int v0 = 0; v0 < V; v0 += group) {
         hepk_chain_desc t = *d;
         t.n_variants = v0 + group <= V ? group : V - v0;

@@ -1,0 +1,346 @@
+// hepk_hist.cu — weighted histogram fills with the sum of squared weights, and the event weight from a lookup
+// (include/hepk.h: hepk_fill_histogram_w2, hepk_fill_histogram_2d_w2, hepk_event_weight_lookup; SURVEY.md 8(f-2),
+// PAPER.md:L109, L134).
+//
+// One fill kernel for one and two dimensions.  Bins are privatised per CTA in shared memory, one ROW per slot
+// holding all columns of that slot (sumw, sumw2 value, sumw2 remainder, count), so an entry's updates are
+// immediate offsets from one address.  Small histograms (<= FIXED_WORDS words) take fixed-point int32 bins — native
+// shared-memory integer atomics, exact sums, any order — when a pre-pass over the weights finds them finite and
+// within a factor 8 of each other; every CTA checks all its bins after each step of 1024 entries and moves a bin
+// to its 64-bit global accumulator before it can leave the int32 range.  Everything else takes float32 bins
+// (compare-and-swap atomics) flushed into float64 accumulators at bounded intervals.
+#include "hepk_common.cuh"
+
+namespace hepk {
+namespace dev {
+
+enum { HH_WMAX = 0, HH_WMIN = 1, HH_BAD = 2, HH_WORDS = 4 };
+constexpr int HIST_FIXED_WORDS = 1024;      // privatised words a CTA can afford to check after every step
+constexpr int HIST_FLUSH_AT = 1 << 29;
+
+struct HistParams {
+    const float *x, *y, *w;
+    long long n;
+    const float *edges_x, *edges_y;
+    int nx, ny;                 // ny = 0: one dimension
+    int slots, WS, col_w2, col_cnt, want_sumw;      // columns: [sumw] [w2 value, w2 remainder] [count]; -1 = absent
+    long long* acc;             // [slots][WS] int64 fixed point or float64 bits
+    const unsigned int* hdr;    // weight range (HH_*)
+    float *sumw, *sumw2;
+    long long* counts;
+    int fixed_allowed;          // the histogram is small enough for the fixed-point scheme
+};
+
+__global__ void hist_weight_range_kernel(const float* __restrict__ w, long long n, unsigned int* __restrict__ hdr)
+{
+    float m = 0.0f, mn = CUDART_INF_F;
+    bool bad = false;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float a = fabsf(__ldg(w + i));
+        bad = bad || !(a < CUDART_INF_F);
+        m = fmaxf(m, a);
+        if (a > 0.0f) mn = fminf(mn, a);
+    }
+    const unsigned int b = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
+    const unsigned int c = __reduce_min_sync(0xffffffffu, __float_as_uint(mn));
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(hdr + HH_BAD, 1u);
+    if ((threadIdx.x & 31) == 0) {
+        if (b) atomicMax(hdr + HH_WMAX, b);
+        atomicMin(hdr + HH_WMIN, c);
+    }
+}
+
+// fixed-point scales 2^k (weights) and 2^k2 (squared weights): |w| 2^k < 2^19; 0: float bins
+__device__ __forceinline__ void hist_fill_scales(const HistParams& P, float& sc, float& sc2)
+{
+    sc = sc2 = 0.0f;
+    if (!P.fixed_allowed) return;
+    float wm = 1.0f, wn = 1.0f;
+    if (P.w) {
+        if (P.hdr[HH_BAD]) return;
+        wm = __uint_as_float(P.hdr[HH_WMAX]);
+        wn = __uint_as_float(P.hdr[HH_WMIN]);
+    }
+    if (!(wm > 0.0f && wm < CUDART_INF_F && wn > 0.0f && wm <= 8.0f * wn)) return;
+    if (!(wm * wm < CUDART_INF_F && wn * wn > 0.0f)) return;
+    int e, e2;
+    frexpf(wm, &e);
+    frexpf(wm * wm, &e2);
+    const int k = 19 - e, k2 = 19 - e2;
+    if (k <= -100 || k >= 100 || k2 <= -100 || k2 >= 100) return;
+    sc = ldexpf(1.0f, k);
+    sc2 = ldexpf(1.0f, k2);
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(256) hist_fill_kernel(const __grid_constant__ HistParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* s_ex = (float*)smem_raw;
+    float* s_ey = s_ex + (P.nx + 1);
+    int* s_bins = (int*)(s_ey + (P.ny > 0 ? P.ny + 1 : 0));
+    __shared__ float s_sc[2];
+    const int n_words = P.slots * P.WS;
+    for (int i = threadIdx.x; i <= P.nx; i += blockDim.x) s_ex[i] = P.edges_x[i];
+    if (P.ny > 0) for (int i = threadIdx.x; i <= P.ny; i += blockDim.x) s_ey[i] = P.edges_y[i];
+    for (int i = threadIdx.x; i < n_words; i += blockDim.x) s_bins[i] = 0;
+    if (threadIdx.x == 0) hist_fill_scales(P, s_sc[0], s_sc[1]);
+    __syncthreads();
+    const float sc = s_sc[0], sc2 = s_sc[1];
+    const bool fixed = sc != 0.0f;
+    const float lox = s_ex[0], invx = (float)P.nx / (s_ex[P.nx] - lox);
+    const float loy = P.ny > 0 ? s_ey[0] : 0.0f, invy = P.ny > 0 ? (float)P.ny / (s_ey[P.ny] - loy) : 0.0f;
+    const uint32_t bins_a = smem_u32(s_bins);
+
+    auto add = [&](float xv, float yv, float wv) {
+        int s = hist_slot(xv, s_ex, P.nx, lox, invx);
+        if (P.ny > 0) s = s * (P.ny + 2) + hist_slot(yv, s_ey, P.ny, loy, invy);
+        int* row = s_bins + s * P.WS;
+        if (fixed) {
+            if (P.want_sumw) red_shared_add_u32(row, (unsigned int)__float2int_rn(wv * sc));
+            if (P.col_w2 >= 0) {
+                const float y2 = wv * wv * sc2;
+                const int qh = __float2int_rn(y2);
+                red_shared_add_u32(row + P.col_w2, (unsigned int)qh);
+                red_shared_add_u32(row + P.col_w2 + 1, (unsigned int)__float2int_rn((y2 - (float)qh) * 1048576.0f));
+            }
+        } else {
+            if (P.want_sumw) red_shared_add_f32(row, wv);
+            if (P.col_w2 >= 0) red_shared_add_f32(row + P.col_w2, wv * wv);
+        }
+        if (P.col_cnt >= 0) red_shared_add_u32(row + P.col_cnt, 1u);
+    };
+    // move bins into the global accumulators; `all`: everything non-zero, else only integers about to overflow
+    auto flush = [&](bool all) {
+        for (int i = threadIdx.x; i < n_words; i += blockDim.x) {
+            const int v = s_bins[i];
+            if (v == 0) continue;
+            const bool is_int = fixed || (i % P.WS) == P.col_cnt;
+            if (is_int) {
+                if (!all && (unsigned)(v + HIST_FLUSH_AT) < 2u * (unsigned)HIST_FLUSH_AT) continue;
+                const int y = atomicExch(s_bins + i, 0);
+                if (y) atomicAdd((unsigned long long*)P.acc + i, (unsigned long long)(long long)y);
+            } else {
+                const float y = atomicExch((float*)s_bins + i, 0.0f);
+                if (y != 0.0f) atomicAdd((double*)P.acc + i, (double)y);
+            }
+        }
+    };
+    (void)bins_a;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // fixed point: a step adds at most 1024 entries < 2^19 each to a bin, so a check per step keeps |bin| < 2^31;
+    // float: bounded partial sums (a flush every 32 steps)
+    const int check_every = fixed ? 1 : 32;
+    if (VEC) {
+        const long long n4 = P.n / 4;
+        const long long iters = (n4 + stride - 1) / stride;
+        for (long long it = 0; it < iters; ++it) {
+            const long long g = t0 + it * stride;
+            if (g < n4) {
+                const float4 xv = __ldg((const float4*)P.x + g);
+                const float4 yv = P.ny > 0 ? __ldg((const float4*)P.y + g) : make_float4(0.f, 0.f, 0.f, 0.f);
+                const float4 wv = P.w ? __ldg((const float4*)P.w + g) : make_float4(1.f, 1.f, 1.f, 1.f);
+                add(xv.x, yv.x, wv.x); add(xv.y, yv.y, wv.y); add(xv.z, yv.z, wv.z); add(xv.w, yv.w, wv.w);
+            }
+            if ((it + 1) % check_every == 0) flush(!fixed);
+        }
+        for (long long i = n4 * 4 + t0; i < P.n; i += stride) add(P.x[i], P.ny > 0 ? P.y[i] : 0.f, P.w ? P.w[i] : 1.f);
+    } else {
+        const long long iters = (P.n + stride - 1) / stride;
+        for (long long it = 0; it < iters; ++it) {
+            const long long i = t0 + it * stride;
+            if (i < P.n) add(P.x[i], P.ny > 0 ? P.y[i] : 0.f, P.w ? P.w[i] : 1.f);
+            if ((it + 1) % (4 * check_every) == 0) flush(!fixed);
+        }
+    }
+    __syncthreads();
+    flush(true);
+}
+
+// the caller's arrays from the accumulators (one thread per slot)
+__global__ void hist_finalize_kernel(const __grid_constant__ HistParams P)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.slots) return;
+    float sc, sc2;
+    hist_fill_scales(P, sc, sc2);
+    const long long* row = P.acc + (long long)s * P.WS;
+    if (P.want_sumw && P.sumw) {
+        const double add = sc != 0.0f ? (double)row[0] / (double)sc : __longlong_as_double(row[0]);
+        P.sumw[s] = (float)((double)P.sumw[s] + add);
+    }
+    if (P.col_w2 >= 0) {
+        const double add = sc2 != 0.0f ? ((double)row[P.col_w2] + (double)row[P.col_w2 + 1] * (1.0 / 1048576.0)) / (double)sc2
+                                       : __longlong_as_double(row[P.col_w2]);
+        P.sumw2[s] = (float)((double)P.sumw2[s] + add);
+    }
+    if (P.col_cnt >= 0) P.counts[s] += row[P.col_cnt];
+}
+
+// w_out = w_in * table[B(x)]: one float32 multiply per event (exact class)
+__global__ void __launch_bounds__(256) event_weight_lookup_kernel(const float* __restrict__ w_in, const float* __restrict__ x,
+                                                                  long long n, const float* __restrict__ edges, int nb,
+                                                                  const float* __restrict__ table, float* __restrict__ w_out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* s_e = (float*)smem_raw;
+    float* s_t = s_e + (nb + 1);
+    for (int i = threadIdx.x; i <= nb; i += blockDim.x) s_e[i] = edges[i];
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) s_t[i] = table[i];
+    __syncthreads();
+    const AxisGuess ax = classify_axis(s_e, nb);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool vec = ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(w_out) | reinterpret_cast<uintptr_t>(w_in)) & 15u) == 0;
+    if (vec) {
+        const long long n4 = n / 4;
+        for (long long g = t0; g < n4; g += stride) {
+            const float4 xv = __ldg((const float4*)x + g);
+            const float4 wv = w_in ? __ldg((const float4*)w_in + g) : make_float4(1.f, 1.f, 1.f, 1.f);
+            float4 o;
+            o.x = __fmul_rn(wv.x, s_t[find_bin_guess(xv.x, s_e, nb, ax)]);
+            o.y = __fmul_rn(wv.y, s_t[find_bin_guess(xv.y, s_e, nb, ax)]);
+            o.z = __fmul_rn(wv.z, s_t[find_bin_guess(xv.z, s_e, nb, ax)]);
+            o.w = __fmul_rn(wv.w, s_t[find_bin_guess(xv.w, s_e, nb, ax)]);
+            ((float4*)w_out)[g] = o;
+        }
+        for (long long i = n4 * 4 + t0; i < n; i += stride)
+            w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, s_t[find_bin_guess(x[i], s_e, nb, ax)]);
+    } else {
+        for (long long i = t0; i < n; i += stride)
+            w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, s_t[find_bin_guess(x[i], s_e, nb, ax)]);
+    }
+}
+
+}  // namespace dev
+
+static unsigned grid_for_items(long long items)
+{
+    long long g = (items + 255) / 256;
+    const long long maxb = (long long)sm_count() * 8;
+    if (g > maxb) g = maxb;
+    return (unsigned)(g < 1 ? 1 : g);
+}
+
+struct HistShape { int slots, ncol, WS, col_w2, col_cnt, want_sumw; };
+static HistShape hist_shape(int nx, int ny, bool sumw, bool sumw2, bool counts)
+{
+    HistShape h;
+    h.slots = (nx + 2) * (ny > 0 ? ny + 2 : 1);
+    h.want_sumw = sumw ? 1 : 0;
+    h.ncol = 1;                                   // column 0 is sumw (kept, unused, when not asked for)
+    h.col_w2 = -1; h.col_cnt = -1;
+    if (sumw2) { h.col_w2 = h.ncol; h.ncol += 2; }
+    if (counts) { h.col_cnt = h.ncol; h.ncol += 1; }
+    h.WS = (h.ncol & 1) ? h.ncol : h.ncol + 1;    // odd row length: the rows of a column cover all banks
+    return h;
+}
+
+static int32_t hist_fill_launch(const char* who, const float* x, const float* y, const float* weights, long long n,
+                                const float* edges_x, int nx, const float* edges_y, int ny, float* sumw, float* sumw2,
+                                long long* counts, void* workspace, size_t workspace_bytes, cudaStream_t st)
+{
+    const HistShape h = hist_shape(nx, ny, sumw != nullptr, sumw2 != nullptr, counts != nullptr);
+    if (n == 0 || (!sumw && !sumw2 && !counts)) return HEPK_OK;
+    const size_t need = dev::HH_WORDS * 4 + (size_t)h.slots * h.WS * 8;
+    if (!workspace || workspace_bytes < need) {
+        set_error("%s: workspace is NULL or smaller than %zu bytes", who, need);
+        return HEPK_ERR_INVALID;
+    }
+    const size_t smem = ((size_t)(nx + 1) + (ny > 0 ? (size_t)(ny + 1) : 0) + (size_t)h.slots * h.WS) * 4;
+    if (smem > 200 * 1024) {
+        set_error("%s: %d slots x %d columns do not fit 200 KB of shared memory", who, h.slots, h.WS);
+        return HEPK_ERR_UNSUPPORTED;
+    }
+    dev::HistParams P;
+    P.x = x; P.y = y; P.w = weights; P.n = n;
+    P.edges_x = edges_x; P.edges_y = edges_y; P.nx = nx; P.ny = ny;
+    P.slots = h.slots; P.WS = h.WS; P.col_w2 = h.col_w2; P.col_cnt = h.col_cnt; P.want_sumw = h.want_sumw;
+    P.hdr = (const unsigned int*)workspace;
+    P.acc = (long long*)((char*)workspace + dev::HH_WORDS * 4);
+    P.sumw = sumw; P.sumw2 = sumw2; P.counts = counts;
+    P.fixed_allowed = h.slots * h.WS <= dev::HIST_FIXED_WORDS ? 1 : 0;
+    HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, need, st));
+    if (weights && P.fixed_allowed) {
+        static const unsigned int inf_bits = 0x7f800000u;
+        HEPK_CUDA_TRY(cudaMemcpyAsync((unsigned int*)workspace + dev::HH_WMIN, &inf_bits, 4, cudaMemcpyHostToDevice, st));
+        dev::hist_weight_range_kernel<<<grid_for_items((n + 7) / 8), 256, 0, st>>>(weights, n, (unsigned int*)workspace);
+        HEPK_CUDA_TRY(cudaGetLastError());
+    }
+    const bool vec = aligned16(x) && (!y || aligned16(y)) && (!weights || aligned16(weights));
+    auto kern = vec ? dev::hist_fill_kernel<true> : dev::hist_fill_kernel<false>;
+    HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem) != cudaSuccess || occ < 1) occ = 1;
+    long long grid = (long long)sm_count() * occ;
+    const long long items = (n + 1023) / 1024;
+    if (grid > items) grid = items;
+    if (grid < 1) grid = 1;
+    kern<<<(unsigned)grid, 256, smem, st>>>(P);
+    HEPK_CUDA_TRY(cudaGetLastError());
+    dev::hist_finalize_kernel<<<(unsigned)((h.slots + 255) / 256), 256, 0, st>>>(P);
+    HEPK_CUDA_TRY(cudaGetLastError());
+    return HEPK_OK;
+}
+
+}  // namespace hepk
+
+using namespace hepk;
+
+extern "C" size_t hepk_hist_workspace_bytes(int32_t nx, int32_t ny)
+{
+    if (nx < 1 || ny < 0) return 0;
+    const HistShape h = hist_shape(nx, ny, true, true, true);      // the largest shape: every output asked for
+    return dev::HH_WORDS * 4 + (size_t)h.slots * h.WS * 8;
+}
+
+extern "C" int32_t hepk_fill_histogram_w2(const float* data, const float* weights, int64_t n, const float* edges, int32_t nbins,
+                                          float* sumw, float* sumw2, int64_t* counts, void* workspace, size_t workspace_bytes,
+                                          void* stream)
+{
+    HEPK_REQUIRE(n >= 0, "n < 0");
+    HEPK_REQUIRE(edges && nbins >= 1, "edges is NULL or nbins < 1");
+    if (nbins + 2 > 16384) {
+        set_error("hepk_fill_histogram_w2: nbins+2 = %d exceeds 16384", nbins + 2);
+        return HEPK_ERR_UNSUPPORTED;
+    }
+    HEPK_REQUIRE(n == 0 || data, "data is NULL");
+    return hist_fill_launch("hepk_fill_histogram_w2", data, nullptr, weights, n, edges, nbins, nullptr, 0, sumw, sumw2,
+                            (long long*)counts, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+extern "C" int32_t hepk_fill_histogram_2d_w2(const float* x, const float* y, const float* weights, int64_t n,
+                                             const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
+                                             float* sumw, float* sumw2, int64_t* counts, void* workspace, size_t workspace_bytes,
+                                             void* stream)
+{
+    HEPK_REQUIRE(n >= 0, "n < 0");
+    HEPK_REQUIRE(edges_x && edges_y && nx >= 1 && ny >= 1, "edges are NULL or an axis has no bins");
+    if ((long long)(nx + 2) * (ny + 2) > 16384) {
+        set_error("hepk_fill_histogram_2d_w2: (nx+2)*(ny+2) = %lld exceeds 16384", (long long)(nx + 2) * (ny + 2));
+        return HEPK_ERR_UNSUPPORTED;
+    }
+    HEPK_REQUIRE(n == 0 || (x && y), "x/y is NULL");
+    return hist_fill_launch("hepk_fill_histogram_2d_w2", x, y, weights, n, edges_x, nx, edges_y, ny, sumw, sumw2,
+                            (long long*)counts, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+extern "C" int32_t hepk_event_weight_lookup(const float* w_in, const float* x, int64_t n, const float* edges, int32_t nbins,
+                                            const float* table, float* w_out, void* stream)
+{
+    HEPK_REQUIRE(n >= 0, "n < 0");
+    HEPK_REQUIRE(edges && table && nbins >= 1, "edges/table is NULL or nbins < 1");
+    if ((size_t)(2 * nbins + 1) * 4 > 200 * 1024) {
+        set_error("hepk_event_weight_lookup: %d bins do not fit 200 KB of shared memory", nbins);
+        return HEPK_ERR_UNSUPPORTED;
+    }
+    if (n == 0) return HEPK_OK;
+    HEPK_REQUIRE(x && w_out, "x/w_out is NULL");
+    const size_t smem = (size_t)(2 * nbins + 1) * 4;
+    HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::event_weight_lookup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dev::event_weight_lookup_kernel<<<grid_for_items((n + 3) / 4), 256, smem, (cudaStream_t)stream>>>(w_in, x, n, edges, nbins,
+                                                                                                    table, w_out);
+    HEPK_CUDA_TRY(cudaGetLastError());
+    return HEPK_OK;
+}

@@ -153,6 +153,8 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
     const bool has_el = d->electrons.offsets != nullptr;
     const int V = d->n_variants, W = d->n_wvar;
     const long long N = d->n_events;
+    const long long w_stride = d->weights_stride > 0 ? d->weights_stride : N;      // host rows
+    const long long o_stride = d->out_stride > 0 ? d->out_stride : N;
 
     // tables shared by every batch
     hepk_chain_desc tmpl = *d;
@@ -193,6 +195,7 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
         const long long e0 = b * p.B, e1 = (e0 + p.B < N) ? e0 + p.B : N, nb = e1 - e0;
         hepk_chain_desc bd = tmpl;
         bd.n_events = nb;
+        bd.weights_stride = 0; bd.out_stride = 0;      // the staged batch is contiguous
         auto stage_coll = [&](const hepk_collection& hc, hepk_collection& dc, size_t off_o, const size_t* col_o, int ncol) -> cudaError_t {
             const long long g0 = hc.offsets[e0], g1 = hc.offsets[e1], n = g1 - g0;
             cudaError_t e = cudaMemcpyAsync(sb + off_o, hc.offsets + e0, (size_t)(nb + 1) * 8, cudaMemcpyHostToDevice, q);
@@ -217,7 +220,7 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
         if (has_el) HEPK_CUDA_TRY(stage_coll(d->electrons, bd.electrons, p.slot.eoff, p.slot.ecol, 3));
         if (d->weights) {
             for (int w = 0; w < W; ++w)
-                HEPK_CUDA_TRY(cudaMemcpyAsync(sb + p.slot.weights + (size_t)w * nb * 4, d->weights + (size_t)w * N + e0,
+                HEPK_CUDA_TRY(cudaMemcpyAsync(sb + p.slot.weights + (size_t)w * nb * 4, d->weights + (size_t)w * w_stride + e0,
                                               (size_t)nb * 4, cudaMemcpyHostToDevice, q));
             bd.weights = (const float*)(sb + p.slot.weights);
         }
@@ -240,11 +243,11 @@ extern "C" int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t ba
         // per-event outputs: device [V][nb] -> host [V][N] at column e0, ONE strided copy per output and batch
         for (int c = 0; c < 2; ++c)
             if (out_i_host[c])
-                HEPK_CUDA_TRY(cudaMemcpy2DAsync(out_i_host[c] + e0, (size_t)N * 4, sb + p.slot.out_i[c], (size_t)nb * 4,
+                HEPK_CUDA_TRY(cudaMemcpy2DAsync(out_i_host[c] + e0, (size_t)o_stride * 4, sb + p.slot.out_i[c], (size_t)nb * 4,
                                                 (size_t)nb * 4, (size_t)V, cudaMemcpyDeviceToHost, q));
         for (int c = 0; c < 5; ++c)
             if (out_f_host[c])
-                HEPK_CUDA_TRY(cudaMemcpy2DAsync(out_f_host[c] + e0, (size_t)N * 4, sb + p.slot.out_f[c], (size_t)nb * 4,
+                HEPK_CUDA_TRY(cudaMemcpy2DAsync(out_f_host[c] + e0, (size_t)o_stride * 4, sb + p.slot.out_f[c], (size_t)nb * 4,
                                                 (size_t)nb * 4, (size_t)V, cudaMemcpyDeviceToHost, q));
         for (int v = 0; v < V; ++v) {
             if (d->out_jet_mask && bd.jets.n_objects > 0)
