@@ -294,9 +294,18 @@ def test_chain_host_streaming(hk, overlap):
         assert_exact(to_np(out["hist_counts"]), 2 * ref["hist_counts"])
 
 
-def test_chain_full_size_config2_sampled(hk):
-    """BASELINE.json config 2 at full size (10 M events) in the launch configuration bench.py times:
-    per-event outputs on sampled event ranges the oracle recomputes, histogram counts over ALL events."""
+BENCH_OUTPUTS = ("njet", "ht", "maxpt", "argmax", "mjj")       # what bench.py asks for (the common-shape build)
+
+
+def _oracle_full(wl):
+    """The oracle over ALL events of a full-size workload, on every host core (the all-cores leg is pinned to the
+    single-thread checker in tests/test_oracle_weights.py: per-event outputs and counts identical, sums in tolerance)."""
+    return hepo.analysis_chain(wl, want_mask=False, threads=0)
+
+
+def test_chain_full_size_config2_generic_build(hk):
+    """BASELINE.json config 2 at full size (10 M events), all seven per-event outputs (the GENERIC kernel build):
+    per-event outputs on sampled event ranges the single-thread oracle recomputes, histograms over ALL events."""
     wl = hepgen.generate(2)
     inp = hk.upload(wl)
     plan = hk.ChainPlan(inp)
@@ -315,6 +324,61 @@ def test_chain_full_size_config2_sampled(hk):
         sw, ct = plan.hist_view(name)
         assert to_np(ct).sum() == N
         assert abs(to_np(sw).astype(np.float64).sum() - tot) <= 1e-5 * tot
+
+
+def _compare_all_events(out, ref, names):
+    for k in names:
+        if k in ("ht", "mjj"):
+            assert_tol(to_np(out[k]), ref[k], k)
+        else:
+            assert_exact(to_np(out[k]), ref[k], k)
+
+
+def test_chain_full_size_config2_bench_launch(hk):
+    """Config 2, 10 M events, in the launch configuration bench.py times (its five outputs: the common-shape build):
+    EVERY per-event output of EVERY event against the oracle, histogram counts exact, weighted bins in tolerance."""
+    wl = hepgen.generate(2)
+    ref = _oracle_full(wl)
+    plan = hk.ChainPlan(hk.upload(wl), want_event_outputs=BENCH_OUTPUTS)
+    plan.run()
+    torch.cuda.synchronize()
+    _compare_all_events(plan.out, ref, BENCH_OUTPUTS)
+    assert_exact(to_np(plan.out["hist_counts"]), ref["hist_counts"])
+    assert_tol(to_np(plan.out["hist_sumw"]), ref["hist_sumw"])
+
+
+def test_chain_full_size_config3(hk):
+    """BASELINE.json config 3 at full size: 10 M events x 5 calibration variants, bench.py's launch configuration."""
+    wl = hepgen.generate(3)
+    ref = _oracle_full(wl)
+    plan = hk.ChainPlan(hk.upload(wl), want_event_outputs=BENCH_OUTPUTS)
+    plan.run()
+    torch.cuda.synchronize()
+    _compare_all_events(plan.out, ref, BENCH_OUTPUTS)
+    assert_exact(to_np(plan.out["hist_counts"]), ref["hist_counts"])
+    assert_tol(to_np(plan.out["hist_sumw"]), ref["hist_sumw"])
+    e0 = 7_000_000                      # and a range through the single-thread checker
+    chk = hepo.analysis_chain(wl, e0, e0 + 100_000, want_mask=False)
+    for k in ("njet", "argmax", "maxpt"):
+        assert_exact(to_np(plan.out[k][:, e0:e0 + 100_000]), chk[k], k)
+
+
+@pytest.mark.parametrize("group", [0, 5])
+def test_chain_full_size_config4_batch(hk, group):
+    """One batch of BASELINE.json config 4 at full size: 5 M events, 300 weighted histograms, histograms only
+    (bench.py's launch configuration).  Every CTA sees ~34 k events, so the hot bins cross the overflow threshold of
+    the privatised bins many times and are moved out while other warps keep filling (group = 5: all variants in one
+    launch, the 33,660-bin layout; 0: the automatic variant groups)."""
+    wl = hepgen.generate(4)
+    ref = _oracle_full(wl)
+    plan = hk.ChainPlan(hk.upload(wl), want_event_outputs=False, tune=dict(variants_per_pass=group) if group else None)
+    plan.run()
+    torch.cuda.synchronize()
+    assert_exact(to_np(plan.out["hist_counts"]), ref["hist_counts"])
+    assert_tol(to_np(plan.out["hist_sumw"]), ref["hist_sumw"])
+    plan.run()                          # accumulates
+    torch.cuda.synchronize()
+    assert_exact(to_np(plan.out["hist_counts"]), 2 * ref["hist_counts"])
 
 
 # ---------------------------------------------------------------------------------------------- SURVEY.md 8(f-2)
@@ -349,19 +413,20 @@ def test_chain_event_weight_lookup_and_sumw2(hk, cfg, n):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("kind", ["outlier", "mixed_sign", "one_bin", "tiny_and_huge"])
+@pytest.mark.parametrize("kind", ["outlier", "mixed_sign", "one_bin", "one_bin_1M", "tiny_and_huge"])
 def test_chain_weight_dynamic_range(hk, kind):
     """Weighted bins with a dynamic range inside one launch: the fixed-point bins are only used when the
     weights span at most a factor 8; every case must stay within the tolerance of the float64 oracle."""
-    wl = hepgen.generate(2, n_events=150_001)
+    wl = hepgen.generate(2, n_events=1_000_003 if kind == "one_bin_1M" else 150_001)
     rng = np.random.default_rng(11)
     w = wl.weights.copy()
     if kind == "outlier":
         w[0, 12345] = 2000.0                                   # one large generator weight sets max|w|
     elif kind == "mixed_sign":
         w[0] *= rng.choice(np.float32([-1.0, 1.0]), w.shape[1], p=[0.1, 0.9])
-    elif kind == "one_bin":
+    elif kind in ("one_bin", "one_bin_1M"):
         wl.jets.pt[:] = 25.0                                   # no clean jets: every event lands in the first HT bin
+        # (1 M events: ~6.8 k entries per CTA in one fixed-point bin, moved out several times before 2^31)
     elif kind == "tiny_and_huge":
         w[0] *= np.float32(10.0) ** rng.integers(-3, 4, w.shape[1]).astype(np.float32)
     wl.weights = np.ascontiguousarray(w, dtype=np.float32)
