@@ -17,7 +17,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-__all__ = ["CONFIGS", "Workload", "Collection", "generate", "hist_axes", "calibration_table",
+__all__ = ["CONFIGS", "Workload", "Collection", "generate", "concat", "hist_axes", "calibration_table",
            "OBSERVABLES"]
 
 # Fixed observable order used by the fused chain on both sides (names only; no arithmetic here).
@@ -150,3 +150,24 @@ def generate(config: int, n_events: int | None = None, seed: int | None = None, 
                     electrons=electrons, weights=weights, cuts=dict(CUTS), hists=tuple(cfg["hists"]),
                     axes=hist_axes(cfg["hists"]), calib=calib,
                     meta=dict(lam_jet=cfg["lam_jet"], cap_jet=cfg["cap_jet"], tail=cfg["tail"]))
+
+
+def concat(workloads) -> Workload:
+    """Several batches of one config laid end to end as ONE workload (offsets shifted, columns concatenated): the
+    host-resident input of a streamed run (BASELINE.json config 4: 10 batches of 5 M events).  Layout only."""
+    first = workloads[0]
+
+    def cat(get):
+        cols = [get(w) for w in workloads]
+        if cols[0] is None:
+            return None
+        offs, base = [cols[0].offsets], int(cols[0].offsets[-1])
+        for c in cols[1:]:
+            offs.append(c.offsets[1:] + base)
+            base += int(c.offsets[-1])
+        return Collection(np.concatenate(offs), *(np.concatenate([getattr(c, k) for c in cols]) for k in ("pt", "eta", "phi", "mass")))
+
+    return Workload(config=first.config, n_events=sum(w.n_events for w in workloads), seed=first.seed, batch=first.batch,
+                    jets=cat(lambda w: w.jets), muons=cat(lambda w: w.muons), electrons=cat(lambda w: w.electrons),
+                    weights=np.ascontiguousarray(np.concatenate([w.weights for w in workloads], axis=1)), cuts=dict(first.cuts),
+                    hists=first.hists, axes=first.axes, calib=first.calib, meta=dict(first.meta))

@@ -227,6 +227,7 @@ typedef struct hepk_chain_desc {
     int32_t tune_warps_per_cta;  /* warps (each owning its own tiles and staging region) per CTA, at most 24 */
     int32_t tune_warps_per_sm;   /* resident warps per SM the launch aims for (default 20) */
     int32_t tune_variants_per_pass; /* variants per kernel launch (default: all, fewer when the histograms crowd out the warps) */
+    int32_t tune_generic_build;  /* != 0: never take the build specialised for the common output shape */
 } hepk_chain_desc;
 
 /* `d` is a HOST pointer to a descriptor whose array pointers are DEVICE pointers.  `workspace` is a
@@ -362,9 +363,17 @@ int32_t hepk_validate_offsets(const int64_t* offsets, int64_t n_events, int64_t 
  * pair on its launch stream directly around the fused chain kernel (at most 4096 launches are kept).
  * hepk_profile_end() waits for the recorded events, stores the summed kernel time in milliseconds in
  * *total_ms (HOST pointer) and the number of timed launches in *n_launches (HOST pointer; either may be
- * NULL), and switches the recording off.  Not thread-safe; one profiling session per process at a time. */
+ * NULL), and switches the recording off.  One profiling session per process at a time (the event table is
+ * guarded by a mutex; launches from several host threads are all recorded into it). */
 int32_t hepk_profile_begin(void);
 int32_t hepk_profile_end(double* total_ms, int32_t* n_launches);
+/* Measurement hook (no part of the method): the rate of native shared-memory integer atomics on this device,
+ * red.shared.add.s32 to pseudo-random addresses among `nbins` words by `warps_per_sm` warps on every SM, in
+ * lane-atomics per second over the whole device (the bound of histogram-heavy chain launches; bench.py).
+ * `scratch`: device buffer of at least 4 bytes per SM.  Synchronises. */
+int32_t hepk_probe_shared_atomics(int32_t warps_per_sm, int32_t nbins, void* scratch, double* lane_atomics_per_second);
+/* Number of kernels this library has enqueued in this process so far (all entry points, all threads). */
+int64_t hepk_kernel_launches(void);
 
 #ifdef __cplusplus
 }

@@ -55,7 +55,7 @@ class ChainDesc(C.Structure):
         ("weights_stride", C.c_int64), ("out_stride", C.c_int64),
         ("tune_cap_jets", C.c_int32), ("tune_cap_leptons", C.c_int32),
         ("tune_ctas_per_sm", C.c_int32), ("tune_warps_per_cta", C.c_int32), ("tune_warps_per_sm", C.c_int32),
-        ("tune_variants_per_pass", C.c_int32),
+        ("tune_variants_per_pass", C.c_int32), ("tune_generic_build", C.c_int32),
     ]
 
 
@@ -123,6 +123,22 @@ def version():
 
 def last_error():
     return lib().hepk_last_error().decode()
+
+
+def kernel_launches():
+    """Kernels this library has enqueued in this process so far."""
+    L = lib()
+    L.hepk_kernel_launches.restype = C.c_int64
+    return int(L.hepk_kernel_launches())
+
+
+def probe_shared_atomics(warps_per_sm=16, nbins=32768):
+    """Measured red.shared.add.s32 rate of the device (lane-atomics per second, random addresses)."""
+    scratch = torch.zeros(4096, dtype=torch.int32, device="cuda")
+    r = C.c_double(0.0)
+    _check(lib().hepk_probe_shared_atomics(C.c_int32(warps_per_sm), C.c_int32(nbins), C.c_void_p(scratch.data_ptr()), C.byref(r)),
+           "probe_shared_atomics")
+    return r.value
 
 
 def profile_begin():

@@ -1,6 +1,9 @@
 // hepk_api.cu — error reporting, device queries, version.
 #include <stdarg.h>
 
+#include <atomic>
+#include <mutex>
+
 #include "hepk_common.cuh"
 
 namespace hepk {
@@ -40,6 +43,10 @@ static DevInfo& devinfo()
 }
 
 // ---- optional device-side timing of the dominant kernel (hepk_profile_begin / hepk_profile_end) -------------
+static std::atomic<long long> g_launches{0};
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+static std::mutex g_prof_mutex;      // the event table is shared by every thread that launches the chain
 static const int PROF_MAX = 4096;
 static bool g_prof_on = false;
 static int g_prof_n = 0;
@@ -48,6 +55,7 @@ static bool g_prof_created = false;
 
 void profile_mark(cudaStream_t st, int which)
 {
+    std::lock_guard<std::mutex> lock(g_prof_mutex);
     if (!g_prof_on || g_prof_n >= PROF_MAX) return;
     cudaEventRecord(g_prof_ev[g_prof_n][which], st);
     if (which == 1) g_prof_n++;
@@ -58,9 +66,12 @@ int max_smem_optin() { return devinfo().smem_optin; }
 
 }  // namespace hepk
 
+extern "C" int64_t hepk_kernel_launches(void) { return hepk::g_launches.load(std::memory_order_relaxed); }
+
 extern "C" int32_t hepk_profile_begin(void)
 {
     using namespace hepk;
+    std::lock_guard<std::mutex> lock(g_prof_mutex);
     if (!g_prof_created) {
         for (int i = 0; i < PROF_MAX; ++i)
             for (int k = 0; k < 2; ++k) HEPK_CUDA_TRY(cudaEventCreate(&g_prof_ev[i][k]));
@@ -74,6 +85,7 @@ extern "C" int32_t hepk_profile_begin(void)
 extern "C" int32_t hepk_profile_end(double* total_ms, int32_t* n_launches)
 {
     using namespace hepk;
+    std::lock_guard<std::mutex> lock(g_prof_mutex);
     g_prof_on = false;
     double tot = 0.0;
     for (int i = 0; i < g_prof_n; ++i) {

@@ -1495,7 +1495,7 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (P.evw_table) feat_host |= dev::F_EVW;
     if (d->weights) feat_host |= dev::F_WEIGHTS;
     if (P.W > 1) feat_host |= dev::F_MULTIW;
-    const bool common = (int)feat_host == FEAT_COMMON && !d->out_jet_mask && has_el;
+    const bool common = (int)feat_host == FEAT_COMMON && !d->out_jet_mask && has_el && !d->tune_generic_build;
 #define HEPK_PICK_COMMON(MAXT) (calib ? dev::chain_kernel<true, true, MAXT, FEAT_COMMON> : dev::chain_kernel<false, true, MAXT, FEAT_COMMON>)
     // several weight columns and few warps (large histograms): a build that keeps the event's weights in registers
     const bool multiw = P.W > 1 && d->weights && wpc <= 16;
@@ -1525,15 +1525,15 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         if (blocks > 4 * sm_count()) blocks = 4 * sm_count();
         if (blocks < 1) blocks = 1;
         dev::chain_weight_range_kernel<<<(unsigned)blocks, 256, 0, st>>>(d->weights, P.n_events, P.w_stride, P.W, d->evw_table,
-                                                                         d->evw_nbins, P.hist_hdr);
+                                                                         d->evw_nbins, P.hist_hdr); count_launch();
         HEPK_CUDA_TRY(cudaGetLastError());
     }
     profile_mark(st, 0);
-    kern<<<(unsigned)grid, wpc * 32, smem, st>>>(P);
+    kern<<<(unsigned)grid, wpc * 32, smem, st>>>(P); count_launch();
     profile_mark(st, 1);
     HEPK_CUDA_TRY(cudaGetLastError());
     if (want_hist) {
-        dev::chain_finalize_hist<<<(unsigned)((n_words + 255) / 256), 256, 0, st>>>(P);
+        dev::chain_finalize_hist<<<(unsigned)((n_words + 255) / 256), 256, 0, st>>>(P); count_launch();
         HEPK_CUDA_TRY(cudaGetLastError());
     }
     return HEPK_OK;

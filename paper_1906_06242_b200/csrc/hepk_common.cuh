@@ -18,6 +18,7 @@ int32_t cuda_fail(cudaError_t e, const char* what);
 int sm_count();                 // SMs of the current device (cached per device)
 int max_smem_optin();           // max opt-in dynamic shared memory per CTA
 void profile_mark(cudaStream_t st, int which);   // no-op unless hepk_profile_begin() is active (which: 0 before, 1 after)
+void count_launch();            // one more kernel of this library enqueued (hepk_kernel_launches)
 
 #define HEPK_CUDA_TRY(call)                                         \
     do {                                                            \

@@ -213,6 +213,23 @@ __global__ void __launch_bounds__(256) event_weight_lookup_kernel(const float* _
     }
 }
 
+// measurement hook: lane-atomics of red.shared.add.s32 per launch, random addresses in `nbins` words
+__global__ void probe_shared_atomics_kernel(int iters, int nbins, unsigned int* out)
+{
+    extern __shared__ unsigned int h[];
+    for (int i = threadIdx.x; i < nbins; i += blockDim.x) h[i] = 0u;
+    __syncthreads();
+    const uint32_t base = smem_u32(h);
+    unsigned int x = threadIdx.x * 2654435761u + blockIdx.x * 97u + 12345u;
+    for (int i = 0; i < iters; ++i) {
+        x = x * 1664525u + 1013904223u;
+        const unsigned int idx = (x >> 8) % (unsigned)nbins;
+        asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(base + 4u * idx), "r"(1) : "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) out[blockIdx.x] = h[0];
+}
+
 }  // namespace dev
 
 static unsigned grid_for_items(long long items)
@@ -265,7 +282,7 @@ static int32_t hist_fill_launch(const char* who, const float* x, const float* y,
     if (weights && P.fixed_allowed) {
         static const unsigned int inf_bits = 0x7f800000u;
         HEPK_CUDA_TRY(cudaMemcpyAsync((unsigned int*)workspace + dev::HH_WMIN, &inf_bits, 4, cudaMemcpyHostToDevice, st));
-        dev::hist_weight_range_kernel<<<grid_for_items((n + 7) / 8), 256, 0, st>>>(weights, n, (unsigned int*)workspace);
+        dev::hist_weight_range_kernel<<<grid_for_items((n + 7) / 8), 256, 0, st>>>(weights, n, (unsigned int*)workspace); count_launch();
         HEPK_CUDA_TRY(cudaGetLastError());
     }
     const bool vec = aligned16(x) && (!y || aligned16(y)) && (!weights || aligned16(weights));
@@ -277,9 +294,9 @@ static int32_t hist_fill_launch(const char* who, const float* x, const float* y,
     const long long items = (n + 1023) / 1024;
     if (grid > items) grid = items;
     if (grid < 1) grid = 1;
-    kern<<<(unsigned)grid, 256, smem, st>>>(P);
+    kern<<<(unsigned)grid, 256, smem, st>>>(P); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
-    dev::hist_finalize_kernel<<<(unsigned)((h.slots + 255) / 256), 256, 0, st>>>(P);
+    dev::hist_finalize_kernel<<<(unsigned)((h.slots + 255) / 256), 256, 0, st>>>(P); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -340,7 +357,29 @@ extern "C" int32_t hepk_event_weight_lookup(const float* w_in, const float* x, i
     const size_t smem = (size_t)(2 * nbins + 1) * 4;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::event_weight_lookup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dev::event_weight_lookup_kernel<<<grid_for_items((n + 3) / 4), 256, smem, (cudaStream_t)stream>>>(w_in, x, n, edges, nbins,
-                                                                                                    table, w_out);
+                                                                                                    table, w_out); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
+    return HEPK_OK;
+}
+
+extern "C" int32_t hepk_probe_shared_atomics(int32_t warps_per_sm, int32_t nbins, void* scratch, double* lane_atomics_per_second)
+{
+    HEPK_REQUIRE(warps_per_sm >= 1 && warps_per_sm <= 32 && nbins >= 32 && nbins <= 32768, "warps 1..32, bins 32..32768");
+    HEPK_REQUIRE(scratch && lane_atomics_per_second, "scratch/result is NULL");
+    auto kern = dev::probe_shared_atomics_kernel;
+    HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, nbins * 4));
+    const int iters = 20000, grid = sm_count();
+    cudaEvent_t a, b;
+    HEPK_CUDA_TRY(cudaEventCreate(&a));
+    HEPK_CUDA_TRY(cudaEventCreate(&b));
+    kern<<<grid, warps_per_sm * 32, nbins * 4>>>(200, nbins, (unsigned int*)scratch); count_launch();
+    cudaEventRecord(a);
+    kern<<<grid, warps_per_sm * 32, nbins * 4>>>(iters, nbins, (unsigned int*)scratch); count_launch();
+    cudaEventRecord(b);
+    HEPK_CUDA_TRY(cudaEventSynchronize(b));
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    *lane_atomics_per_second = (double)iters * warps_per_sm * 32 * grid / ((double)ms * 1e-3);
     return HEPK_OK;
 }

@@ -570,14 +570,14 @@ static int32_t segreduce_dispatch(const float* data, const int64_t* offsets, int
         long long blocks = (warps + 7) / 8;
         const long long maxb = (long long)sm_count() * 32;
         if (blocks > maxb) blocks = maxb;
-        kern<<<(unsigned)blocks, 256, 0, st>>>(data, (const long long*)offsets, n_events, base, mask_rows, mask_content, (T*)out);
+        kern<<<(unsigned)blocks, 256, 0, st>>>(data, (const long long*)offsets, n_events, base, mask_rows, mask_content, (T*)out); count_launch();
     } else {
         constexpr int TILE = 128;
         const int cap = 2560;
         auto kern = dev::segreduce_tile_kernel<OP, TILE>;
         const size_t smem = 16 + ((TILE + 1) * 4 + 15) / 16 * 16 + (size_t)cap * 4 + cap + 16;
         const int grid = persistent_grid((const void*)kern, TILE, smem, (n_events + TILE - 1) / TILE);
-        kern<<<grid, TILE, smem, st>>>(data, (const long long*)offsets, n_events, base, mask_rows, mask_content, (T*)out, cap);
+        kern<<<grid, TILE, smem, st>>>(data, (const long long*)offsets, n_events, base, mask_rows, mask_content, (T*)out, cap); count_launch();
     }
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
@@ -597,12 +597,12 @@ extern "C" int32_t hepk_select_mask(const float* pt, const float* eta, int64_t n
     if (aligned16(pt) && aligned16(out_mask) && (!eta || aligned16(eta))) {
         const long long groups = (n + 15) / 16;
         dev::select_mask_vec<<<(unsigned)((groups + 255) / 256), 256, 0, st>>>((const float4*)pt, (const float4*)eta, n, pt_min,
-                                                                               abs_eta_max, (uint4*)out_mask);
+                                                                               abs_eta_max, (uint4*)out_mask); count_launch();
     } else {
         long long blocks = (n + 255) / 256;
         const long long maxb = (long long)sm_count() * 16;
         if (blocks > maxb) blocks = maxb;
-        dev::select_mask_scalar<<<(unsigned)blocks, 256, 0, st>>>(pt, eta, n, pt_min, abs_eta_max, out_mask);
+        dev::select_mask_scalar<<<(unsigned)blocks, 256, 0, st>>>(pt, eta, n, pt_min, abs_eta_max, out_mask); count_launch();
     }
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
@@ -626,7 +626,7 @@ extern "C" int32_t hepk_lookup_binned(const float* x, const float* y, int64_t n,
     auto kern = vec ? dev::lookup_kernel<true> : dev::lookup_kernel<false>;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int grid = persistent_grid((const void*)kern, 256, smem, (n + 1023) / 1024);
-    kern<<<grid, 256, smem, st>>>(x, y, n, edges_x, nx, edges_y, ny, table, out);
+    kern<<<grid, 256, smem, st>>>(x, y, n, edges_x, nx, edges_y, ny, table, out); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -648,7 +648,7 @@ extern "C" int32_t hepk_fill_histogram(const float* data, const float* weights, 
     auto kern = vec ? dev::fill_hist_kernel<true> : dev::fill_hist_kernel<false>;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int grid = persistent_grid((const void*)kern, 256, smem, (n + 1023) / 1024);
-    kern<<<grid, 256, smem, st>>>(data, weights, n, edges, nbins, sumw, (unsigned long long*)counts);
+    kern<<<grid, 256, smem, st>>>(data, weights, n, edges, nbins, sumw, (unsigned long long*)counts); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -683,7 +683,7 @@ extern "C" int32_t hepk_deltar_mask(const float* eta1, const float* phi1, const 
     const float dr2_max = dr_max * dr_max;      // float32 product (exact class)
     kern<<<grid, TILE, smem, (cudaStream_t)stream>>>(eta1, phi1, (const long long*)offsets1, base1, sel1, eta2, phi2,
                                                      (const long long*)offsets2, base2, sel2, n_events, dr2_max,
-                                                     out_matched, cap1, cap2);
+                                                     out_matched, cap1, cap2); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -702,7 +702,7 @@ extern "C" int32_t hepk_pair_invmass(const float* pt, const float* eta, const fl
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int grid = persistent_grid((const void*)kern, TILE, smem, (n_events + TILE - 1) / TILE);
     kern<<<grid, TILE, smem, (cudaStream_t)stream>>>(pt, eta, phi, mass, (const long long*)offsets, n_events, content_base,
-                                                     mask_content, out_mass, out_i1, out_i2, cap);
+                                                     mask_content, out_mass, out_i1, out_i2, cap); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }

@@ -110,7 +110,7 @@ extern "C" int32_t hepk_get_in_offsets(const float* data, const int64_t* offsets
     if (n_events == 0) return HEPK_OK;
     HEPK_REQUIRE(offsets && out, "offsets/out is NULL");
     dev::get_in_offsets_kernel<<<grid_for(n_events), 256, 0, (cudaStream_t)stream>>>(
-        data, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, index, fill, out);
+        data, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, index, fill, out); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -124,7 +124,7 @@ extern "C" int32_t hepk_set_in_offsets(float* data, const int64_t* offsets, int6
     if (n_events == 0) return HEPK_OK;
     HEPK_REQUIRE(offsets, "offsets is NULL");
     dev::set_in_offsets_kernel<<<grid_for(n_events), 256, 0, (cudaStream_t)stream>>>(
-        data, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, index, values, value);
+        data, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, index, values, value); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -137,7 +137,7 @@ extern "C" int32_t hepk_select_opposite_sign(const float* pt, const int32_t* cha
     if (n_events == 0) return HEPK_OK;
     HEPK_REQUIRE(offsets && charge && out_mask, "offsets/charge/out_mask is NULL");
     dev::select_opposite_sign_kernel<<<grid_for(n_events), 256, 0, (cudaStream_t)stream>>>(
-        pt, charge, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, out_mask);
+        pt, charge, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, out_mask); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -240,7 +240,7 @@ extern "C" int32_t hepk_lookup_interp(const float* x, int64_t n, const float* xs
     HEPK_REQUIRE(x && out, "x/out is NULL");
     const size_t smem = (size_t)nk * 8;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::lookup_interp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dev::lookup_interp_kernel<<<grid_for(n), 256, smem, (cudaStream_t)stream>>>(x, n, xs, ys, nk, out);
+    dev::lookup_interp_kernel<<<grid_for(n), 256, smem, (cudaStream_t)stream>>>(x, n, xs, ys, nk, out); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -274,10 +274,10 @@ extern "C" int32_t hepk_fill_histogram_2d(const float* x, const float* y, const 
     if (sumw) HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)slots * sizeof(double), st));
     unsigned grid = grid_for((n + 3) / 4);
     dev::fill_hist2d_kernel<<<grid, 256, smem, st>>>(x, y, weights, n, edges_x, nx, edges_y, ny, sumw ? (double*)workspace : nullptr,
-                                                     (unsigned long long*)counts);
+                                                     (unsigned long long*)counts); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     if (sumw) {
-        dev::hist2d_finalize<<<(unsigned)((slots + 255) / 256), 256, 0, st>>>(sumw, (const double*)workspace, (int)slots);
+        dev::hist2d_finalize<<<(unsigned)((slots + 255) / 256), 256, 0, st>>>(sumw, (const double*)workspace, (int)slots); count_launch();
         HEPK_CUDA_TRY(cudaGetLastError());
     }
     return HEPK_OK;
@@ -424,7 +424,7 @@ extern "C" int32_t hepk_triplet_mass(const float* pt, const float* eta, const fl
     const long long maxb = (long long)sm_count() * 12;
     if (blocks > maxb) blocks = maxb;
     dev::triplet_kernel<<<(unsigned)blocks, 32 * dev::TRIPLET_WARPS, 0, (cudaStream_t)stream>>>(
-        pt, eta, phi, mass, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, target, out_mass, out_idx);
+        pt, eta, phi, mass, (const long long*)offsets, n_events, content_base, mask_rows, mask_content, target, out_mass, out_idx); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -456,7 +456,7 @@ extern "C" int32_t hepk_validate_offsets(const int64_t* offsets, int64_t n_event
     cudaStream_t st = (cudaStream_t)stream;
     HEPK_CUDA_TRY(cudaMemsetAsync(n_bad, 0, sizeof(int64_t), st));
     dev::validate_offsets_kernel<<<grid_for(n_events), 256, 0, st>>>((const long long*)offsets, n_events, content_base, n_objects,
-                                                                    (unsigned long long*)n_bad);
+                                                                    (unsigned long long*)n_bad); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
