@@ -52,6 +52,7 @@ struct ChainParams {
     int n_col;                      // NCOL, or 0 when the staged path is disabled
     int sh_add[NCOL];               // (col_mis - content_base) mod 4: shift = (lo32(offsets[e0]) + sh_add) & 3
     int col_stride[3];              // bytes between the staging buffers of consecutive columns of a collection
+    int col_n32[3];                 // valid elements per collection (the staged path requires them to fit an int)
     const long long* off[3];        // offsets arrays: jets, muons, electrons (electrons nullptr if absent)
     long long jn;
     const float *jpt, *jeta, *jphi, *jmass; long long jbase;
@@ -255,7 +256,9 @@ __device__ __forceinline__ int find_bin_fast(float v, uint32_t edges_a, int n, u
         }
         return lo;
     }
-    const float pos = mode == 1.0f ? v : __log2f(v);
+    float lg;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(v));      // a guess: denormals flush to -inf and clamp to bin 0, where they belong
+    const float pos = mode == 1.0f ? v : lg;
     int g = (int)((pos - lds_f32(axis_a + 4u)) * lds_f32(axis_a + 8u));       // NaN -> 0, +-inf saturate
     g = max(0, min(g, n - 1));
     const float a = lds_f32(edges_a + 4u * (unsigned)g), b = lds_f32(edges_a + 4u * (unsigned)g + 4u);
@@ -740,7 +743,7 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
         const int sh = (l0 + P.col_mis[c0]) & 3;
         a0[k] = l0 - sh;
         const int ln = (cnt[k] + sh + 3) & ~3;
-        ok = ok && (cnt[k] == 0 || ((unsigned)cnt[k] <= (unsigned)P.col_cap[c0] && (a0[k] | ((int)P.col_n[c0] - a0[k] - ln)) >= 0));
+        ok = ok && (cnt[k] == 0 || ((unsigned)cnt[k] <= (unsigned)P.col_cap[c0] && (a0[k] | (P.col_n32[k] - a0[k] - ln)) >= 0));
         len[k] = cnt[k] != 0 ? ln : 0;
         total += (uint32_t)len[k] * (k == 0 ? 16u : 12u);
     }
@@ -870,10 +873,12 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     const long long n_static = dyn ? (long long)per_cta * gridDim.x : P.n_tiles;
     const long long cta_lo = (long long)blockIdx.x * per_cta;
     const uint32_t next_a = smem_u32(S.next);
+    unsigned int ticket = 0;          // of the tile taken last: also picks the slice of bins this warp checks next
     auto take_tile = [&]() -> long long {
         unsigned int i = 0;
         if (lane == 0) i = atom_add_shared_u32(next_a, 1u);
         i = __shfl_sync(0xffffffffu, i, 0);
+        ticket = i;
         if (i < per_cta) return cta_lo + i < P.n_tiles ? cta_lo + i : P.n_tiles;
         if (!dyn) return P.n_tiles;
         unsigned int g = 0;
@@ -1169,9 +1174,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
 
         if (P.hist_acc) {
             // every finished tile checks one slice of the CTA's bins for values about to leave the int32 range
-            unsigned int t = 0;
-            if (lane == 0) t = atom_add_shared_u32(smem_u32(S.scan), 1u);
-            t = __shfl_sync(0xffffffffu, t, 0) % SCAN_SLICES;
+            const unsigned int t = ticket % SCAN_SLICES;      // tickets are consecutive: 32 finished tiles cover all slices
             const int n = P.obs_prefix[HEPK_N_OBS] * P.V * P.WS;
             const int len = (n + SCAN_SLICES - 1) / SCAN_SLICES;
             const int i0 = (int)t * len;
@@ -1444,6 +1447,12 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         const int first = P.col_coll[c] == 0 ? 0 : (P.col_coll[c] == 1 ? 4 : 7);
         if (P.col_ptr[c] && P.col_ptr[first] && P.col_mis[c] != P.col_mis[first]) P.n_col = 0;
     }
+    // the staged path indexes with 32-bit object counts
+    const long long big = 0x7fffffffll - 64;
+    if (d->jets.n_objects > big || d->muons.n_objects > big || (has_el && d->electrons.n_objects > big)) P.n_col = 0;
+    P.col_n32[0] = (int)(d->jets.n_objects > big ? big : d->jets.n_objects);
+    P.col_n32[1] = (int)(d->muons.n_objects > big ? big : d->muons.n_objects);
+    P.col_n32[2] = has_el ? (int)(d->electrons.n_objects > big ? big : d->electrons.n_objects) : 0;
 
     // CTA shape: as many warps per SM as shared memory allows (up to 20), in as few CTAs as possible so that
     // the privatised histograms are shared by many warps
