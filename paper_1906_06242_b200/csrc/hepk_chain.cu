@@ -132,6 +132,7 @@ __host__ __device__ inline size_t chain_shared_layout(const ChainParams& P, bool
     return align_up(o, 128);
 }
 
+// [profile phase: shared-memory / atomic helpers]
 // ---- shared-memory atomics in the shared state space (no generic-address dispatch) ----------------------
 __device__ __forceinline__ unsigned int atom_add_shared_u32(uint32_t addr, unsigned int v)
 {
@@ -215,6 +216,7 @@ __device__ __forceinline__ float sqrt_approx(float x)
     return r;
 }
 
+// [profile phase: histogram slot]
 // Histogram slot (0 underflow, 1+b, nbins+1 overflow/NaN).  inv != 0 means the kernel has verified at start-up
 // that |(edges[i] - lo) * inv - i| <= 0.5 for every edge; the same monotone float32 expression applied to x then
 // lands within one bin of the right one, and a single +-1 step against the edges makes the result exact.
@@ -239,6 +241,7 @@ __device__ __forceinline__ int slot_lean(float x, uint32_t edges_a, int nb, floa
     return (x != x) ? nb + 1 : s;
 }
 
+// [profile phase: calibration bin]
 // B(v) of the lookup tables (clamped bin, include/hepk.h hepk_lookup_binned) without a search: for an axis the
 // kernel has verified at start-up to be uniform in v (mode 1) or in log2 v (mode 2) to within 0.45 bins, the
 // arithmetic guess lands within one bin of the right one (the log2 approximation is good to 1e-5 bins), and one
@@ -268,6 +271,7 @@ __device__ __forceinline__ int find_bin_fast(float v, uint32_t edges_a, int n, u
     return (v != v) ? n - 1 : g;
 }
 
+// [profile phase: dR^2]
 // dR^2, exact class.  Same value as dr2_exact: with a = |dphi| and t = a - 2PI_F, the wrapped magnitude is
 // min(a, |t|): a > PI_F  =>  |t| <= PI_F < a (rn is monotone), a < PI_F  =>  |t| >= PI_F > a, and at a == PI_F
 // both are PI_F.  Three instructions for the wrap instead of four (|.| is a free operand modifier).
@@ -305,6 +309,7 @@ __device__ __forceinline__ float dr2_packed(float2 jet, float2 lep)
     return r;
 }
 
+// [profile phase: pair mass]
 // pair_mass_fast (hepk_common.cuh) with the hardware approximations (ex2, rcp, sqrt: 1-2 ulp each) in place of
 // the library calls; tolerance class, every term of M^2 >= 0, ~60 instructions.
 __device__ __forceinline__ float pair_mass_lean(float pt1, float eta1, float phi1, float m1,
@@ -346,6 +351,7 @@ __device__ __forceinline__ float pair_mass_lean(float pt1, float eta1, float phi
     return sqrt_approx(fmaxf(msq, 0.0f));
 }
 
+// [profile phase: feature word]
 // What the launch asked for, as one register of flags (tested with one instruction instead of a pointer compare).
 enum : unsigned {
     F_NJET = 1u << 0, F_ARGMAX = 1u << 1, F_HT = 1u << 2, F_MAXPT = 1u << 3, F_MINPT = 1u << 4, F_MJJ = 1u << 5,
@@ -374,6 +380,7 @@ __device__ __forceinline__ unsigned chain_features(const ChainParams& P)
     return f;
 }
 
+// [profile phase: histogram fill]
 // Slot of one observable: bumps its count and returns the shared-memory address of its bin in weight column 0
 // (0 when the observable is not histogrammed).  sumw layout [v][o][w][nbins_o + 2].
 // Shared-memory address of the slot row (all columns of one slot) of observable OB for value x; 0: not histogrammed.
@@ -439,6 +446,7 @@ __device__ __forceinline__ void add_weights(const ChainParams& P, unsigned feat,
     }
 }
 
+// [profile phase: finish_event: outputs, slots, fills]
 // Per event and variant: leading-pair mass, outputs, histograms.  Shared by the staged path and the per-event
 // path.  The leading jets' (eta, phi, mass) are passed in by value; i2 < 0 means fewer than two clean jets.
 template <int NW>
@@ -491,6 +499,7 @@ __device__ __forceinline__ void finish_event(const ChainParams& P, const ChainSh
     else add_weights<false, NW>(P, feat, row, wt, ev, evf, 0.0f, 0.0f);
 }
 
+// [profile phase: per-event reduction state (push)]
 // Order-preserving map float -> unsigned (and back): a < b  <=>  ord_key(a) < ord_key(b); no finite value maps to 0.
 __device__ __forceinline__ unsigned int ord_key(float f)
 {
@@ -583,6 +592,7 @@ struct EventAcc {
     }
 };
 
+// [profile phase: histogram scales]
 // Fixed-point scales of the weighted bins (R18) from the weight range in the workspace header: entries are
 // rint(w * 2^k) with |w| * 2^k < 2^19 (2^k2 likewise for w^2).  A bin is checked at least every ~1024 events of the
 // CTA plus the tiles in flight and moved out at 2^29, so it stays below 2^31.  The rounding error per entry is
@@ -607,6 +617,7 @@ __device__ __forceinline__ void hist_scales(const ChainParams& P, float& sc, flo
     sc2 = ldexpf(1.0f, k2);
 }
 
+// [profile phase: event-weight factor]
 // Per-event weight factor table[B(x)] (hepk_lookup_binned's clamped bin, 1-D) from the staged lookup.
 __device__ __forceinline__ float evw_factor(const ChainParams& P, const ChainShared& S, long long ev)
 {
@@ -627,6 +638,7 @@ __device__ __forceinline__ float evw_factor(const ChainParams& P, const ChainSha
     return lds_f32(smem_u32(S.evw_table) + 4u * (unsigned)b);
 }
 
+// [profile phase: per-event fallback path]
 // dR match of one jet against one lepton collection of event `ev`, straight from global memory.
 __device__ inline bool match_global(const ChainParams& P, float eta, float phi, const long long* off, long long base,
                                     const float* lpt, const float* leta, const float* lphi, long long ev)
@@ -681,6 +693,7 @@ __device__ __noinline__ void chain_event_global(const ChainParams& P, unsigned c
     }
 }
 
+// [profile phase: histogram flush]
 // Move privatised bins [i0, i1) of the CTA into the global accumulators (thread t of nt).  Safe against concurrent
 // fills by other warps: a bin is taken with an atomic exchange.  Fixed-point and count columns are exact integers,
 // so they only move when `all` is set or the bin is about to leave the int32 range (|bin| >= FLUSH_AT); float bins
@@ -705,6 +718,7 @@ __device__ __forceinline__ void flush_bins(const ChainParams& P, const ChainShar
     }
 }
 
+// [profile phase: offsets load]
 // Low words of offsets[e] and offsets[e+1] of the lane's event (lane = event of the tile), three collections.
 struct EventOffsets { int j0, j1, m0, m1, q0, q1; };
 
@@ -720,6 +734,7 @@ __device__ __forceinline__ void load_event_offsets(const ChainParams& P, long lo
     else { o.q0 = 0; o.q1 = 0; }
 }
 
+// [profile phase: TMA issue]
 // Start the bulk copies of a tile whose slices start at global element lo[k] and hold cnt[k] elements (k: jets, muons,
 // electrons) into the warp's staging region; all 32 lanes call it, converged, with the same arguments in every lane.
 // Returns false (nothing issued) when a slice does not fit: capacity, 16-byte alignment at the array ends.
@@ -766,6 +781,7 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
     return true;
 }
 
+// [profile phase: kernel setup]
 // NW: weight columns of an event kept in registers (1, or HEPK_MAX_WVAR for launches with several columns)
 template <bool CALIB, bool HAS_EL, int MAXT, int FEAT, int NW = 1>
 __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ ChainParams P)
@@ -864,6 +880,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     // so everything it does not ask for is compiled out
     const unsigned feat = FEAT >= 0 ? (unsigned)FEAT : chain_features(P);
 
+    // [profile phase: tile hand-out, prefetch of offsets and weights]
     // Tile hand-out.  Every CTA owns a contiguous range of tiles and its warps draw from it through a shared-memory
     // ticket, so a scheduler with one warp more than its neighbours (or a warp that met long events) simply takes
     // fewer tiles; the last eighth of the launch is handed out by a global counter so that no SM idles at the end.
@@ -930,6 +947,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         fit = false;
 
         if (staged) {
+            // [profile phase: phase 0: tile geometry, buckets]
             // ---- phase 0: one lane per event.  Offsets are in registers.
             const int jb = __shfl_sync(0xffffffffu, eo.j0, 0);
             const int mb = __shfl_sync(0xffffffffu, eo.m0, 0);
@@ -963,6 +981,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             mbar_wait(bar, parity);
             parity ^= 1u;
             if (staged) {
+                // [profile phase: phase 0: lepton list]
                 // combined (eta, phi) list of the event: muons then electrons; eta = +inf marks "not selected"
                 // (deta^2 = inf, so dR^2 = inf or NaN and the minimum below ignores it).  Straight-line predicated
                 // code for the first few leptons of each kind (a divergent loop costs more than the work it does).
@@ -999,6 +1018,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     }
                 }
                 if (c & 1) sts_v2(out + 8u * (unsigned)c, CUDART_INF_F, 0.0f);     // pad entry
+                // [profile phase: phase 0: permutation]
                 __syncwarp();       // bucket totals complete
                 const int4 t0 = lds_v4i(bk), t1 = lds_v4i(bk + 16);
                 int base = 0;
@@ -1025,6 +1045,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                 }
                 __syncwarp();
 
+                // [profile phase: phase 1: dR and cuts (lane = jet)]
                 // ---- phase 1: one lane per jet, in bucket order (neighbouring lanes: same lepton count)
                 const uint32_t aend1 = order_a + 4u * (unsigned)njt;
 #pragma unroll 1
@@ -1052,6 +1073,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     }
                 }
                 __syncwarp();
+                // [profile phase: jet mask output]
                 if (P.out_jet_mask) {
                     // clean-jet mask, jets in their original order (coalesced bytes), from the verdicts just stored
                     const long long lj0 = __ldg(P.off[0] + e0) - P.jbase;
@@ -1068,6 +1090,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     }
                 }
 
+                // [profile phase: phase 2: per-event reductions (lane = event)]
                 // ---- phase 2: one lane per event (lanes past the last event run with nj = 0)
                 const uint32_t a_ev = a_jpt + 4u * (unsigned)kj0;
                 const uint32_t d_corr = d_corr0;
@@ -1134,6 +1157,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                             }
                         }
                     }
+                    // [profile phase: phase 2: leading pair, release, next TMA issue]
                     float e1 = 0, p1 = 0, m1 = 0, e2 = 0, p2 = 0, m2 = 0;
                     if (a.i2 >= 0) {
                         const uint32_t x = a_ev + 4u * (unsigned)a.i1, y = a_ev + 4u * (unsigned)a.i2;
@@ -1151,12 +1175,14 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         }
                         released = true;
                     }
+                    // [profile phase: finish_event call]
                     if (live)
                         finish_event<NW>(P, S, feat, e0 + lane, v, wt, evf, a.cnt, (float)a.sum, a.mn, a.b1, a.b2, a.i1, a.i2, e1, p1, m1, e2, p2, m2);
                 }
             }
             bsel ^= 1;
         }
+        // [profile phase: tile epilogue, overflow scan]
         if (!released) {
             fence_proxy_async_smem();
             __syncwarp();
@@ -1181,6 +1207,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
             flush_bins(P, S, i0, i0 + len < n ? i0 + len : n, lane, 32, false);
         }
     }
+    // [profile phase: final flush]
     __syncthreads();
     if (P.hist_acc) flush_bins(P, S, 0, P.obs_prefix[HEPK_N_OBS] * P.V * P.WS, tid, nthr, true);
 }
