@@ -734,6 +734,14 @@ __device__ __forceinline__ void load_event_offsets(const ChainParams& P, long lo
     else { o.q0 = 0; o.q1 = 0; }
 }
 
+// one lane of the (converged) warp
+__device__ __forceinline__ bool elect_one()
+{
+    unsigned int pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0u;
+}
+
 // [profile phase: TMA issue]
 // Start the bulk copies of a tile whose slices start at global element lo[k] and hold cnt[k] elements (k: jets, muons,
 // electrons) into the warp's staging region; all 32 lanes call it, converged, with the same arguments in every lane.
@@ -748,7 +756,7 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
 {
     int a0[3];
     int len[3];
-    bool ok = true;
+    int bad = 0;
     uint32_t total = 0;
 #pragma unroll
     for (int k = 0; k < (HAS_EL ? 3 : 2); ++k) {
@@ -758,12 +766,17 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
         const int sh = (l0 + P.col_mis[c0]) & 3;
         a0[k] = l0 - sh;
         const int ln = (cnt[k] + sh + 3) & ~3;
-        ok = ok && (cnt[k] == 0 || ((unsigned)cnt[k] <= (unsigned)P.col_cap[c0] && (a0[k] | (P.col_n32[k] - a0[k] - ln)) >= 0));
+        // fits: 0 <= cnt <= capacity and 0 <= a0, a0 + ln <= n (an empty slice always fits).  Sign bits, no branches.
+        const int e0k = cnt[k] != 0 ? a0[k] : 0;
         len[k] = cnt[k] != 0 ? ln : 0;
+        bad |= cnt[k] | (P.col_cap[c0] - cnt[k]) | e0k | (P.col_n32[k] - e0k - len[k]);
         total += (uint32_t)len[k] * (k == 0 ? 16u : 12u);
     }
-    if (!ok) return false;
-    if (lane == 0) {
+    if (bad < 0) return false;
+    // One elected lane issues all copies.  Under elect.sync (and with operands that come from warp reductions, hence
+    // uniform registers) each copy is one UBLKCP; under `lane == 0` the compiler wraps every copy in a loop over the
+    // lanes that might be active.
+    if (elect_one()) {
         uint64_t* bar = nullptr;
         const uint32_t bar_a = region_a;
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_a), "r"(total) : "memory");
@@ -790,7 +803,7 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     ChainShared S;
     chain_shared_layout(P, CALIB, smem_raw, &S);
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // through a shuffle: the compiler then knows it is warp-uniform
+    const int warp = __reduce_min_sync(0xffffffffu, tid >> 5);  // through a warp reduction: its result lives in a uniform register, and so does every address derived from it
     const int lane = tid & 31, nwarp = nthr >> 5;
     unsigned char* R = smem_raw + P.shared_bytes + (size_t)warp * P.region_bytes;   // this warp's staging region
     uint64_t* bar = (uint64_t*)R;
@@ -894,13 +907,13 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     auto take_tile = [&]() -> long long {
         unsigned int i = 0;
         if (lane == 0) i = atom_add_shared_u32(next_a, 1u);
-        i = __shfl_sync(0xffffffffu, i, 0);
+        i = __reduce_max_sync(0xffffffffu, i);      // lane 0's value, in a uniform register
         ticket = i;
         if (i < per_cta) return cta_lo + i < P.n_tiles ? cta_lo + i : P.n_tiles;
         if (!dyn) return P.n_tiles;
         unsigned int g = 0;
         if (lane == 0) g = atom_add_global_u32(P.tile_counter, 1u);
-        return n_static + (long long)__shfl_sync(0xffffffffu, g, 0);
+        return n_static + (long long)__reduce_max_sync(0xffffffffu, g);
     };
     long long tile = take_tile();
     uint32_t parity = 0;
@@ -910,13 +923,15 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     eo.j0 = eo.j1 = eo.m0 = eo.m1 = eo.q0 = eo.q1 = 0;
     // object counts of a tile from the per-lane offsets (lanes past the last event hold offsets[n_events])
     auto tile_counts = [&](const EventOffsets& o, int (&lo)[3], int (&cnt)[3]) {
-        lo[0] = __shfl_sync(0xffffffffu, o.j0, 0); cnt[0] = __shfl_sync(0xffffffffu, o.j1, 31) - lo[0];
-        lo[1] = __shfl_sync(0xffffffffu, o.m0, 0); cnt[1] = __shfl_sync(0xffffffffu, o.m1, 31) - lo[1];
-        lo[2] = HAS_EL ? __shfl_sync(0xffffffffu, o.q0, 0) : 0;
-        cnt[2] = HAS_EL ? __shfl_sync(0xffffffffu, o.q1, 31) - lo[2] : 0;
+        // offsets do not decrease: lane 0 holds the smallest start, lane 31 the largest end.  Warp reductions rather
+        // than shuffles: their results are uniform registers, so the slice arithmetic runs on the uniform datapath
+        lo[0] = __reduce_min_sync(0xffffffffu, o.j0); cnt[0] = __reduce_max_sync(0xffffffffu, o.j1) - lo[0];
+        lo[1] = __reduce_min_sync(0xffffffffu, o.m0); cnt[1] = __reduce_max_sync(0xffffffffu, o.m1) - lo[1];
+        lo[2] = HAS_EL ? __reduce_min_sync(0xffffffffu, o.q0) : 0;
+        cnt[2] = HAS_EL ? __reduce_max_sync(0xffffffffu, o.q1) - lo[2] : 0;
     };
+    int lo[3] = {0, 0, 0}, cnt[3] = {0, 0, 0};      // first object and object count of the current tile's slices (uniform)
     if (tile < P.n_tiles) {
-        int lo[3], cnt[3];
         load_event_offsets<HAS_EL>(P, tile, lane, eo);
         tile_counts(eo, lo, cnt);
         fit = P.n_col > 0 && issue_tile<HAS_EL>(P, smem_u32(R), lane, lo, cnt);
@@ -945,14 +960,13 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         bool staged = fit;
         bool released = false;
         fit = false;
+        int nlo[3] = {0, 0, 0}, ncnt[3] = {0, 0, 0};                    // the same for the next tile
 
         if (staged) {
             // [profile phase: phase 0: tile geometry, buckets]
             // ---- phase 0: one lane per event.  Offsets are in registers.
-            const int jb = __shfl_sync(0xffffffffu, eo.j0, 0);
-            const int mb = __shfl_sync(0xffffffffu, eo.m0, 0);
-            const int qb = __shfl_sync(0xffffffffu, eo.q0, 0);
-            const int njt = __shfl_sync(0xffffffffu, eo.j1, ne - 1) - jb;
+            const int jb = lo[0], mb = lo[1], qb = lo[2];
+            const int njt = cnt[0];
             // shared-memory byte addresses; the columns of one collection share alignment and sit STRIDE apart
             const uint32_t a_jpt = region_a + (uint32_t)P.col_dst[0] + 4u * (unsigned)((jb + P.sh_add[0]) & 3);
             const uint32_t a_mpt = region_a + (uint32_t)P.col_dst[4] + 4u * (unsigned)((mb + P.sh_add[4]) & 3);
@@ -985,7 +999,10 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                 // combined (eta, phi) list of the event: muons then electrons; eta = +inf marks "not selected"
                 // (deta^2 = inf, so dR^2 = inf or NaN and the minimum below ignores it).  Straight-line predicated
                 // code for the first few leptons of each kind (a divergent loop costs more than the work it does).
-                const uint32_t out = lep_a + 8u * (unsigned)l0;      // (l0 <= MAX_LIST by the capacities)
+                uint32_t out = lep_a + 8u * (unsigned)l0;            // (l0 <= MAX_LIST by the capacities)
+                float lep_pt_min = P.lep_pt_min;
+                // pinned in registers: the predicated blocks below would otherwise each recompute the address and reload the cut
+                asm volatile("" : "+r"(out), "+f"(lep_pt_min));
                 {
                     const uint32_t a = a_mpt + 4u * (unsigned)km0;
                     constexpr int UNR_M = 5;
@@ -993,12 +1010,12 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     for (int k = 0; k < UNR_M; ++k)
                         if (k < nm) {
                             const float pt = lds_f32(a + 4u * k), eta = lds_f32(a + ms + 4u * k), phi = lds_f32(a + 2 * ms + 4u * k);
-                            sts_v2(out + 8u * k, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                            sts_v2(out + 8u * k, pt > lep_pt_min ? eta : CUDART_INF_F, phi);
                         }
 #pragma unroll 1
                     for (int k = UNR_M; k < nm; ++k) {
                         const float pt = lds_f32(a + 4u * k), eta = lds_f32(a + ms + 4u * k), phi = lds_f32(a + 2 * ms + 4u * k);
-                        sts_v2(out + 8u * k, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                        sts_v2(out + 8u * k, pt > lep_pt_min ? eta : CUDART_INF_F, phi);
                     }
                 }
                 if (HAS_EL) {
@@ -1009,12 +1026,12 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                     for (int k = 0; k < UNR_E; ++k)
                         if (k < nq) {
                             const float pt = lds_f32(a + 4u * k), eta = lds_f32(a + es + 4u * k), phi = lds_f32(a + 2 * es + 4u * k);
-                            sts_v2(oe + 8u * k, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                            sts_v2(oe + 8u * k, pt > lep_pt_min ? eta : CUDART_INF_F, phi);
                         }
 #pragma unroll 1
                     for (int k = UNR_E; k < nq; ++k) {
                         const float pt = lds_f32(a + 4u * k), eta = lds_f32(a + es + 4u * k), phi = lds_f32(a + 2 * es + 4u * k);
-                        sts_v2(oe + 8u * k, pt > P.lep_pt_min ? eta : CUDART_INF_F, phi);
+                        sts_v2(oe + 8u * k, pt > lep_pt_min ? eta : CUDART_INF_F, phi);
                     }
                 }
                 if (c & 1) sts_v2(out + 8u * (unsigned)c, CUDART_INF_F, 0.0f);     // pad entry
@@ -1049,23 +1066,41 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                 // ---- phase 1: one lane per jet, in bucket order (neighbouring lanes: same lepton count)
                 const uint32_t aend1 = order_a + 4u * (unsigned)njt;
 #pragma unroll 1
+                // the column bases are uniform registers (they derive from warp reductions), so a jet's three loads and
+                // its store address as [offset + uniform base] without any per-jet address arithmetic
+                const uint32_t u_jpt = __reduce_min_sync(0xffffffffu, a_jpt), u_jeta = __reduce_min_sync(0xffffffffu, a_jpt + js),
+                               u_jphi = __reduce_min_sync(0xffffffffu, a_jpt + 2 * js);
                 for (uint32_t ao = order_a + 4u * lane; ao < aend1; ao += 128) {
                     const unsigned int word = lds_u32(ao);
-                    const uint32_t aj = a_jpt + (word & 0x7ffu);
-                    const float pt = lds_f32(aj), eta = lds_f32(aj + js), phi = lds_f32(aj + 2 * js);
-                    uint32_t al = lep_a + ((word >> 11) & 0x1fffu);
+                    const uint32_t oj = word & 0x7ffu;
+                    const uint32_t aj = u_jpt + oj;
+                    const float pt = lds_f32(u_jpt + oj), eta = lds_f32(u_jeta + oj), phi = lds_f32(u_jphi + oj);
+                    uint32_t al = (word >> 11) & 0x1fffu;
                     const uint32_t alend = al + (word >> 24);
                     float dmin = CUDART_INF_F;
 #pragma unroll 1
                     for (; al != alend; al += 16) {
-                        const float4 l = lds_v4(al);
+                        const float4 l = lds_v4(lep_a + al);
                         dmin = fminf(dmin, fminf(dr2_packed(make_float2(eta, phi), make_float2(l.x, l.y)),
                                                  dr2_packed(make_float2(eta, phi), make_float2(l.z, l.w))));
                     }
-                    const bool base_ok = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
                     if (!CALIB) {
-                        sts_f32(aj, (base_ok && (pt > P.jet_pt_min)) ? pt : -CUDART_INF_F);
+                        // pt if (pt > pt_min && |eta| < eta_max && !(dmin < dr2_max)) else -inf: one chained predicate
+                        float r;
+                        asm("{\n\t"
+                            ".reg .pred p;\n\t"
+                            ".reg .f32 ae;\n\t"
+                            "abs.f32 ae, %2;\n\t"
+                            "setp.gt.f32 p, %1, %4;\n\t"
+                            "setp.lt.and.f32 p, ae, %5, p;\n\t"
+                            "setp.geu.and.f32 p, %3, %6, p;\n\t"
+                            "selp.f32 %0, %1, 0fFF800000, p;\n\t"
+                            "}"
+                            : "=f"(r)
+                            : "f"(pt), "f"(eta), "f"(dmin), "f"(P.jet_pt_min), "f"(P.jet_abs_eta_max), "f"(P.dr2_max));
+                        sts_f32(aj, r);
                     } else {
+                        const bool base_ok = (fabsf(eta) < P.jet_abs_eta_max) && !(dmin < P.dr2_max);
                         const int bx = find_bin_fast(pt, smem_u32(S.cal_pt_edges), P.cal_npt, smem_u32(S.cal_axis));
                         const int by = find_bin_fast(eta, smem_u32(S.cal_eta_edges), P.cal_neta, smem_u32(S.cal_axis) + 16u);
                         sts_f32(aj + d_corr0, lds_f32(smem_u32(S.cal_table) + 4u * (unsigned)(bx * P.cal_neta + by)));
@@ -1168,10 +1203,9 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                         // the staging region is dead from here: start the next tile's copies under the finishing math
                         fence_proxy_async_smem();
                         __syncwarp();
-                        if (has_next && P.n_col > 0) {
-                            int nlo[3], ncnt[3];
+                        if (has_next) {
                             tile_counts(neo, nlo, ncnt);
-                            fit = issue_tile<HAS_EL>(P, region_a, lane, nlo, ncnt);
+                            fit = P.n_col > 0 && issue_tile<HAS_EL>(P, region_a, lane, nlo, ncnt);
                         }
                         released = true;
                     }
@@ -1186,15 +1220,16 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         if (!released) {
             fence_proxy_async_smem();
             __syncwarp();
-            if (has_next && P.n_col > 0) {
-                int nlo[3], ncnt[3];
+            if (has_next) {
                 tile_counts(neo, nlo, ncnt);
-                fit = issue_tile<HAS_EL>(P, smem_u32(R), lane, nlo, ncnt);
+                fit = P.n_col > 0 && issue_tile<HAS_EL>(P, smem_u32(R), lane, nlo, ncnt);
             }
         }
         if (!staged && lane < ne) chain_event_global<CALIB>(P, smem_raw, e0 + lane);
         __syncwarp();
         eo = neo;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { lo[k] = nlo[k]; cnt[k] = ncnt[k]; }
         tile = tile_next;
         tile_next = take_tile();
 
