@@ -726,8 +726,11 @@ template <bool HAS_EL>
 __device__ __forceinline__ void load_event_offsets(const ChainParams& P, long long tile, int lane, EventOffsets& o)
 {
     const long long e = tile * TILE_EVENTS + lane;
-    const long long i0 = e < P.n_events ? e : P.n_events;
-    const long long i1 = e + 1 < P.n_events ? e + 1 : P.n_events;
+    long long i0 = e, i1 = e + 1;
+    if ((tile + 1) * TILE_EVENTS > P.n_events) {        // only the last tile can be ragged (uniform branch)
+        i0 = e < P.n_events ? e : P.n_events;
+        i1 = e + 1 < P.n_events ? e + 1 : P.n_events;
+    }
     o.j0 = (int)__ldg(P.off[0] + i0); o.j1 = (int)__ldg(P.off[0] + i1);
     o.m0 = (int)__ldg(P.off[1] + i0); o.m1 = (int)__ldg(P.off[1] + i1);
     if (HAS_EL) { o.q0 = (int)__ldg(P.off[2] + i0); o.q1 = (int)__ldg(P.off[2] + i1); }
@@ -898,24 +901,26 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
     // ticket, so a scheduler with one warp more than its neighbours (or a warp that met long events) simply takes
     // fewer tiles; the last eighth of the launch is handed out by a global counter so that no SM idles at the end.
     const bool dyn = P.tile_counter != nullptr;
-    const unsigned int per_cta = dyn ? (unsigned int)((P.n_tiles - P.n_tiles / 8) / gridDim.x)
-                                     : (unsigned int)((P.n_tiles + gridDim.x - 1) / gridDim.x);
-    const long long n_static = dyn ? (long long)per_cta * gridDim.x : P.n_tiles;
-    const long long cta_lo = (long long)blockIdx.x * per_cta;
+    // (tile indices fit 32 bits: the host refuses launches of 2^31 tiles or more)
+    const unsigned int NT = (unsigned int)P.n_tiles;
+    const unsigned int per_cta = dyn ? (NT - NT / 8u) / gridDim.x : (NT + gridDim.x - 1u) / gridDim.x;
+    const unsigned int n_static = dyn ? per_cta * gridDim.x : NT;
+    const unsigned int cta_lo = blockIdx.x * per_cta;
     const uint32_t next_a = smem_u32(S.next);
     unsigned int ticket = 0;          // of the tile taken last: also picks the slice of bins this warp checks next
-    auto take_tile = [&]() -> long long {
+    auto take_tile = [&]() -> unsigned int {
         unsigned int i = 0;
-        if (lane == 0) i = atom_add_shared_u32(next_a, 1u);
-        i = __reduce_max_sync(0xffffffffu, i);      // lane 0's value, in a uniform register
+        if (elect_one()) i = atom_add_shared_u32(next_a, 1u);
+        i = __reduce_max_sync(0xffffffffu, i);      // the elected lane's value, in a uniform register
         ticket = i;
-        if (i < per_cta) return cta_lo + i < P.n_tiles ? cta_lo + i : P.n_tiles;
-        if (!dyn) return P.n_tiles;
+        if (i < per_cta) return min(cta_lo + i, NT);
+        if (!dyn) return NT;
         unsigned int g = 0;
-        if (lane == 0) g = atom_add_global_u32(P.tile_counter, 1u);
-        return n_static + (long long)__reduce_max_sync(0xffffffffu, g);
+        if (elect_one()) g = atom_add_global_u32(P.tile_counter, 1u);
+        g = __reduce_max_sync(0xffffffffu, g);
+        return g < NT - n_static ? n_static + g : NT;
     };
-    long long tile = take_tile();
+    unsigned int tile = take_tile();
     uint32_t parity = 0;
     int bsel = 0;
     bool fit = false;
@@ -931,19 +936,19 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
         cnt[2] = HAS_EL ? __reduce_max_sync(0xffffffffu, o.q1) - lo[2] : 0;
     };
     int lo[3] = {0, 0, 0}, cnt[3] = {0, 0, 0};      // first object and object count of the current tile's slices (uniform)
-    if (tile < P.n_tiles) {
+    if (tile < NT) {
         load_event_offsets<HAS_EL>(P, tile, lane, eo);
         tile_counts(eo, lo, cnt);
         fit = P.n_col > 0 && issue_tile<HAS_EL>(P, smem_u32(R), lane, lo, cnt);
     }
 
-    long long tile_next = take_tile();
+    unsigned int tile_next = take_tile();
 
-    for (; tile < P.n_tiles;) {
-        const long long e0 = tile * TILE_EVENTS;
+    for (; tile < NT;) {
+        const long long e0 = (long long)tile * TILE_EVENTS;
         const long long rest = P.n_events - e0;
         const int ne = rest < TILE_EVENTS ? (int)rest : TILE_EVENTS;
-        const bool has_next = tile_next < P.n_tiles;
+        const bool has_next = tile_next < NT;
         float wt[NW];                                                    // weights of the lane's event, loaded early
         float evf = 1.0f;                                                // its weight factor from the lookup
         if ((feat & F_EVW) && (feat & (F_SUMW | F_SUMW2)) && lane < ne) evf = evw_factor(P, S, e0 + lane);
@@ -1420,6 +1425,11 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     memset(&P, 0, sizeof(P));
     P.n_events = d->n_events;
     P.n_tiles = (d->n_events + TILE_EVENTS - 1) / TILE_EVENTS;
+    if (P.n_tiles >= (1ll << 31)) {          // the kernel indexes tiles with 32 bits (the offsets alone would be > 500 GB)
+        if (plan_warps) return HEPK_OK;
+        set_error("hepk_analysis_chain: n_events = %lld is beyond the 2^36 a launch supports", (long long)d->n_events);
+        return HEPK_ERR_UNSUPPORTED;
+    }
     P.w_stride = d->weights_stride > 0 ? d->weights_stride : d->n_events;
     P.out_stride = d->out_stride > 0 ? d->out_stride : d->n_events;
     P.off[0] = (const long long*)d->jets.offsets;

@@ -1,7 +1,5 @@
-// hepk_kernels.cu — the single kernels of include/hepk.h:
-//   select_mask, lookup_binned, fill_histogram           (flat, 128-bit vectorised streaming)
-//   segmented_reduce_{sum,max,min,count,argmax}          (warp-per-event and block-per-tile variants)
-//   deltar_mask, pair_invmass                            (tiles of events staged through shared memory)
+// hepk_kernels.cu — the flat single kernels of include/hepk.h: select_mask, lookup_binned, fill_histogram
+// (128-bit vectorised streaming).  The kernels that walk jagged collections are in hepk_tiles.cu.
 #include <string.h>
 
 #include "hepk_common.cuh"
@@ -158,388 +156,6 @@ __global__ void __launch_bounds__(256) fill_hist_kernel(const float* __restrict_
     flush();
 }
 
-// =========================================================================================== segmented reductions
-enum { OP_SUM = 0, OP_MAX = 1, OP_MIN = 2, OP_COUNT = 3, OP_ARGMAX = 4 };
-
-template <int OP> struct OutT { typedef float type; };
-template <> struct OutT<OP_COUNT> { typedef int type; };
-template <> struct OutT<OP_ARGMAX> { typedef int type; };
-
-// Running state of one reduction.  push() follows the oracle's update rules; merge() combines partial
-// states so that count / max / min / argmax do not depend on the order of combination.
-template <int OP>
-struct Acc {
-    float v;
-    int i;
-    __device__ __forceinline__ void init()
-    {
-        v = OP == OP_MAX ? -CUDART_INF_F : (OP == OP_MIN ? CUDART_INF_F : 0.f);
-        i = OP == OP_ARGMAX ? -1 : 0;
-    }
-    __device__ __forceinline__ void push(float x, int k)
-    {
-        if (OP == OP_SUM) v += x;
-        else if (OP == OP_COUNT) i += 1;
-        else if (OP == OP_MAX) { if (x > v) v = x; }
-        else if (OP == OP_MIN) { if (x < v) v = x; }
-        else { if (x == x && (i < 0 || x > v)) { v = x; i = k; } }     // k ascending within a thread
-    }
-    __device__ __forceinline__ void merge(float ov, int oi)
-    {
-        if (OP == OP_SUM) v += ov;
-        else if (OP == OP_COUNT) i += oi;
-        else if (OP == OP_MAX) { if (ov > v) v = ov; }
-        else if (OP == OP_MIN) { if (ov < v) v = ov; }
-        else { if (oi >= 0 && (i < 0 || ov > v || (ov == v && oi < i))) { v = ov; i = oi; } }
-    }
-    __device__ __forceinline__ typename OutT<OP>::type result() const
-    {
-        if (OP == OP_COUNT || OP == OP_ARGMAX) return (typename OutT<OP>::type)i;
-        return (typename OutT<OP>::type)v;
-    }
-    __device__ __forceinline__ void warp_reduce()
-    {
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            const float ov = __shfl_xor_sync(0xffffffffu, v, d);
-            const int oi = __shfl_xor_sync(0xffffffffu, i, d);
-            merge(ov, oi);
-        }
-    }
-};
-
-// Variant 1: one warp per event, lanes stride over the event's particles (coalesced), shuffle reduction.
-template <int OP>
-__global__ void __launch_bounds__(256) segreduce_warp_kernel(const float* __restrict__ data, const long long* __restrict__ offsets,
-                                                             long long n_events, long long base,
-                                                             const unsigned char* __restrict__ mask_rows,
-                                                             const unsigned char* __restrict__ mask_content,
-                                                             typename OutT<OP>::type* __restrict__ out)
-{
-    const int lane = threadIdx.x & 31;
-    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long e = warp0; e < n_events; e += nwarps) {
-        Acc<OP> acc;
-        acc.init();
-        if (!mask_rows || mask_rows[e]) {
-            const long long g0 = offsets[e], g1 = offsets[e + 1];
-            for (long long g = g0 + lane; g < g1; g += 32) {
-                const long long i = g - base;
-                if (mask_content && !mask_content[i]) continue;
-                acc.push(OP == OP_COUNT ? 0.f : data[i], (int)(g - g0));
-            }
-        }
-        acc.warp_reduce();
-        if (lane == 0) out[e] = acc.result();
-    }
-}
-
-// Variant 2: a tile of TILE events per step; the tile's data (and content-mask) slice is staged into shared
-// memory by bulk copies, then one thread reduces one event; outputs are written coalesced.
-template <int OP, int TILE>
-__global__ void __launch_bounds__(TILE) segreduce_tile_kernel(const float* __restrict__ data, const long long* __restrict__ offsets,
-                                                              long long n_events, long long base,
-                                                              const unsigned char* __restrict__ mask_rows,
-                                                              const unsigned char* __restrict__ mask_content,
-                                                              typename OutT<OP>::type* __restrict__ out, int cap)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint64_t* bar = (uint64_t*)smem_raw;
-    int* loc = (int*)(smem_raw + 16);
-    float* s_data = (float*)(smem_raw + 16 + ((TILE + 1) * 4 + 15) / 16 * 16);
-    unsigned char* s_mask = (unsigned char*)(s_data + cap);
-    __shared__ float red_v[TILE / 32];
-    __shared__ int red_i[TILE / 32];
-    const int tid = threadIdx.x;
-    const bool need_data = OP != OP_COUNT;
-    if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
-    __syncthreads();
-    uint32_t parity = 0;
-    const long long n_total = offsets[n_events] - base;
-    const long long n_tiles = (n_events + TILE - 1) / TILE;
-    const int capm = cap - 40;
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const long long e0 = tile * TILE;
-        const int ne = (int)((n_events - e0) < TILE ? (n_events - e0) : TILE);
-        const long long gb = offsets[e0];
-        for (int i = tid; i <= ne; i += TILE) loc[i] = (int)(offsets[e0 + i] - gb);
-        __syncthreads();
-        int ev0 = 0;
-        while (ev0 < ne) {
-            const int b = loc[ev0];
-            int n_fit;
-            if (loc[ne] - b <= capm) n_fit = ne - ev0;
-            else n_fit = __syncthreads_count(tid >= ev0 && tid < ne && loc[tid + 1] - b <= capm);
-            if (n_fit == 0) {
-                // one event larger than the buffer: the whole CTA strides over it in global memory
-                const long long e = e0 + ev0;
-                Acc<OP> acc;
-                acc.init();
-                if (!mask_rows || mask_rows[e]) {
-                    const long long g0 = gb + b, g1 = gb + loc[ev0 + 1];
-                    for (long long g = g0 + tid; g < g1; g += TILE) {
-                        const long long i = g - base;
-                        if (mask_content && !mask_content[i]) continue;
-                        acc.push(need_data ? data[i] : 0.f, (int)(g - g0));
-                    }
-                }
-                acc.warp_reduce();
-                if ((tid & 31) == 0) { red_v[tid >> 5] = acc.v; red_i[tid >> 5] = acc.i; }
-                __syncthreads();
-                if (tid == 0) {
-                    Acc<OP> t;
-                    t.v = red_v[0]; t.i = red_i[0];
-                    for (int w = 1; w < TILE / 32; ++w) t.merge(red_v[w], red_i[w]);
-                    out[e] = t.result();
-                }
-                ev0 += 1;
-                __syncthreads();
-                continue;
-            }
-            const int ev1 = ev0 + n_fit;
-            const int nd = loc[ev1] - b;
-            const long long l0 = gb + b - base;
-            long long a0;
-            int sh_d = 0, sh_m = 0;
-            uint32_t bytes = 0;
-            if (tid == 0) fence_proxy_async_smem();
-            if (need_data) { bytes += stage_column(s_data, data, l0, l0 + nd, n_total, bar, tid, 0, &a0); sh_d = (int)(l0 - a0); }
-            if (mask_content) { bytes += stage_column(s_mask, mask_content, l0, l0 + nd, n_total, bar, tid, 0, &a0); sh_m = (int)(l0 - a0); }
-            if (tid == 0) mbar_arrive_expect_tx(bar, bytes);
-            mbar_wait(bar, parity);
-            parity ^= 1u;
-            __syncthreads();
-            if (tid < n_fit) {
-                const long long e = e0 + ev0 + tid;
-                Acc<OP> acc;
-                acc.init();
-                if (!mask_rows || mask_rows[e]) {
-                    const int k0 = loc[ev0 + tid] - b, k1 = loc[ev0 + tid + 1] - b;
-                    for (int k = k0; k < k1; ++k) {
-                        if (mask_content && !s_mask[k + sh_m]) continue;
-                        acc.push(need_data ? s_data[k + sh_d] : 0.f, k - k0);
-                    }
-                }
-                out[e] = acc.result();
-            }
-            fence_proxy_async_smem();
-            __syncthreads();
-            ev0 = ev1;
-        }
-    }
-}
-
-// =========================================================================================== deltar_mask
-template <int TILE>
-__global__ void __launch_bounds__(TILE) deltar_tile_kernel(const float* __restrict__ eta1, const float* __restrict__ phi1,
-                                                           const long long* __restrict__ off1, long long base1,
-                                                           const unsigned char* __restrict__ sel1,
-                                                           const float* __restrict__ eta2, const float* __restrict__ phi2,
-                                                           const long long* __restrict__ off2, long long base2,
-                                                           const unsigned char* __restrict__ sel2,
-                                                           long long n_events, float dr2_max,
-                                                           unsigned char* __restrict__ out, int cap1, int cap2)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint64_t* bar = (uint64_t*)smem_raw;
-    int* loc1 = (int*)(smem_raw + 16);
-    int* loc2 = loc1 + (TILE + 1);
-    unsigned char* p = smem_raw + 16 + (2 * (TILE + 1) * 4 + 15) / 16 * 16;
-    float* s_eta1 = (float*)p; p += (size_t)cap1 * 4;
-    float* s_phi1 = (float*)p; p += (size_t)cap1 * 4;
-    float* s_eta2 = (float*)p; p += (size_t)cap2 * 4;
-    float* s_phi2 = (float*)p; p += (size_t)cap2 * 4;
-    unsigned short* evid = (unsigned short*)p; p += (size_t)cap1 * 2;
-    unsigned char* s_sel1 = p; p += cap1;
-    unsigned char* s_sel2 = p;
-    const int tid = threadIdx.x;
-    if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
-    __syncthreads();
-    uint32_t parity = 0;
-    const long long n1 = off1[n_events] - base1, n2 = off2[n_events] - base2;
-    const long long n_tiles = (n_events + TILE - 1) / TILE;
-    const int c1 = cap1 - 40, c2 = cap2 - 40;
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const long long e0 = tile * TILE;
-        const int ne = (int)((n_events - e0) < TILE ? (n_events - e0) : TILE);
-        const long long gb1 = off1[e0], gb2 = off2[e0];
-        for (int i = tid; i <= ne; i += TILE) { loc1[i] = (int)(off1[e0 + i] - gb1); loc2[i] = (int)(off2[e0 + i] - gb2); }
-        __syncthreads();
-        int ev0 = 0;
-        while (ev0 < ne) {
-            const int b1 = loc1[ev0], b2 = loc2[ev0];
-            int n_fit;
-            if (loc1[ne] - b1 <= c1 && loc2[ne] - b2 <= c2) n_fit = ne - ev0;
-            else n_fit = __syncthreads_count(tid >= ev0 && tid < ne && loc1[tid + 1] - b1 <= c1 && loc2[tid + 1] - b2 <= c2);
-            if (n_fit == 0) {
-                // one event larger than the buffers: the CTA strides over its collection-1 objects in global memory
-                const long long g0 = gb1 + b1, g1 = gb1 + loc1[ev0 + 1];
-                const long long h0 = gb2 + b2, h1 = gb2 + loc2[ev0 + 1];
-                for (long long g = g0 + tid; g < g1; g += TILE) {
-                    const long long j = g - base1;
-                    bool matched = false;
-                    if (!sel1 || sel1[j]) {
-                        const float eta = eta1[j], phi = phi1[j];
-                        for (long long h = h0; h < h1 && !matched; ++h) {
-                            const long long m = h - base2;
-                            if (sel2 && !sel2[m]) continue;
-                            matched = dr2_exact(eta, phi, eta2[m], phi2[m]) < dr2_max;
-                        }
-                    }
-                    out[j] = matched ? 1 : 0;
-                }
-                ev0 += 1;
-                __syncthreads();
-                continue;
-            }
-            const int ev1 = ev0 + n_fit;
-            const int na = loc1[ev1] - b1, nb = loc2[ev1] - b2;
-            const long long l1 = gb1 + b1 - base1, l2 = gb2 + b2 - base2;
-            long long a0;
-            int sh_e1, sh_p1, sh_e2, sh_p2, sh_s1 = 0, sh_s2 = 0;
-            uint32_t bytes = 0;
-            if (tid == 0) fence_proxy_async_smem();
-            bytes += stage_column(s_eta1, eta1, l1, l1 + na, n1, bar, tid, 0, &a0); sh_e1 = (int)(l1 - a0);
-            bytes += stage_column(s_phi1, phi1, l1, l1 + na, n1, bar, tid, 0, &a0); sh_p1 = (int)(l1 - a0);
-            bytes += stage_column(s_eta2, eta2, l2, l2 + nb, n2, bar, tid, 0, &a0); sh_e2 = (int)(l2 - a0);
-            bytes += stage_column(s_phi2, phi2, l2, l2 + nb, n2, bar, tid, 0, &a0); sh_p2 = (int)(l2 - a0);
-            if (sel1) { bytes += stage_column(s_sel1, sel1, l1, l1 + na, n1, bar, tid, 0, &a0); sh_s1 = (int)(l1 - a0); }
-            if (sel2) { bytes += stage_column(s_sel2, sel2, l2, l2 + nb, n2, bar, tid, 0, &a0); sh_s2 = (int)(l2 - a0); }
-            if (tid == 0) mbar_arrive_expect_tx(bar, bytes);
-            if (tid < n_fit) {
-                const int k0 = loc1[ev0 + tid] - b1, k1 = loc1[ev0 + tid + 1] - b1;
-                for (int k = k0; k < k1; ++k) evid[k] = (unsigned short)tid;
-            }
-            mbar_wait(bar, parity);
-            parity ^= 1u;
-            __syncthreads();
-            if (sel2) {   // unselected objects of collection 2 never match: NaN eta
-                for (int m = tid; m < nb; m += TILE)
-                    if (!s_sel2[m + sh_s2]) s_eta2[m + sh_e2] = CUDART_NAN_F;
-                __syncthreads();
-            }
-            for (int j = tid; j < na; j += TILE) {
-                bool matched = false;
-                if (!sel1 || s_sel1[j + sh_s1]) {
-                    const float eta = s_eta1[j + sh_e1], phi = s_phi1[j + sh_p1];
-                    const int a = ev0 + (int)evid[j];
-                    const int m0 = loc2[a] - b2, m1 = loc2[a + 1] - b2;
-                    for (int m = m0; m < m1; ++m)
-                        matched |= dr2_exact(eta, phi, s_eta2[m + sh_e2], s_phi2[m + sh_p2]) < dr2_max;
-                }
-                out[l1 + j] = matched ? 1 : 0;
-            }
-            fence_proxy_async_smem();
-            __syncthreads();
-            ev0 = ev1;
-        }
-    }
-}
-
-// =========================================================================================== pair_invmass
-template <int TILE>
-__global__ void __launch_bounds__(TILE) invmass_tile_kernel(const float* __restrict__ pt, const float* __restrict__ eta,
-                                                            const float* __restrict__ phi, const float* __restrict__ mass,
-                                                            const long long* __restrict__ offsets, long long n_events, long long base,
-                                                            const unsigned char* __restrict__ mask,
-                                                            float* __restrict__ out_mass, int* __restrict__ out_i1,
-                                                            int* __restrict__ out_i2, int cap)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint64_t* bar = (uint64_t*)smem_raw;
-    int* loc = (int*)(smem_raw + 16);
-    unsigned char* p = smem_raw + 16 + ((TILE + 1) * 4 + 15) / 16 * 16;
-    float* s_pt = (float*)p; p += (size_t)cap * 4;
-    float* s_eta = (float*)p; p += (size_t)cap * 4;
-    float* s_phi = (float*)p; p += (size_t)cap * 4;
-    float* s_mass = (float*)p; p += (size_t)cap * 4;
-    unsigned char* s_mask = p;
-    const int tid = threadIdx.x;
-    if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
-    __syncthreads();
-    uint32_t parity = 0;
-    const long long n_total = offsets[n_events] - base;
-    const long long n_tiles = (n_events + TILE - 1) / TILE;
-    const int capm = cap - 40;
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const long long e0 = tile * TILE;
-        const int ne = (int)((n_events - e0) < TILE ? (n_events - e0) : TILE);
-        const long long gb = offsets[e0];
-        for (int i = tid; i <= ne; i += TILE) loc[i] = (int)(offsets[e0 + i] - gb);
-        __syncthreads();
-        int ev0 = 0;
-        while (ev0 < ne) {
-            const int b = loc[ev0];
-            int n_fit;
-            if (loc[ne] - b <= capm) n_fit = ne - ev0;
-            else n_fit = __syncthreads_count(tid >= ev0 && tid < ne && loc[tid + 1] - b <= capm);
-            if (n_fit == 0) {
-                // one event larger than the buffers: one thread, the paper's loop shape, global memory
-                if (tid == 0) {
-                    const long long e = e0 + ev0, g0 = gb + b, g1 = gb + loc[ev0 + 1];
-                    Top2 top;
-                    top.init();
-                    for (long long g = g0; g < g1; ++g) {
-                        const long long i = g - base;
-                        if (mask && !mask[i]) continue;
-                        top.push_any(pt[i], (int)(g - g0));
-                    }
-                    float m = 0.f;
-                    if (top.i2 >= 0) {
-                        const long long a = g0 - base + top.i1, c = g0 - base + top.i2;
-                        m = pair_mass_f32(top.b1, eta[a], phi[a], mass[a], top.b2, eta[c], phi[c], mass[c]);
-                    }
-                    out_mass[e] = m;
-                    if (out_i1) out_i1[e] = top.i1;
-                    if (out_i2) out_i2[e] = top.i2;
-                }
-                ev0 += 1;
-                __syncthreads();
-                continue;
-            }
-            const int ev1 = ev0 + n_fit;
-            const int nd = loc[ev1] - b;
-            const long long l0 = gb + b - base;
-            long long a0;
-            int sh_pt, sh_eta, sh_phi, sh_mass, sh_m = 0;
-            uint32_t bytes = 0;
-            if (tid == 0) fence_proxy_async_smem();
-            bytes += stage_column(s_pt, pt, l0, l0 + nd, n_total, bar, tid, 0, &a0);     sh_pt = (int)(l0 - a0);
-            bytes += stage_column(s_eta, eta, l0, l0 + nd, n_total, bar, tid, 0, &a0);   sh_eta = (int)(l0 - a0);
-            bytes += stage_column(s_phi, phi, l0, l0 + nd, n_total, bar, tid, 0, &a0);   sh_phi = (int)(l0 - a0);
-            bytes += stage_column(s_mass, mass, l0, l0 + nd, n_total, bar, tid, 0, &a0); sh_mass = (int)(l0 - a0);
-            if (mask) { bytes += stage_column(s_mask, mask, l0, l0 + nd, n_total, bar, tid, 0, &a0); sh_m = (int)(l0 - a0); }
-            if (tid == 0) mbar_arrive_expect_tx(bar, bytes);
-            mbar_wait(bar, parity);
-            parity ^= 1u;
-            __syncthreads();
-            if (tid < n_fit) {
-                const long long e = e0 + ev0 + tid;
-                const int k0 = loc[ev0 + tid] - b, k1 = loc[ev0 + tid + 1] - b;
-                Top2 top;
-                top.init();
-                for (int k = k0; k < k1; ++k) {
-                    if (mask && !s_mask[k + sh_m]) continue;
-                    top.push_any(s_pt[k + sh_pt], k - k0);
-                }
-                float m = 0.f;
-                if (top.i2 >= 0) {
-                    const int a = k0 + top.i1, c = k0 + top.i2;
-                    m = pair_mass_f32(top.b1, s_eta[a + sh_eta], s_phi[a + sh_phi], s_mass[a + sh_mass],
-                                      top.b2, s_eta[c + sh_eta], s_phi[c + sh_phi], s_mass[c + sh_mass]);
-                }
-                out_mass[e] = m;
-                if (out_i1) out_i1[e] = top.i1;
-                if (out_i2) out_i2[e] = top.i2;
-            }
-            fence_proxy_async_smem();
-            __syncthreads();
-            ev0 = ev1;
-        }
-    }
-}
-
 }  // namespace dev
 
 // ------------------------------------------------------------------------------------------ host helpers
@@ -550,37 +166,6 @@ static int persistent_grid(const void* kern, int block, size_t smem, long long w
     long long g = (long long)sm_count() * occ;
     if (g > work_items) g = work_items;
     return (int)(g < 1 ? 1 : g);
-}
-
-template <int OP>
-static int32_t segreduce_dispatch(const float* data, const int64_t* offsets, int64_t n_events, int64_t base,
-                                  const uint8_t* mask_rows, const uint8_t* mask_content, void* out, int32_t variant,
-                                  void* stream)
-{
-    typedef typename dev::OutT<OP>::type T;
-    HEPK_REQUIRE(n_events >= 0, "n_events < 0");
-    HEPK_REQUIRE(variant >= 0 && variant <= 2, "unknown variant");
-    if (n_events == 0) return HEPK_OK;
-    HEPK_REQUIRE(offsets && out, "offsets/out is NULL");
-    HEPK_REQUIRE(OP == dev::OP_COUNT || data, "data is NULL");
-    cudaStream_t st = (cudaStream_t)stream;
-    if (variant == HEPK_VARIANT_WARP_PER_EVENT) {
-        auto kern = dev::segreduce_warp_kernel<OP>;
-        const long long warps = n_events;
-        long long blocks = (warps + 7) / 8;
-        const long long maxb = (long long)sm_count() * 32;
-        if (blocks > maxb) blocks = maxb;
-        kern<<<(unsigned)blocks, 256, 0, st>>>(data, (const long long*)offsets, n_events, base, mask_rows, mask_content, (T*)out); count_launch();
-    } else {
-        constexpr int TILE = 128;
-        const int cap = 2560;
-        auto kern = dev::segreduce_tile_kernel<OP, TILE>;
-        const size_t smem = 16 + ((TILE + 1) * 4 + 15) / 16 * 16 + (size_t)cap * 4 + cap + 16;
-        const int grid = persistent_grid((const void*)kern, TILE, smem, (n_events + TILE - 1) / TILE);
-        kern<<<grid, TILE, smem, st>>>(data, (const long long*)offsets, n_events, base, mask_rows, mask_content, (T*)out, cap); count_launch();
-    }
-    HEPK_CUDA_TRY(cudaGetLastError());
-    return HEPK_OK;
 }
 
 }  // namespace hepk
@@ -649,60 +234,6 @@ extern "C" int32_t hepk_fill_histogram(const float* data, const float* weights, 
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int grid = persistent_grid((const void*)kern, 256, smem, (n + 1023) / 1024);
     kern<<<grid, 256, smem, st>>>(data, weights, n, edges, nbins, sumw, (unsigned long long*)counts); count_launch();
-    HEPK_CUDA_TRY(cudaGetLastError());
-    return HEPK_OK;
-}
-
-#define HEPK_DEFINE_SEGREDUCE(NAME, OP, T)                                                                             \
-    extern "C" int32_t hepk_segmented_reduce_##NAME(const float* data, const int64_t* offsets, int64_t n_events,       \
-                                                    int64_t content_base, const uint8_t* mask_rows,                   \
-                                                    const uint8_t* mask_content, T* out, int32_t variant, void* stream) \
-    {                                                                                                                  \
-        return segreduce_dispatch<OP>(data, offsets, n_events, content_base, mask_rows, mask_content, out, variant,    \
-                                      stream);                                                                         \
-    }
-HEPK_DEFINE_SEGREDUCE(sum, dev::OP_SUM, float)
-HEPK_DEFINE_SEGREDUCE(max, dev::OP_MAX, float)
-HEPK_DEFINE_SEGREDUCE(min, dev::OP_MIN, float)
-HEPK_DEFINE_SEGREDUCE(count, dev::OP_COUNT, int32_t)
-HEPK_DEFINE_SEGREDUCE(argmax, dev::OP_ARGMAX, int32_t)
-
-extern "C" int32_t hepk_deltar_mask(const float* eta1, const float* phi1, const int64_t* offsets1, int64_t base1, const uint8_t* sel1,
-                                    const float* eta2, const float* phi2, const int64_t* offsets2, int64_t base2, const uint8_t* sel2,
-                                    int64_t n_events, float dr_max, uint8_t* out_matched, void* stream)
-{
-    HEPK_REQUIRE(n_events >= 0, "n_events < 0");
-    if (n_events == 0) return HEPK_OK;
-    HEPK_REQUIRE(offsets1 && offsets2, "offsets is NULL");
-    constexpr int TILE = 128;
-    const int cap1 = 2560, cap2 = 1024;
-    const size_t smem = 16 + (2 * (TILE + 1) * 4 + 15) / 16 * 16 + (size_t)cap1 * (8 + 2 + 1) + (size_t)cap2 * (8 + 1) + 16;
-    auto kern = dev::deltar_tile_kernel<TILE>;
-    HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int grid = persistent_grid((const void*)kern, TILE, smem, (n_events + TILE - 1) / TILE);
-    const float dr2_max = dr_max * dr_max;      // float32 product (exact class)
-    kern<<<grid, TILE, smem, (cudaStream_t)stream>>>(eta1, phi1, (const long long*)offsets1, base1, sel1, eta2, phi2,
-                                                     (const long long*)offsets2, base2, sel2, n_events, dr2_max,
-                                                     out_matched, cap1, cap2); count_launch();
-    HEPK_CUDA_TRY(cudaGetLastError());
-    return HEPK_OK;
-}
-
-extern "C" int32_t hepk_pair_invmass(const float* pt, const float* eta, const float* phi, const float* mass,
-                                     const int64_t* offsets, int64_t n_events, int64_t content_base, const uint8_t* mask_content,
-                                     float* out_mass, int32_t* out_i1, int32_t* out_i2, void* stream)
-{
-    HEPK_REQUIRE(n_events >= 0, "n_events < 0");
-    if (n_events == 0) return HEPK_OK;
-    HEPK_REQUIRE(offsets && out_mass, "offsets/out_mass is NULL");
-    constexpr int TILE = 128;
-    const int cap = 2560;
-    const size_t smem = 16 + ((TILE + 1) * 4 + 15) / 16 * 16 + (size_t)cap * 17 + 16;
-    auto kern = dev::invmass_tile_kernel<TILE>;
-    HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int grid = persistent_grid((const void*)kern, TILE, smem, (n_events + TILE - 1) / TILE);
-    kern<<<grid, TILE, smem, (cudaStream_t)stream>>>(pt, eta, phi, mass, (const long long*)offsets, n_events, content_base,
-                                                     mask_content, out_mass, out_i1, out_i2, cap); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
