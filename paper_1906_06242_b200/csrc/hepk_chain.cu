@@ -1547,6 +1547,21 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         *plan_warps = best_total;
         return HEPK_OK;
     }
+    // Shared memory the chosen shape leaves unused goes to the jet buffers.  The capacity above is the mean + 4 sigma
+    // of a Poisson-like tile; workloads with a tail of busy events overflow it now and then, and an overflowing tile
+    // takes the per-event path, where one 40-jet event holds its warp for ~100 us (measured: a straggler SM 12 %
+    // behind the rest at the end of the launch).
+    if (d->tune_cap_jets <= 0) {
+        int budget = sm_total / best_ctas - 1024;
+        if (budget > smem_max) budget = smem_max;
+        while (cap_j + 4 <= MAX_JETS_TILE && cap_j + 4 <= 2 * round_up4(cap_for((double)d->jets.n_objects / nev, 64))) {
+            const int r = chain_region_layout(P, d, calib, cap_j + 4, cap_m, cap_e);
+            if (shared_bytes + wpc * r > budget) break;
+            cap_j += 4;
+        }
+        region = chain_region_layout(P, d, calib, cap_j, cap_m, cap_e);
+        P.region_bytes = region;
+    }
     const size_t smem = (size_t)shared_bytes + (size_t)wpc * region;
     P.tile_counter = want_hist ? P.hist_hdr + HDR_TILE : nullptr;
 
