@@ -758,7 +758,7 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
                                            const int (&cnt)[3])
 {
     int a0[3];
-    int len[3];
+    int len[3], tail[3] = {0, 0, 0};
     int bad = 0;
     uint32_t total = 0;
 #pragma unroll
@@ -769,13 +769,31 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
         const int sh = (l0 + P.col_mis[c0]) & 3;
         a0[k] = l0 - sh;
         const int ln = (cnt[k] + sh + 3) & ~3;
-        // fits: 0 <= cnt <= capacity and 0 <= a0, a0 + ln <= n (an empty slice always fits).  Sign bits, no branches.
+        // fits: 0 <= cnt <= capacity, 0 <= a0 and the slice ends inside the array (an empty slice always fits).  Sign
+        // bits, no branches.  At the very end of an array the aligned window may reach past it: the bulk copy then
+        // stops at the last full 16 bytes and the (at most three) elements beyond are moved by ordinary loads.
         const int e0k = cnt[k] != 0 ? a0[k] : 0;
         len[k] = cnt[k] != 0 ? ln : 0;
-        bad |= cnt[k] | (P.col_cap[c0] - cnt[k]) | e0k | (P.col_n32[k] - e0k - len[k]);
+        const int over = e0k + len[k] - P.col_n32[k];
+        tail[k] = 0;
+        if (over > 0) {
+            const int lb = (P.col_n32[k] - e0k) & ~3;
+            tail[k] = l0 + cnt[k] - e0k - lb;          // elements of the slice past the bulk copy (0..3)
+            len[k] = lb;
+        }
+        bad |= cnt[k] | (P.col_cap[c0] - cnt[k]) | e0k | (P.col_n32[k] - l0 - cnt[k]);
         total += (uint32_t)len[k] * (k == 0 ? 16u : 12u);
     }
     if (bad < 0) return false;
+    if ((tail[0] | tail[1] | tail[2]) != 0) {          // (uniform, rare: the last tile of a launch)
+#pragma unroll
+        for (int c = 0; c < (HAS_EL ? NCOL : 7); ++c) {
+            const int k = c < 4 ? 0 : (c < 7 ? 1 : 2);
+            if (lane < tail[k])
+                sts_f32(region_a + (uint32_t)P.col_dst[c] + 4u * (unsigned)(len[k] + lane),
+                        __ldg(reinterpret_cast<const float*>(P.col_ptr[c]) + a0[k] + len[k] + lane));
+        }
+    }
     // One elected lane issues all copies.  Under elect.sync (and with operands that come from warp reductions, hence
     // uniform registers) each copy is one UBLKCP; under `lane == 0` the compiler wraps every copy in a loop over the
     // lanes that might be active.
