@@ -1487,18 +1487,22 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     P.hist_counts = want_hist ? (long long*)d->hist_counts : nullptr;
     P.evw_x = d->evw_x; P.evw_edges = d->evw_edges; P.evw_table = d->evw_table; P.evw_nbins = d->evw_nbins;
 
-    // staging capacities per 32-event tile from the mean multiplicities: mean + ~4 sigma of a Poisson-like
-    // tile total (a tile that does not fit takes the per-event path)
+    // staging capacities per 32-event tile from the mean multiplicities: mean + k sigma of a Poisson-like tile total
+    // (a tile that does not fit takes the per-event path).  Leptons: k = 4.  Jets: k = 8, because jet multiplicities
+    // have tails (BASELINE.json configs 2-4: 1 % of the events carry 30-40 jets), a tile that overflows contains
+    // several such events, and on the per-event path one of them holds its warp for ~100 us: measured as a straggler
+    // SM 12-18 % behind the rest at the end of a launch.
     const double nev = (double)(d->n_events > 0 ? d->n_events : 1);
-    auto cap_for = [&](double mean, int floor_) {
+    auto cap_for = [&](double mean, int floor_, double k) {
         const double t = TILE_EVENTS * mean;
-        long long c = (long long)(t + 4.0 * sqrt(2.0 * t + 1.0)) + 8;
+        long long c = (long long)(t + k * sqrt(2.0 * t + 1.0)) + 8;
         return c < floor_ ? floor_ : (int)c;
     };
-    int cap_j = round_up4(d->tune_cap_jets > 0 ? d->tune_cap_jets : cap_for((double)d->jets.n_objects / nev, 64));
-    int cap_m = round_up4(d->tune_cap_leptons > 0 ? d->tune_cap_leptons : cap_for((double)d->muons.n_objects / nev, 32));
+    const int cap_j4 = round_up4(cap_for((double)d->jets.n_objects / nev, 64, 4.0));
+    int cap_j = round_up4(d->tune_cap_jets > 0 ? d->tune_cap_jets : cap_for((double)d->jets.n_objects / nev, 64, 8.0));
+    int cap_m = round_up4(d->tune_cap_leptons > 0 ? d->tune_cap_leptons : cap_for((double)d->muons.n_objects / nev, 32, 4.0));
     int cap_e = has_el ? round_up4(d->tune_cap_leptons > 0 ? d->tune_cap_leptons
-                                                              : cap_for((double)d->electrons.n_objects / nev, 32)) : 0;
+                                                              : cap_for((double)d->electrons.n_objects / nev, 32, 4.0)) : 0;
     if (cap_j < 16) cap_j = 16;
     if (cap_j > MAX_JETS_TILE) cap_j = MAX_JETS_TILE;      // the jet's byte offset is packed in 11 bits
     if (cap_m < 4) cap_m = 4;
@@ -1514,6 +1518,12 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         return HEPK_ERR_UNSUPPORTED;
     }
     int region = chain_region_layout(P, d, calib, cap_j, cap_m, cap_e);
+    // large histogram sets leave room for few warps: below 16 per SM the warps matter more than the rare overflowing
+    // tile, and the jet buffers go back to 4 sigma
+    if (d->tune_cap_jets <= 0 && (smem_max - shared_bytes) / region < 16 && cap_j > cap_j4) {
+        cap_j = cap_j4;
+        region = chain_region_layout(P, d, calib, cap_j, cap_m, cap_e);
+    }
     while (shared_bytes + region > smem_max && cap_j > 64) {      // shrink the jet buffers before giving up
         cap_j = round_up4(cap_j / 2);
         region = chain_region_layout(P, d, calib, cap_j, cap_m, cap_e);
@@ -1565,14 +1575,11 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
         *plan_warps = best_total;
         return HEPK_OK;
     }
-    // Shared memory the chosen shape leaves unused goes to the jet buffers.  The capacity above is the mean + 4 sigma
-    // of a Poisson-like tile; workloads with a tail of busy events overflow it now and then, and an overflowing tile
-    // takes the per-event path, where one 40-jet event holds its warp for ~100 us (measured: a straggler SM 12 %
-    // behind the rest at the end of the launch).
+    // Shared memory the chosen shape leaves unused also goes to the jet buffers (fewer overflowing tiles still).
     if (d->tune_cap_jets <= 0) {
         int budget = sm_total / best_ctas - 1024;
         if (budget > smem_max) budget = smem_max;
-        while (cap_j + 4 <= MAX_JETS_TILE && cap_j + 4 <= 2 * round_up4(cap_for((double)d->jets.n_objects / nev, 64))) {
+        while (cap_j + 4 <= MAX_JETS_TILE && cap_j + 4 <= 2 * cap_j4) {
             const int r = chain_region_layout(P, d, calib, cap_j + 4, cap_m, cap_e);
             if (shared_bytes + wpc * r > budget) break;
             cap_j += 4;
