@@ -1620,7 +1620,15 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
 #define HEPK_PICK_COMMON(MAXT) (calib ? dev::chain_kernel<true, true, MAXT, FEAT_COMMON> : dev::chain_kernel<false, true, MAXT, FEAT_COMMON>)
     // several weight columns and few warps (large histograms): a build that keeps the event's weights in registers
     const bool multiw = P.W > 1 && d->weights && wpc <= 16;
-    if (multiw)
+    // The histograms-only shape (the paper's own output: all six observables, counts and weighted sums
+    // over several weight columns, no per-event arrays) also has its feature word fixed at compile time: the generic
+    // build is ~13,000 instructions of which such a launch executes ~4,000, scattered among the rest, and it spent
+    // more time waiting for instruction fetches than for anything else (profiles/r02: stall `no_instruction`).
+    constexpr int FEAT_HISTS = (int)((dev::F_OBS0 * 63u) | dev::F_COUNTS | dev::F_SUMW | dev::F_WEIGHTS | dev::F_MULTIW);
+    const bool hists_shape = multiw && (int)feat_host == FEAT_HISTS && !d->out_jet_mask && has_el && !d->tune_generic_build;
+    if (hists_shape)
+        kern = calib ? dev::chain_kernel<true, true, 512, FEAT_HISTS, HEPK_MAX_WVAR> : dev::chain_kernel<false, true, 512, FEAT_HISTS, HEPK_MAX_WVAR>;
+    else if (multiw)
         kern = calib ? (has_el ? dev::chain_kernel<true, true, 512, -1, HEPK_MAX_WVAR> : dev::chain_kernel<true, false, 512, -1, HEPK_MAX_WVAR>)
                      : (has_el ? dev::chain_kernel<false, true, 512, -1, HEPK_MAX_WVAR> : dev::chain_kernel<false, false, 512, -1, HEPK_MAX_WVAR>);
     else if (wpc <= 20) kern = common ? HEPK_PICK_COMMON(640) : HEPK_PICK(640, -1);
