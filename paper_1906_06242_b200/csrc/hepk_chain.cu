@@ -603,9 +603,9 @@ __device__ __forceinline__ void hist_scales(const ChainParams& P, float& sc, flo
     sc = sc2 = 0.0f;
     if (!P.hist_hdr || P.hist_hdr[HDR_BAD] != 0u) return;
     const float tmax = P.evw_table ? __uint_as_float(P.hist_hdr[HDR_TMAX]) : 1.0f;
-    const float tmin = P.evw_table ? __uint_as_float(P.hist_hdr[HDR_TMIN]) : 1.0f;
+    const float tmin = P.evw_table ? __uint_as_float(~P.hist_hdr[HDR_TMIN]) : 1.0f;      // (never updated: NaN, and the scheme is off)
     const float wm = __uint_as_float(P.hist_hdr[HDR_WMAX]) * tmax;
-    const float wn = __uint_as_float(P.hist_hdr[HDR_WMIN]) * tmin;
+    const float wn = __uint_as_float(~P.hist_hdr[HDR_WMIN]) * tmin;
     if (!(wm > 0.0f && wm < CUDART_INF_F && wn > 0.0f && wm <= 8.0f * wn)) return;
     if (!(wm * wm < CUDART_INF_F && wn * wn > 0.0f)) return;
     int e, e2;
@@ -1272,8 +1272,8 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
 
 // Range of the launch's weights: max |w|, min non-zero |w| (bits of a non-negative float order like unsigned
 // integers) and a flag for non-finite values, into the workspace header; the same for the event-weight table.
-// hdr[HDR_WMAX] = hdr[HDR_TMAX] = 0, hdr[HDR_WMIN] = hdr[HDR_TMIN] = +inf bits, hdr[HDR_BAD] = 0 set by the caller.
-// w == nullptr: every weight is 1.
+// The minima are kept as the COMPLEMENT of their bits and updated with atomicMax, so the caller's memset of the header to
+// zero is the whole initialisation (0 = "no non-zero value seen").  w == nullptr: every weight is 1.
 __global__ void chain_weight_range_kernel(const float* __restrict__ w, long long n, long long stride, int rows,
                                           const float* __restrict__ table, int nt, unsigned int* __restrict__ hdr)
 {
@@ -1281,22 +1281,39 @@ __global__ void chain_weight_range_kernel(const float* __restrict__ w, long long
     auto fold = [&](const float* p, long long cnt, long long rs, int nrow, int imax, int imin) {
         float m = 0.0f, mn = CUDART_INF_F;
         bool bad = false;
-        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt * nrow; i += (long long)gridDim.x * blockDim.x) {
-            const float a = fabsf(p[(i / cnt) * rs + i % cnt]);
+        auto take = [&](float x) {
+            const float a = fabsf(x);
             bad = bad || !(a < CUDART_INF_F);
             m = fmaxf(m, a);
             if (a > 0.0f) mn = fminf(mn, a);
+        };
+        const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x, nt_ = (long long)gridDim.x * blockDim.x;
+        for (int r = 0; r < nrow; ++r) {
+            const float* q = p + r * rs;
+            // 16-byte loads over the aligned body of the row, four in flight per thread; scalar head and tail
+            const long long head = min((long long)((4 - ((reinterpret_cast<uintptr_t>(q) >> 2) & 3)) & 3), cnt);
+            const long long n4 = (cnt - head) >> 2;
+            const float4* q4 = reinterpret_cast<const float4*>(q + head);
+            long long g = t0;
+            for (; g + 3 * nt_ < n4; g += 4 * nt_) {
+                const float4 a = __ldg(q4 + g), b = __ldg(q4 + g + nt_), c = __ldg(q4 + g + 2 * nt_), e = __ldg(q4 + g + 3 * nt_);
+                take(a.x); take(a.y); take(a.z); take(a.w); take(b.x); take(b.y); take(b.z); take(b.w);
+                take(c.x); take(c.y); take(c.z); take(c.w); take(e.x); take(e.y); take(e.z); take(e.w);
+            }
+            for (; g < n4; g += nt_) { const float4 a = __ldg(q4 + g); take(a.x); take(a.y); take(a.z); take(a.w); }
+            for (long long i = t0; i < head; i += nt_) take(q[i]);
+            for (long long i = head + 4 * n4 + t0; i < cnt; i += nt_) take(q[i]);
         }
         const unsigned int b = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
         const unsigned int c = __reduce_min_sync(0xffffffffu, __float_as_uint(mn));
         if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(hdr + HDR_BAD, 1u);
         if ((threadIdx.x & 31) == 0) {
             if (b) atomicMax(hdr + imax, b);
-            atomicMin(hdr + imin, c);
+            if (c != 0x7f800000u) atomicMax(hdr + imin, ~c);
         }
     };
     if (w) fold(w, n, stride, rows, HDR_WMAX, HDR_WMIN);
-    else if (blockIdx.x == 0 && threadIdx.x == 0) hdr[HDR_WMAX] = hdr[HDR_WMIN] = __float_as_uint(1.0f);
+    else if (blockIdx.x == 0 && threadIdx.x == 0) { hdr[HDR_WMAX] = __float_as_uint(1.0f); hdr[HDR_WMIN] = ~__float_as_uint(1.0f); }
     if (table) fold(table, nt, nt, 1, HDR_TMAX, HDR_TMIN);
 }
 
@@ -1379,7 +1396,6 @@ static long long hist_slots_per_variant(const hepk_chain_desc* d)
 
 static int round_up4(long long x) { return (int)((x + 3) / 4 * 4); }
 
-static const unsigned int g_inf_bits = 0x7f800000u;      // +inf: start value of the "minimum |w|" header words
 
 // Internal histogram layout (ChainParams): columns of a slot row and the padded row length.
 struct HistLayout { int ncol, ws, col_w2, col_cnt; long long n_words; };
@@ -1647,8 +1663,6 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
 
     if (want_hist) {
         HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, HDR_WORDS * 4 + (size_t)n_words * 8, st));
-        HEPK_CUDA_TRY(cudaMemcpyAsync((unsigned int*)workspace + HDR_WMIN, &g_inf_bits, 4, cudaMemcpyHostToDevice, st));
-        HEPK_CUDA_TRY(cudaMemcpyAsync((unsigned int*)workspace + HDR_TMIN, &g_inf_bits, 4, cudaMemcpyHostToDevice, st));
         const long long nw = (long long)P.W * P.n_events;
         long long blocks = (nw + 256 * 8 - 1) / (256 * 8);
         if (blocks > 4 * sm_count()) blocks = 4 * sm_count();
