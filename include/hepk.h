@@ -77,9 +77,12 @@ int32_t hepk_select_mask(const float* pt, const float* eta, int64_t n,
  * Empty values: sum 0.0f, count 0, max -inf, min +inf, argmax -1.  argmax is the index LOCAL to
  * the event (g - offsets[e]); equal values: the smallest index wins; NaN elements are skipped by
  * max / min / argmax and propagated by sum.  count ignores `data` (may be NULL).
- * variant: 0 = auto, 1 = warp-per-event (lanes stride over the event's particles, shuffle
- * reduction), 2 = block-per-tile (a tile of events staged through shared memory with TMA bulk
- * copies, one thread per event).  count / max / min / argmax are bitwise identical across variants. */
+ * variant: 0 = auto (= 2), 1 = warp-per-event (lanes stride over the event's particles, shuffle
+ * reduction), 2 = block-per-tile (every warp of a persistent block streams tiles of 64 events through
+ * its own double-buffered shared-memory stage with TMA bulk copies; one lane per event, the whole warp
+ * for the elements of an event beyond the 16th).  count / max / min / argmax are bitwise identical
+ * across variants; sums are accumulated in float64 and rounded once (tolerance class).  The calls
+ * enqueue and return (nothing is read back from the device). */
 #define HEPK_VARIANT_AUTO            0
 #define HEPK_VARIANT_WARP_PER_EVENT  1
 #define HEPK_VARIANT_BLOCK_PER_TILE  2

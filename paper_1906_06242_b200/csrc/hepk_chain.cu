@@ -310,8 +310,9 @@ __device__ __forceinline__ float dr2_packed(float2 jet, float2 lep)
 }
 
 // [profile phase: pair mass]
-// pair_mass_fast (hepk_common.cuh) with the hardware approximations (ex2, rcp, sqrt: 1-2 ulp each) in place of
-// the library calls; tolerance class, every term of M^2 >= 0, ~60 instructions.
+// pair_mass_f32 (hepk_common.cuh) with the transcendental pieces written out for the ranges that occur here (exp
+// through ex2.approx, sinh by a Taylor polynomial for h <= 1, sin by an odd polynomial on [-pi/2, pi/2]) and the
+// hardware approximations (ex2, rcp, sqrt: 1-2 ulp each) in place of the library calls; tolerance class, every term of M^2 >= 0, ~60 instructions.
 __device__ __forceinline__ float pair_mass_lean(float pt1, float eta1, float phi1, float m1,
                                                 float pt2, float eta2, float phi2, float m2)
 {

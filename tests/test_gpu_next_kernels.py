@@ -185,7 +185,7 @@ def test_triplet_mass(hk, config, n):
 
 
 def test_triplet_mass_long_events(hk):
-    """Events larger than the kernel's shared-memory cache (96 selected jets) and exact ties."""
+    """Events larger than the kernel's shared-memory cache (64 selected jets) and exact ties."""
     rng = np.random.default_rng(13)
     counts = np.array([0, 2, 3, 120, 5, 97, 96, 1, 40], np.int64)
     off = np.zeros(counts.size + 1, np.int64)
