@@ -376,3 +376,38 @@ def test_fill_histogram_concentrated_and_nonuniform(hk):
     ws, wc = hepo.fill_histogram(x, None, edges)
     gs, gc = hk.fill_histogram(dev(x), None, dev(edges))
     assert_exact(to_np(gc), wc)
+
+
+# --------------------------------------------------------------------------- dense collections (fewer lanes per tile)
+@pytest.mark.parametrize("mean1,mean2", [(30, 6), (90, 20), (400, 3), (7, 70)])
+def test_jagged_kernels_on_dense_collections(hk, mean1, mean2):
+    """Collections dense enough that 32 lanes per tile would overflow the fixed staging buffers: the streaming
+    kernels (hepk_tiles.cu) then take 16, 8, ... lanes per tile, decided on the device from offsets[n_events].
+    Odd total sizes and shifted pointers also exercise the array-end and array-start slices."""
+    rng = np.random.default_rng(1000 + mean1)
+    n = 4003
+    c1 = rng.poisson(mean1, n).astype(np.int64)
+    c2 = rng.poisson(mean2, n).astype(np.int64)
+    c1[17] = 0; c2[23] = 0; c1[n - 1] += 3
+    off1 = np.zeros(n + 1, np.int64); off1[1:] = np.cumsum(c1)
+    off2 = np.zeros(n + 1, np.int64); off2[1:] = np.cumsum(c2)
+    m1, m2 = int(off1[-1]), int(off2[-1])
+    pt = (20 + rng.exponential(30, m1)).astype(np.float32)
+    eta1 = rng.uniform(-2.5, 2.5, m1).astype(np.float32); phi1 = rng.uniform(-np.pi, np.pi, m1).astype(np.float32)
+    mass = rng.exponential(10, m1).astype(np.float32)
+    eta2 = rng.uniform(-2.5, 2.5, m2).astype(np.float32); phi2 = rng.uniform(-np.pi, np.pi, m2).astype(np.float32)
+    s1 = (rng.random(m1) < 0.7).astype(np.uint8); s2 = (rng.random(m2) < 0.8).astype(np.uint8)
+    rows = (rng.random(n) < 0.9).astype(np.uint8)
+    for shift in (0, 3):
+        mk = (lambda a: misaligned(a, shift)) if shift else dev
+        got = _reduce_all(hk, pt, off1, rows, s1, 2, d_data=mk(pt), d_mask=mk(s1))
+        _check_reductions(got, pt, off1, rows, s1)
+        got = _reduce_all(hk, pt, off1, None, None, 2, d_data=mk(pt))
+        _check_reductions(got, pt, off1, None, None)
+        want = hepo.deltar_mask(eta1, phi1, off1, s1, eta2, phi2, off2, s2, 0.4)
+        g = hk.deltar_mask(mk(eta1), mk(phi1), dev(off1), mk(s1), mk(eta2), mk(phi2), dev(off2), mk(s2), 0.4)
+        assert_exact(to_np(g), want)
+        wm, w1, w2 = hepo.pair_invmass(pt, eta1, phi1, mass, off1, s1)
+        gm, g1, g2 = hk.pair_invmass(mk(pt), mk(eta1), mk(phi1), mk(mass), dev(off1), mk(s1))
+        assert_exact(to_np(g1), w1, "i1"); assert_exact(to_np(g2), w2, "i2")
+        assert_tol(to_np(gm), wm, "mass")
