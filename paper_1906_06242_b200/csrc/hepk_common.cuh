@@ -282,6 +282,70 @@ __device__ __forceinline__ float pair_mass_f32(float pt1, float eta1, float phi1
     return sqrtf(fmaxf(msq, 0.0f));
 }
 
+// hardware approximations (1-2 ulp each)
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float sqrt_approx(float x)
+{
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+
+// pair_mass_f32 (hepk_common.cuh) with the transcendental pieces written out for the ranges that occur here (exp
+// through ex2.approx, sinh by a Taylor polynomial for h <= 1, sin by an odd polynomial on [-pi/2, pi/2]) and the
+// hardware approximations (ex2, rcp, sqrt: 1-2 ulp each) in place of the library calls; tolerance class, every term of M^2 >= 0, ~60 instructions.
+__device__ __forceinline__ float pair_mass_lean(float pt1, float eta1, float phi1, float m1,
+                                                float pt2, float eta2, float phi2, float m2)
+{
+    const float LOG2E = 1.44269504088896341f;
+    const float e1 = ex2_approx(eta1 * LOG2E), e2 = ex2_approx(eta2 * LOG2E);
+    const float ch1 = 0.5f * (e1 + rcp_approx(e1));
+    const float ch2 = 0.5f * (e2 + rcp_approx(e2));
+    const float h = 0.5f * fabsf(eta1 - eta2);
+    const float h2 = h * h;
+    float sh_small = fmaf(h2, 1.0f / 39916800.0f, 1.0f / 362880.0f);
+    sh_small = fmaf(sh_small, h2, 1.0f / 5040.0f);
+    sh_small = fmaf(sh_small, h2, 1.0f / 120.0f);
+    sh_small = fmaf(sh_small, h2, 1.0f / 6.0f);
+    sh_small = fmaf(sh_small * h2, h, h);
+    const float eh = ex2_approx(h * LOG2E);
+    const float sh_big = 0.5f * (eh - rcp_approx(eh));
+    const float sh = h <= 1.0f ? sh_small : sh_big;
+    float d = __fsub_rn(phi1, phi2);
+    const float bb = __fsub_rn(d, phi1);
+    float dl = __fsub_rn(__fsub_rn(phi1, __fsub_rn(d, bb)), __fadd_rn(phi2, bb));
+    const float TWO_PI_LO = -1.7484555e-07f;   // 2*pi - TWO_PI_F
+    if (d > HEPK_PI_F) { d = __fsub_rn(d, HEPK_TWO_PI_F); dl = __fsub_rn(dl, TWO_PI_LO); }
+    else if (d < -HEPK_PI_F) { d = __fadd_rn(d, HEPK_TWO_PI_F); dl = __fadd_rn(dl, TWO_PI_LO); }
+    const float x_ = 0.5f * (d + dl), z = x_ * x_;
+    float sn = fmaf(z, 1.0f / 6227020800.0f, -1.0f / 39916800.0f);
+    sn = fmaf(sn, z, 1.0f / 362880.0f);
+    sn = fmaf(sn, z, -1.0f / 5040.0f);
+    sn = fmaf(sn, z, 1.0f / 120.0f);
+    sn = fmaf(sn, z, -1.0f / 6.0f);
+    sn = fmaf(sn * z, x_, x_);
+    const float r1 = m1 * rcp_approx(pt1 * ch1), r2 = m2 * rcp_approx(pt2 * ch2);
+    const float x1 = r1 * r1, x2 = r2 * r2;
+    const float x = x1 + x2 + x1 * x2;
+    const float t = x * rcp_approx(sqrt_approx(1.0f + x) + 1.0f);
+    const float bracket = ch1 * ch2 * t + 2.0f * (sh * sh + sn * sn);
+    const float msq = m1 * m1 + m2 * m2 + 2.0f * pt1 * pt2 * bracket;
+    return sqrt_approx(fmaxf(msq, 0.0f));
+}
+
+
 // The defining form in float64 (include/hepk.h, hepk_pair_invmass).  Used only where the float32 result above
 // lands within its own error band of a histogram edge, so that the bin is decided by the float32 rounding of
 // the float64 value — the precision the result is defined in (R16).

@@ -300,7 +300,7 @@ struct RedAcc {
     int i;
     __device__ __forceinline__ void init()
     {
-        v = OP == OP_MAX ? -CUDART_INF_F : (OP == OP_MIN ? CUDART_INF_F : 0.f);
+        v = (OP == OP_MAX || OP == OP_ARGMAX) ? -CUDART_INF_F : (OP == OP_MIN ? CUDART_INF_F : 0.f);
         s = 0.0;
         i = OP == OP_ARGMAX ? -1 : 0;
     }
@@ -311,7 +311,13 @@ struct RedAcc {
         else if (OP == OP_COUNT) i += take ? 1 : 0;
         else if (OP == OP_MAX) { if (take && x > v) v = x; }       // a NaN compares false: skipped
         else if (OP == OP_MIN) { if (take && x < v) v = x; }
-        else { if (take && x == x && (i < 0 || x > v)) { v = x; i = k; } }     // k ascending within a thread
+        else { if (take && x == x && (i < 0 || x > v)) { v = x; i = k; } }     // k ascending within a thread (full rule)
+    }
+    // argmax only: the rule without its "the first non-NaN element is always taken" clause.  Starting from v = -inf it
+    // differs from push() only when no element exceeds -inf; the caller then redoes the event with push().
+    __device__ __forceinline__ void push_gt(float x, int k)
+    {
+        if (x > v) { v = x; i = k; }
     }
     __device__ __forceinline__ void merge(const RedAcc& o)
     {
@@ -392,14 +398,18 @@ struct ReduceOp {
                 bool t0, t1;
                 if (nmain & 1) {
                     const float x = value(ad, t0);
-                    acc.push(x, 0, t0);
+                    if (OP == OP_ARGMAX) acc.push_gt(x, 0); else acc.push(x, 0, t0);
                     k = 1; ad += ES;
                 }
 #pragma unroll 1
                 for (; k < nmain; k += 2, ad += 2 * ES) {          // two elements per iteration
                     const float x0 = value(ad, t0), x1 = value(ad + ES, t1);
-                    acc.push(x0, k, t0);
-                    acc.push(x1, k + 1, t1);
+                    if (OP == OP_ARGMAX) { acc.push_gt(x0, k); acc.push_gt(x1, k + 1); }
+                    else { acc.push(x0, k, t0); acc.push(x1, k + 1, t1); }
+                }
+                if (OP == OP_ARGMAX && acc.i < 0 && nmain > 0) {   // nothing above -inf: the full rule (rare)
+                    acc.init();
+                    for (int kk = 0; kk < nmain; ++kk) acc.push(lds_f(a0 + ES * (unsigned)kk), kk, true);
                 }
                 // long events: the rest of their elements, 32 at a time, one per lane, folded into the owner's state
                 for (unsigned lm = __ballot_sync(0xffffffffu, n > TAIL); lm; lm &= lm - 1) {
@@ -601,24 +611,52 @@ struct InvmassOp {
     int *out_i1, *out_i2;
 
     __device__ __forceinline__ void staged(const TileParams&, const uint32_t (&ca)[Shape::NCA], uint32_t, long long e0, int ne, int lane,
-                                           const int (&o)[1][2], const int (&lo)[1], const int (&)[1])
+                                           const int (&o)[1][2], const int (&lo)[1], const int (&cnt)[1])
     {
         const bool live = lane < ne;
         const int k0 = o[0][0] - lo[0], n = live ? o[0][1] - o[0][0] : 0;
+        // masked-out jets become NaN in a flat pass (one lane per jet), so the per-event loop never looks at the mask
+        if (HAS_MASK) {
+            for (int j = lane; j < cnt[0]; j += 32)
+                if (!lds_b(ca[4] + (unsigned)j)) sts_w(ca[0] + 4u * (unsigned)j, 0x7fc00000u);
+            __syncwarp();
+        }
+        constexpr int TAIL = 16;          // jets of an event beyond this many are taken by the whole warp
         Top2 top;
         top.init();
-        uint32_t ap = ca[0] + 4u * (unsigned)k0, ak = HAS_MASK ? ca[4] + (unsigned)k0 : 0u;
+        const uint32_t a0 = ca[0] + 4u * (unsigned)k0;
+        const int nmain = n < TAIL ? n : TAIL;
 #pragma unroll 1
-        for (int k = 0; k < n; ++k, ap += 4, ak += 1) {
-            const float p = lds_f(ap);
-            if (HAS_MASK && !lds_b(ak)) continue;
-            top.push_any(p, k);
+        for (int k = 0; k < nmain; ++k) top.push_any(lds_f(a0 + 4u * (unsigned)k), k);
+        for (unsigned lm = __ballot_sync(0xffffffffu, n > TAIL); lm; lm &= lm - 1) {
+            const int src = __ffs(lm) - 1;
+            const uint32_t as = __shfl_sync(0xffffffffu, a0, src);
+            const int ns = __shfl_sync(0xffffffffu, n, src);
+            // 32 jets at a time, one per lane: the two best of the chunk by (value desc, index asc), folded into the
+            // owner's state in that order (their indices exceed every index seen so far, so the tie rule holds)
+            for (int kb = TAIL; kb < ns; kb += 32) {
+                const int k = kb + lane;
+                const float p = k < ns ? lds_f(as + 4u * (unsigned)k) : CUDART_NAN_F;
+                const bool ok = p == p;
+                // order-preserving key: a < b <=> key(a) < key(b); 0 marks "no value"
+                const unsigned bits = p == 0.f ? 0u : __float_as_uint(p);      // (-0 and +0 are one value)
+                const unsigned u = ok ? (bits ^ ((unsigned)((int)bits >> 31) | 0x80000000u)) : 0u;
+                const unsigned k1 = __reduce_max_sync(0xffffffffu, u);
+                const int j1 = __reduce_min_sync(0xffffffffu, (ok && u == k1) ? k : 0x7fffffff);
+                const unsigned u2 = k == j1 ? 0u : u;
+                const unsigned k2 = __reduce_max_sync(0xffffffffu, u2);
+                const int j2 = __reduce_min_sync(0xffffffffu, (u2 != 0u && u2 == k2) ? k : 0x7fffffff);
+                if (lane == src) {
+                    if (k1 != 0u) top.push_any(__uint_as_float(k1 ^ ((k1 & 0x80000000u) ? 0x80000000u : 0xffffffffu)), j1);
+                    if (k2 != 0u) top.push_any(__uint_as_float(k2 ^ ((k2 & 0x80000000u) ? 0x80000000u : 0xffffffffu)), j2);
+                }
+            }
         }
         float m = 0.f;
         if (top.i2 >= 0) {
             const unsigned a = 4u * (unsigned)(k0 + top.i1), c = 4u * (unsigned)(k0 + top.i2);
-            m = pair_mass_f32(top.b1, lds_f(ca[1] + a), lds_f(ca[2] + a), lds_f(ca[3] + a),
-                              top.b2, lds_f(ca[1] + c), lds_f(ca[2] + c), lds_f(ca[3] + c));
+            m = pair_mass_lean(top.b1, lds_f(ca[1] + a), lds_f(ca[2] + a), lds_f(ca[3] + a),
+                               top.b2, lds_f(ca[1] + c), lds_f(ca[2] + c), lds_f(ca[3] + c));
         }
         if (live) {
             out_mass[e0 + lane] = m;
