@@ -335,6 +335,14 @@ def run_hepk(args):
     else:
         roof = chain_roofline(wl, kern_ms, kern_n, hists_only, args.config, args.variants)
 
+    # the same bytes over the WHOLE step's device time (weight-range pre-pass, header memset, chain kernel(s), histogram
+    # finalize), the pre-pass's second read of the weights added to the bytes: what a user of the call gets
+    prepass = 4.0 * inp.n_events * (wl.weights.shape[0] if wl.weights is not None else 0) * kern_n
+    step_bytes = roof["algorithmic_bytes_per_step"] + prepass
+    roof["whole_step"] = {"ms": ms_step, "bytes": step_bytes, "achieved": step_bytes / (ms_step * 1e-3) / 1e9,
+                          "frac": step_bytes / (ms_step * 1e-3) / 1e9 / roof["peak"],
+                          "note": "chain kernel + weight-range pre-pass + memset + finalize; bytes include the pre-pass's read of the weights"}
+
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None,
@@ -567,6 +575,12 @@ def single_kernels(args, hk, torch, hepgen, steps=None):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / steps
         out[name] = {"ms": ms, "algorithmic_bytes": nbytes, "GBps": nbytes / ms / 1e6, "frac_of_peak": nbytes / ms / 1e6 / peak}
+    # one 4-byte element per event costs the memory system a 32-byte sector: the f-1 gathers are bound by sectors, not
+    # by the method's bytes (profiles/r02c_single_kernels.md: their DRAM traffic runs at ~0.9 of the copy peak)
+    for name, sect in (("get_in_offsets[index 0]", (8 + 32 + 4) * N), ("set_in_offsets[index 0]", (8 + 32 + 32) * N)):
+        if name in out:
+            out[name]["sector_bytes"] = sect
+            out[name]["frac_of_peak_by_sectors"] = sect / out[name]["ms"] / 1e6 / peak
     return {"metric": "single-kernel throughput (algorithmic GB/s; side measurement)", "unit": "GB/s",
             "config": {"workload": workload_name(cfg, wl), "events": N, "jets": Mj, "muons": Mm,
                        "l2": "config 1 (132 MB) is L2-resident on B200; config 2 gives HBM figures",
