@@ -916,9 +916,8 @@ __global__ void __launch_bounds__(MAXT, 1) chain_kernel(const __grid_constant__ 
                 wt[w] = __ldg(P.weights + (long long)w * P.w_stride + e0 + lane);
             if (feat & F_EVW) wt[w] = __fmul_rn(wt[w], evf);             // one float32 multiply (exact class)
         }
-        EventOffsets neo;
-        neo.j0 = neo.j1 = neo.m0 = neo.m1 = neo.q0 = neo.q1 = 0;
-        if (has_next) load_event_offsets<HAS_EL>(P, tile_next, lane, neo);
+        EventOffsets neo;      // (without a next tile the current one is read again: harmless, and no branch)
+        load_event_offsets<HAS_EL>(P, has_next ? tile_next : tile, lane, neo);
         bool staged = fit;
         bool released = false;
         fit = false;
