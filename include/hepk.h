@@ -255,7 +255,10 @@ int32_t hepk_analysis_chain(const hepk_chain_desc* d, void* workspace, size_t wo
  * end and ADDED to the host arrays.  overlap != 0 double-buffers the copies against the kernels on
  * internal streams; overlap == 0 runs copy -> compute -> copy serially.  The call returns after all work
  * has finished (it synchronises).  `workspace` is a DEVICE buffer of at least
- * hepk_chain_host_workspace_bytes(d, batch_events) bytes.  calib / axis edge arrays are HOST too. */
+ * hepk_chain_host_workspace_bytes(d, batch_events) bytes.  calib / axis edge arrays are HOST too.
+ * Thread safety: the call creates its two internal streams itself and destroys them before it returns
+ * (after draining them, also on an error return), so calls from several host threads are independent as
+ * long as each passes its own workspace and output buffers. */
 size_t  hepk_chain_host_workspace_bytes(const hepk_chain_desc* d, int64_t batch_events);
 int32_t hepk_analysis_chain_host(const hepk_chain_desc* d, int64_t batch_events, int32_t overlap,
                                  void* workspace, size_t workspace_bytes, void* stream);
