@@ -348,7 +348,9 @@ struct RedAcc {
 
 template <int OP, bool HAS_MASK>
 struct ReduceOp {
-    static constexpr int H = 2;           // events per lane: these kernels do little per event, so tiles are large
+    // events per lane: these kernels do little per event, so tiles are large (count stages one byte per element at most
+    // and can afford 128 events per tile)
+    static constexpr int H = OP == OP_COUNT ? 4 : 2;
     typedef TileShape<H, 1, OP != OP_COUNT ? 1 : 0, HAS_MASK ? 1 : 0> Shape;
     const float* data;
     const unsigned char* mask_rows;
@@ -360,11 +362,24 @@ struct ReduceOp {
     {
         return OP == OP_MAX ? -CUDART_INF_F : (OP == OP_MIN ? CUDART_INF_F : (OP == OP_ARGMAX ? CUDART_NAN_F : 0.f));
     }
-    __device__ __forceinline__ void staged(const TileParams&, const uint32_t (&ca)[Shape::NCA], uint32_t,
+    __device__ __forceinline__ void staged(const TileParams&, const uint32_t (&ca)[Shape::NCA], uint32_t extra_a,
                                            long long e0, int ne, int lane, const int (&o)[1][H + 1],
                                            const int (&lo)[1], const int (&cnt)[1])
     {
         constexpr bool DATA = OP != OP_COUNT;
+        // count over a mask: a flat pass turns the tile's mask bytes into a bit string (one ballot per 32 elements), and
+        // an event's count is the population count of its bit range
+        constexpr bool BITS = OP == OP_COUNT && HAS_MASK;
+        if (BITS) {
+            int j0 = 0;
+            for (; j0 < cnt[0]; j0 += 32) {
+                const int j = j0 + lane;
+                const unsigned w = __ballot_sync(0xffffffffu, j < cnt[0] && lds_b(ca[0] + (unsigned)j) != 0u);
+                if (lane == 0) sts_w(extra_a + 4u * (unsigned)(j0 >> 5), w);
+            }
+            if (lane == 0) sts_w(extra_a + 4u * (unsigned)(j0 >> 5), 0u);        // (a range may end exactly at a word boundary)
+            __syncwarp();
+        }
         constexpr int TAIL = 16;          // elements of an event beyond this many are reduced by the whole warp
         constexpr unsigned ES = DATA ? 4u : 1u;
         // Flat pass, one lane per element: a masked-out element becomes the reduction's neutral value, so the
@@ -390,6 +405,17 @@ struct ReduceOp {
             acc.init();
             if (!DATA && !HAS_MASK) {
                 acc.i = n;
+            } else if (BITS) {
+                int pos = o[0][h] - lo[0], rem = n, c = 0;
+                while (rem > 0) {
+                    const int take = rem < 32 ? rem : 32;
+                    const uint32_t wa = extra_a + 4u * (unsigned)(pos >> 5);
+                    unsigned v = __funnelshift_r(lds_w(wa), lds_w(wa + 4u), (unsigned)(pos & 31));
+                    if (take < 32) v &= (1u << take) - 1u;
+                    c += __popc(v);
+                    pos += take; rem -= take;
+                }
+                acc.i = c;
             } else {
                 const uint32_t a0 = ca[0] + ES * (unsigned)(o[0][h] - lo[0]);
                 const int nmain = n < TAIL ? n : TAIL;
@@ -806,9 +832,9 @@ static int32_t segreduce_dispatch(const float* data, const int64_t* offsets, int
     const int n_cls[4] = {has_data ? 1 : 0, mask_content ? 1 : 0, 0, 0};
     const int64_t* offs[1] = {offsets};
     const int64_t bases[1] = {base};
-    const int caps[1] = {CAP_REDUCE};
+    const int caps[1] = {OP == dev::OP_COUNT ? 2 * CAP_REDUCE : CAP_REDUCE};
     TileLayout L;
-    const int32_t rc = tile_layout(L, n_events, 1, offs, bases, n_cls, ptr, caps, 0, 32);
+    const int32_t rc = tile_layout(L, n_events, 1, offs, bases, n_cls, ptr, caps, OP == dev::OP_COUNT ? caps[0] / 8 + 16 : 0, 32);
     if (rc != HEPK_OK) return rc;
     if (mask_content) {
         dev::ReduceOp<OP, true> op;
