@@ -698,8 +698,7 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
 {
     int a0[3];
     int len[3], tail[3] = {0, 0, 0};
-    int bad = 0;
-    uint32_t total = 0;
+    int bad = 0, edge = 0;
 #pragma unroll
     for (int k = 0; k < (HAS_EL ? 3 : 2); ++k) {
         const int c0 = k == 0 ? 0 : (k == 1 ? 4 : 7);
@@ -712,19 +711,23 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
         // bits, no branches.  At the very end of an array the aligned window may reach past it: the bulk copy then
         // stops at the last full 16 bytes and the (at most three) elements beyond are moved by ordinary loads.
         const int e0k = cnt[k] != 0 ? a0[k] : 0;
+        a0[k] = e0k;
         len[k] = cnt[k] != 0 ? ln : 0;
-        const int over = e0k + len[k] - P.col_n32[k];
-        tail[k] = 0;
-        if (over > 0) {
-            const int lb = (P.col_n32[k] - e0k) & ~3;
-            tail[k] = l0 + cnt[k] - e0k - lb;          // elements of the slice past the bulk copy (0..3)
-            len[k] = lb;
-        }
+        edge |= P.col_n32[k] - e0k - len[k];           // negative: the aligned window reaches past the array
         bad |= cnt[k] | (P.col_cap[c0] - cnt[k]) | e0k | (P.col_n32[k] - l0 - cnt[k]);
-        total += (uint32_t)len[k] * (k == 0 ? 16u : 12u);
     }
     if (bad < 0) return false;
-    if ((tail[0] | tail[1] | tail[2]) != 0) {          // (uniform, rare: the last tile of a launch)
+    if (edge < 0) {          // (uniform, rare: the last tile of a launch)
+#pragma unroll
+        for (int k = 0; k < (HAS_EL ? 3 : 2); ++k) {
+            const int c0 = k == 0 ? 0 : (k == 1 ? 4 : 7);
+            if (a0[k] + len[k] > P.col_n32[k]) {
+                const int l0 = (int)((unsigned)lo[k] - (unsigned)P.col_base[c0]);
+                const int lb = (P.col_n32[k] - a0[k]) & ~3;
+                tail[k] = l0 + cnt[k] - a0[k] - lb;    // elements of the slice past the bulk copy (0..3)
+                len[k] = lb;
+            }
+        }
 #pragma unroll
         for (int c = 0; c < (HAS_EL ? NCOL : 7); ++c) {
             const int k = c < 4 ? 0 : (c < 7 ? 1 : 2);
@@ -733,6 +736,7 @@ __device__ __forceinline__ bool issue_tile(const ChainParams& P, uint32_t region
                         __ldg(reinterpret_cast<const float*>(P.col_ptr[c]) + a0[k] + len[k] + lane));
         }
     }
+    const uint32_t total = (uint32_t)len[0] * 16u + (uint32_t)(len[1] + (HAS_EL ? len[2] : 0)) * 12u;
     // One elected lane issues all copies.  Under elect.sync (and with operands that come from warp reductions, hence
     // uniform registers) each copy is one UBLKCP; under `lane == 0` the compiler wraps every copy in a loop over the
     // lanes that might be active.
