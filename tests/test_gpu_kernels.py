@@ -411,3 +411,22 @@ def test_jagged_kernels_on_dense_collections(hk, mean1, mean2):
         gm, g1, g2 = hk.pair_invmass(mk(pt), mk(eta1), mk(phi1), mk(mass), dev(off1), mk(s1))
         assert_exact(to_np(g1), w1, "i1"); assert_exact(to_np(g2), w2, "i2")
         assert_tol(to_np(gm), wm, "mass")
+
+
+def test_jagged_kernels_with_columns_of_different_alignment(hk, wl2):
+    """Columns of one collection that do not share their alignment modulo 16 bytes cannot be staged with one slice
+    geometry: the launch takes the global-memory path (one lane per event).  Same results."""
+    j, l = wl2.jets, wl2.muons
+    n = 20_001
+    jo, lo_ = j.offsets[:n + 1], l.offsets[:n + 1]
+    mj, ml = int(jo[-1]), int(lo_[-1])
+    pt, eta, phi, mass = j.pt[:mj], j.eta[:mj], j.phi[:mj], j.mass[:mj]
+    sel = hepo.select_mask(pt, eta, 30.0, 2.4)
+    want = hepo.deltar_mask(eta, phi, jo, sel, l.eta[:ml], l.phi[:ml], lo_, None, 0.4)
+    got = hk.deltar_mask(misaligned(eta, 1), misaligned(phi, 2), dev(jo), dev(sel), misaligned(l.eta[:ml], 3), dev(l.phi[:ml]),
+                         dev(lo_), None, 0.4)
+    assert_exact(to_np(got), want)
+    wm, w1, w2 = hepo.pair_invmass(pt, eta, phi, mass, jo, sel)
+    gm, g1, g2 = hk.pair_invmass(misaligned(pt, 1), dev(eta), misaligned(phi, 3), misaligned(mass, 2), dev(jo), dev(sel))
+    assert_exact(to_np(g1), w1, "i1"); assert_exact(to_np(g2), w2, "i2")
+    assert_tol(to_np(gm), wm, "mass")
