@@ -168,7 +168,9 @@ __device__ __forceinline__ float dr2_exact(float eta_a, float phi_a, float eta_b
 {
     const float deta = __fsub_rn(eta_a, eta_b);
     const float ad = fabsf(__fsub_rn(phi_a, phi_b));
-    const float w = ad > HEPK_PI_F ? __fsub_rn(ad, HEPK_TWO_PI_F) : ad;
+    // the wrapped magnitude is min(ad, |ad - 2PI_F|): ad > PI_F => |t| <= PI_F < ad (rn is monotone), ad < PI_F =>
+    // |t| >= PI_F > ad, and at ad == PI_F both are PI_F; two instructions (|.| is a free operand modifier)
+    const float w = fminf(ad, fabsf(__fsub_rn(ad, HEPK_TWO_PI_F)));
     return __fadd_rn(__fmul_rn(deta, deta), __fmul_rn(w, w));
 }
 

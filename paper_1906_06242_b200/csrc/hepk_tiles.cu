@@ -188,6 +188,9 @@ __device__ __forceinline__ void tile_col_addrs(const TileParams& P, uint32_t sta
 #pragma unroll
         for (int j = 0; j < SH::count(q); ++j) ca[SH::first(q) + j] = stage_a + (uint32_t)P.dst[SH::first(q) + j] + sh;
     }
+    // pinned: the compiler would otherwise recompute these few adds from the parameters at every use inside the loops
+#pragma unroll
+    for (int k = 0; k < SH::NCOL; ++k) asm volatile("" : "+r"(ca[k]));
 }
 
 // The streaming loop.  Op provides
