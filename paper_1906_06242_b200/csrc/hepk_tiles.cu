@@ -113,37 +113,38 @@ __device__ __forceinline__ bool tile_issue(const TileParams& P, const int (&n_ob
     // part [bA, bB) of the window that lies inside the array goes by bulk copy.  Only at the very ends of an array can
     // bA > A or bB < A + len; the few elements of the slice outside [bA, bB) are then moved by ordinary loads.
     int bad = 0, edge = 0;
-    uint32_t total = 0;
-    int A[4], bA[4], bB[4], L0[4];
+    int A[4], bA[4], bB[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-        A[q] = bA[q] = bB[q] = L0[q] = 0;
+        A[q] = bA[q] = bB[q] = 0;
         if (SH::count(q) == 0) continue;
         const int c = q >> 1;
-        const int per16 = (q & 1) ? 16 : 4, es = (q & 1) ? 1 : 4;
+        const int per16 = (q & 1) ? 16 : 4;
         const int l0 = (int)((unsigned)lo[c] - (unsigned)P.base[c]);
         const int sh = (l0 + P.mis[q]) & (per16 - 1);
         const int n = cnt[c];
-        const int len = (n + sh + per16 - 1) & ~(per16 - 1);
-        L0[q] = l0;
-        A[q] = l0 - sh;
-        bA[q] = A[q] < 0 ? A[q] + per16 : A[q];
-        bB[q] = A[q] + len <= n_obj[c] ? A[q] + len : A[q] + ((n_obj[c] - A[q]) & ~(per16 - 1));
-        if (n == 0 || bB[q] < bA[q]) bB[q] = bA[q];
+        const int len = n != 0 ? (n + sh + per16 - 1) & ~(per16 - 1) : 0;
+        A[q] = n != 0 ? l0 - sh : 0;
+        bA[q] = A[q];
+        bB[q] = A[q] + len;
         // fits: 0 <= n <= capacity, and the slice lies inside the collection (sign bits, no branches)
         bad |= n | (P.cap[c] - n) | l0 | (n_obj[c] - l0 - n);
-        edge |= n != 0 ? (A[q] | (n_obj[c] - A[q] - len)) : 0;
-        total += (uint32_t)((bB[q] - bA[q]) * es * SH::count(q));
+        edge |= A[q] | (n_obj[c] - bB[q]);          // negative: the window reaches past an end of the array
     }
     if (bad < 0) return false;
-    if (edge < 0) {          // (uniform, rare) slice elements outside the bulk windows
+    if (edge < 0) {          // (uniform, rare) clip the bulk windows to the array; slice elements outside them by ordinary loads
         const int lane = (int)(threadIdx.x & 31u);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             if (SH::count(q) == 0) continue;
-            const int es = (q & 1) ? 1 : 4;
-            for (int j = lane; j < cnt[q >> 1]; j += 32) {
-                const int g = L0[q] + j;
+            const int c = q >> 1;
+            const int per16 = (q & 1) ? 16 : 4, es = (q & 1) ? 1 : 4;
+            const int l0 = (int)((unsigned)lo[c] - (unsigned)P.base[c]);
+            if (A[q] < 0) bA[q] = A[q] + per16;
+            if (bB[q] > n_obj[c]) bB[q] = A[q] + ((n_obj[c] - A[q]) & ~(per16 - 1));
+            if (bB[q] < bA[q]) bB[q] = bA[q];
+            for (int j = lane; j < cnt[c]; j += 32) {
+                const int g = l0 + j;
                 if (g >= bA[q] && g < bB[q]) continue;
 #pragma unroll
                 for (int i = 0; i < SH::count(q); ++i) {
@@ -155,6 +156,9 @@ __device__ __forceinline__ bool tile_issue(const TileParams& P, const int (&n_ob
             }
         }
     }
+    uint32_t total = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) total += (uint32_t)((bB[q] - bA[q]) * ((q & 1) ? 1 : 4) * SH::count(q));
     if (elect_one_lane()) {
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(stage_a), "r"(total) : "memory");
 #pragma unroll
