@@ -301,7 +301,8 @@ int32_t hepk_select_opposite_sign(const float* pt, const int32_t* charge, const 
  *   knots xs[0..nk) ascending with values ys[0..nk), nk >= 2;
  *   out[i] = ys[b] + (x[i] - xs[b]) * (ys[b+1] - ys[b]) / (xs[b+1] - xs[b])  for xs[b] <= x[i] < xs[b+1];
  *   x <= xs[0] -> ys[0], x >= xs[nk-1] -> ys[nk-1] (constant extrapolation), NaN -> NaN.
- * Tolerance class (float32 evaluation).  8*nk bytes of shared memory, more than 200 KB -> HEPK_ERR_UNSUPPORTED. */
+ * Tolerance class (float32 evaluation with one slope per segment).  12*nk bytes of shared memory, more than 200 KB ->
+ * HEPK_ERR_UNSUPPORTED. */
 int32_t hepk_lookup_interp(const float* x, int64_t n, const float* xs, const float* ys, int32_t nk, float* out, void* stream);
 
 /* Two-dimensional weighted histogram ("Extension to multidimensional histograms is straightforward"):

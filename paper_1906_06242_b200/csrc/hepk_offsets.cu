@@ -148,32 +148,45 @@ extern "C" int32_t hepk_select_opposite_sign(const float* pt, const int32_t* cha
 namespace hepk {
 namespace dev {
 
+// Knots in shared memory; the segment is found by the arithmetic bin guess of hepk_lookup_binned when the knots are
+// uniform in x or in log2 x (verified at start-up, exact after one +-1 step), else by binary search; four elements per
+// thread and step with 16-byte loads and stores when the pointers allow.
+template <bool VEC>
 __global__ void __launch_bounds__(256) lookup_interp_kernel(const float* __restrict__ x, long long n, const float* __restrict__ xs,
                                                             const float* __restrict__ ys, int nk, float* __restrict__ out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* s_x = (float*)smem_raw;
     float* s_y = s_x + nk;
+    float* s_m = s_y + nk;                                 // slope of segment i (one IEEE division per segment and CTA)
     for (int i = threadIdx.x; i < nk; i += blockDim.x) { s_x[i] = xs[i]; s_y[i] = ys[i]; }
     __syncthreads();
+    for (int i = threadIdx.x; i + 1 < nk; i += blockDim.x) s_m[i] = (s_y[i + 1] - s_y[i]) / (s_x[i + 1] - s_x[i]);
+    __syncthreads();
+    AxisGuess ax;
+    ax.mode = 0; ax.lo = 0.f; ax.inv = 0.f;
+    if (nk >= 2) ax = classify_axis(s_x, nk - 1);          // the knots as the edges of nk - 1 segments
     const float x_lo = s_x[0], x_hi = s_x[nk - 1];
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const float v = __ldg(x + i);
-        float r;
-        if (v != v) r = v;
-        else if (v <= x_lo) r = s_y[0];
-        else if (v >= x_hi) r = s_y[nk - 1];
-        else {
-            int lo = 0, hi = nk - 1;               // s_x[lo] <= v < s_x[hi]
-            while (hi - lo > 1) {
-                const int mid = (lo + hi) >> 1;
-                if (v >= s_x[mid]) lo = mid; else hi = mid;
-            }
-            const float x0 = s_x[lo], y0 = s_y[lo];
-            const float t = (v - x0) / (s_x[lo + 1] - x0);      // tolerance class: a few float32 roundings
-            r = fmaf(t, s_y[lo + 1] - y0, y0);
+    auto interp = [&](float v) {
+        if (v != v) return v;
+        if (v <= x_lo) return s_y[0];
+        if (v >= x_hi) return s_y[nk - 1];
+        const int lo = find_bin_guess(v, s_x, nk - 1, ax);  // s_x[lo] <= v < s_x[lo + 1]
+        return fmaf(v - s_x[lo], s_m[lo], s_y[lo]);        // tolerance class: a few float32 roundings
+    };
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (VEC) {
+        const long long n4 = n >> 2;
+        for (long long g = t0; g < n4; g += stride) {
+            const float4 v = __ldg(reinterpret_cast<const float4*>(x) + g);
+            float4 r;
+            r.x = interp(v.x); r.y = interp(v.y); r.z = interp(v.z); r.w = interp(v.w);
+            reinterpret_cast<float4*>(out)[g] = r;
         }
-        out[i] = r;
+        for (long long i = (n4 << 2) + t0; i < n; i += stride) out[i] = interp(__ldg(x + i));
+    } else {
+        for (long long i = t0; i < n; i += stride) out[i] = interp(__ldg(x + i));
     }
 }
 
@@ -232,15 +245,18 @@ extern "C" int32_t hepk_lookup_interp(const float* x, int64_t n, const float* xs
 {
     HEPK_REQUIRE(n >= 0, "n < 0");
     HEPK_REQUIRE(xs && ys && nk >= 2, "knots are NULL or fewer than 2");
-    if ((size_t)nk * 8 > 200 * 1024) {
+    if ((size_t)nk * 12 > 200 * 1024) {
         set_error("hepk_lookup_interp: %d knots do not fit 200 KB of shared memory", nk);
         return HEPK_ERR_UNSUPPORTED;
     }
     if (n == 0) return HEPK_OK;
     HEPK_REQUIRE(x && out, "x/out is NULL");
-    const size_t smem = (size_t)nk * 8;
-    HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::lookup_interp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dev::lookup_interp_kernel<<<grid_for(n), 256, smem, (cudaStream_t)stream>>>(x, n, xs, ys, nk, out); count_launch();
+    const size_t smem = (size_t)nk * 12;
+    HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::lookup_interp_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::lookup_interp_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const bool vec = aligned16(x) && aligned16(out);
+    auto kern = vec ? dev::lookup_interp_kernel<true> : dev::lookup_interp_kernel<false>;
+    kern<<<grid_for(vec ? (n + 3) / 4 : n), 256, smem, (cudaStream_t)stream>>>(x, n, xs, ys, nk, out); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
