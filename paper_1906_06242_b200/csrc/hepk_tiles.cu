@@ -1,5 +1,6 @@
 // hepk_tiles.cu — the per-event single kernels that walk jagged collections (include/hepk.h):
-//   hepk_segmented_reduce_{sum,max,min,count,argmax} (variant 2, "block-per-tile"), hepk_deltar_mask, hepk_pair_invmass.
+//   hepk_segmented_reduce_{sum,max,min,count,argmax} (variant 2, "block-per-tile"), hepk_deltar_mask, hepk_pair_invmass,
+//   hepk_select_opposite_sign.
 //
 // One streaming skeleton serves them all.  A CTA is a handful of AUTONOMOUS warps; a warp owns a double-buffered
 // staging region of shared memory with one mbarrier per buffer and streams tiles of 32 x H events through it (a lane
@@ -726,6 +727,99 @@ __global__ void __launch_bounds__(256, 2) invmass_stream_kernel(const __grid_con
     tile_stream<typename InvmassOp<HAS_MASK>::Shape>(P, op);
 }
 
+// =========================================================================================== select_opposite_sign
+// Staged columns: pt, charge (int32, moved as 32-bit words), (mask).  One lane per event finds the leading object and
+// the best object of each sign; the two chosen objects are marked in a per-warp byte buffer that a flat pass writes out
+// (coalesced bytes, every object of the tile).
+struct OppSignPick {
+    int lead, bpos, bneg;
+    float plead, ppos, pneg;
+    int qlead;
+    __device__ __forceinline__ void init() { lead = bpos = bneg = -1; plead = ppos = pneg = 0.f; qlead = 0; }
+    // strict > keeps the first index among equal pt; NaN skipped
+    __device__ __forceinline__ void push(float p, int q, int k)
+    {
+        if (p != p) return;
+        if (lead < 0 || p > plead) { lead = k; plead = p; qlead = q; }
+        if (q > 0 && (bpos < 0 || p > ppos)) { bpos = k; ppos = p; }
+        if (q < 0 && (bneg < 0 || p > pneg)) { bneg = k; pneg = p; }
+    }
+    __device__ __forceinline__ int partner() const
+    {
+        if (lead < 0) return -1;
+        return qlead > 0 ? bneg : (qlead < 0 ? bpos : -1);      // charge 0 has no opposite sign
+    }
+};
+
+template <bool HAS_MASK>
+struct OppSignOp {
+    static constexpr int H = 4;          // (lepton collections are sparse: 128 events per tile)
+    typedef TileShape<H, 1, 2, HAS_MASK ? 1 : 0> Shape;
+    const float* pt;
+    const int* charge;
+    const unsigned char *mask_rows, *mask;
+    unsigned char* out;
+
+    __device__ __forceinline__ void staged(const TileParams& P, const uint32_t (&ca)[Shape::NCA], uint32_t extra_a, long long e0, int ne,
+                                           int lane, const int (&o)[1][H + 1], const int (&lo)[1], const int (&cnt)[1])
+    {
+        const int nw = (cnt[0] + 3) >> 2;
+        for (int j = lane; j < nw; j += 32) sts_w(extra_a + 4u * (unsigned)j, 0u);
+        __syncwarp();
+#pragma unroll
+        for (int h = 0; h < H; ++h) {
+            const int ev = lane * H + h;
+            const int k0 = o[0][h] - lo[0];
+            int n = o[0][h + 1] - o[0][h];
+            if (mask_rows && ev < ne && !__ldg(mask_rows + e0 + ev)) n = 0;
+            OppSignPick pk;
+            pk.init();
+            uint32_t ap = ca[0] + 4u * (unsigned)k0, aq = ca[1] + 4u * (unsigned)k0, am = HAS_MASK ? ca[2] + (unsigned)k0 : 0u;
+#pragma unroll 1
+            for (int k = 0; k < n; ++k, ap += 4, aq += 4, am += 1) {
+                if (HAS_MASK && !lds_b(am)) continue;
+                pk.push(lds_f(ap), (int)lds_w(aq), k);
+            }
+            const int part = pk.partner();
+            if (part >= 0) {
+                sts_b(extra_a + (unsigned)(k0 + pk.lead), 1u);
+                sts_b(extra_a + (unsigned)(k0 + part), 1u);
+            }
+        }
+        __syncwarp();
+        unsigned char* dst = out + (long long)(int)((unsigned)lo[0] - (unsigned)P.base[0]);
+        for (int j = lane; j < cnt[0]; j += 32) dst[j] = (unsigned char)lds_b(extra_a + (unsigned)j);
+    }
+    // the paper's loop shape: one lane per event, global memory
+    __device__ __forceinline__ void global(const TileParams& P, long long e0, int ne, int lane)
+    {
+        for (int b = 0; b < ne; b += 32) {
+            if (b + lane >= ne) continue;
+            const long long e = e0 + b + lane;
+            const long long g0 = P.off[0][e], g1 = P.off[0][e + 1];
+            OppSignPick pk;
+            pk.init();
+            if (!mask_rows || mask_rows[e])
+                for (long long g = g0; g < g1; ++g) {
+                    const long long i = g - P.base[0];
+                    if (mask && !mask[i]) continue;
+                    pk.push(pt[i], charge[i], (int)(g - g0));
+                }
+            const int part = pk.partner();
+            for (long long g = g0; g < g1; ++g) {
+                const int k = (int)(g - g0);
+                out[g - P.base[0]] = (part >= 0 && (k == pk.lead || k == part)) ? 1 : 0;
+            }
+        }
+    }
+};
+
+template <bool HAS_MASK>
+__global__ void __launch_bounds__(256, 4) oppsign_stream_kernel(const __grid_constant__ TileParams P, OppSignOp<HAS_MASK> op)
+{
+    tile_stream<typename OppSignOp<HAS_MASK>::Shape>(P, op);
+}
+
 }  // namespace dev
 
 // ------------------------------------------------------------------------------------------ host side
@@ -937,4 +1031,31 @@ extern "C" int32_t hepk_pair_invmass(const float* pt, const float* eta, const fl
     cudaStream_t st = (cudaStream_t)stream;
     if (mask_content) return invmass_launch<true>(L, pt, eta, phi, mass, mask_content, out_mass, out_i1, out_i2, st);
     return invmass_launch<false>(L, pt, eta, phi, mass, mask_content, out_mass, out_i1, out_i2, st);
+}
+
+extern "C" int32_t hepk_select_opposite_sign(const float* pt, const int32_t* charge, const int64_t* offsets, int64_t n_events,
+                                             int64_t content_base, const uint8_t* mask_rows, const uint8_t* mask_content,
+                                             uint8_t* out_mask, void* stream)
+{
+    HEPK_REQUIRE(n_events >= 0, "n_events < 0");
+    if (n_events == 0) return HEPK_OK;
+    HEPK_REQUIRE(offsets && charge && out_mask, "offsets/charge/out_mask is NULL");
+    constexpr int CAP = 416;            // objects per 128-event tile (the kernel takes fewer lanes per tile for denser collections)
+    const void* ptr[3] = {pt, charge, mask_content};
+    const int n_cls[4] = {2, mask_content ? 1 : 0, 0, 0};
+    const int64_t* offs[1] = {offsets};
+    const int64_t bases[1] = {content_base};
+    const int caps[1] = {CAP};
+    TileLayout L;
+    const int32_t rc = tile_layout(L, n_events, 1, offs, bases, n_cls, ptr, caps, CAP + 64, 32);
+    if (rc != HEPK_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (mask_content) {
+        dev::OppSignOp<true> op;
+        op.pt = pt; op.charge = charge; op.mask_rows = mask_rows; op.mask = mask_content; op.out = out_mask;
+        return tile_launch(dev::oppsign_stream_kernel<true>, L, op, st);
+    }
+    dev::OppSignOp<false> op;
+    op.pt = pt; op.charge = charge; op.mask_rows = mask_rows; op.mask = nullptr; op.out = out_mask;
+    return tile_launch(dev::oppsign_stream_kernel<false>, L, op, st);
 }
