@@ -142,6 +142,21 @@ __global__ void __launch_bounds__(256) lookup_interp_kernel(const float* __restr
     }
 }
 
+// Slot of an axis (0 underflow, 1 + b, n + 1 overflow / NaN) through the arithmetic bin guess (linear or log2 axis,
+// exact after one +-1 step; binary search otherwise).
+__device__ __forceinline__ int axis_slot(float v, const float* s_e, int n, const AxisGuess& ax)
+{
+    const int b = find_bin_guess(v, s_e, n, ax);
+    int s = 1 + b;
+    s = (v < s_e[0]) ? 0 : s;
+    s = !(v < s_e[n]) ? n + 1 : s;
+    return s;
+}
+
+// Four entries per thread and step (16-byte loads when the pointers allow).  Without weights only the integer counts are
+// accumulated (native shared-memory atomics) and the weighted sums are taken from them when the bins are flushed;
+// with weights the float32 partial sums (compare-and-swap atomics) are flushed into float64 at bounded intervals.
+template <bool VEC>
 __global__ void __launch_bounds__(256) fill_hist2d_kernel(const float* __restrict__ x, const float* __restrict__ y,
                                                           const float* __restrict__ w, long long n,
                                                           const float* __restrict__ edges_x, int nx,
@@ -158,26 +173,51 @@ __global__ void __launch_bounds__(256) fill_hist2d_kernel(const float* __restric
     for (int i = threadIdx.x; i <= ny; i += blockDim.x) s_ey[i] = edges_y[i];
     for (int i = threadIdx.x; i < slots; i += blockDim.x) { s_sumw[i] = 0.f; s_cnt[i] = 0u; }
     __syncthreads();
-    const float lox = s_ex[0], invx = (float)nx / (s_ex[nx] - lox);
-    const float loy = s_ey[0], invy = (float)ny / (s_ey[ny] - loy);
+    const AxisGuess ax = classify_axis(s_ex, nx), ay = classify_axis(s_ey, ny);
+    const bool fsum = acc != nullptr && w != nullptr;          // float partial sums are needed
+    const bool icnt = counts != nullptr || (acc != nullptr && w == nullptr);
     auto flush = [&]() {
         __syncthreads();
         for (int i = threadIdx.x; i < slots; i += blockDim.x) {
-            if (acc) { const float v = s_sumw[i]; if (v != 0.f) { atomicAdd(acc + i, (double)v); s_sumw[i] = 0.f; } }
-            if (counts) { const unsigned int c = s_cnt[i]; if (c) { atomicAdd(counts + i, (unsigned long long)c); s_cnt[i] = 0u; } }
+            if (fsum) { const float v = s_sumw[i]; if (v != 0.f) { atomicAdd(acc + i, (double)v); s_sumw[i] = 0.f; } }
+            if (icnt) {
+                const unsigned int c = s_cnt[i];
+                if (c) {
+                    if (counts) atomicAdd(counts + i, (unsigned long long)c);
+                    if (acc && !w) atomicAdd(acc + i, (double)c);
+                    s_cnt[i] = 0u;
+                }
+            }
         }
         __syncthreads();
     };
+    auto add = [&](float xv, float yv, float wv) {
+        const int s = axis_slot(xv, s_ex, nx, ax) * (ny + 2) + axis_slot(yv, s_ey, ny, ay);
+        if (fsum) red_shared_add_f32(&s_sumw[s], wv);
+        if (icnt) red_shared_add_u32(&s_cnt[s], 1u);
+    };
     const long long stride = (long long)gridDim.x * blockDim.x;
-    const long long iters = (n + stride - 1) / stride;
-    for (long long it = 0; it < iters; ++it) {
-        const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x + it * stride;
-        if (i < n) {
-            const int s = hist_slot(__ldg(x + i), s_ex, nx, lox, invx) * (ny + 2) + hist_slot(__ldg(y + i), s_ey, ny, loy, invy);
-            if (acc) red_shared_add_f32(&s_sumw[s], w ? __ldg(w + i) : 1.f);
-            if (counts) red_shared_add_u32(&s_cnt[s], 1u);
+    const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (VEC) {
+        const long long n4 = n >> 2;
+        const long long iters = (n4 + stride - 1) / stride;
+        for (long long it = 0; it < iters; ++it) {
+            const long long g = t0 + it * stride;
+            if (g < n4) {
+                const float4 xv = __ldg(reinterpret_cast<const float4*>(x) + g), yv = __ldg(reinterpret_cast<const float4*>(y) + g);
+                const float4 wv = w ? __ldg(reinterpret_cast<const float4*>(w) + g) : make_float4(1.f, 1.f, 1.f, 1.f);
+                add(xv.x, yv.x, wv.x); add(xv.y, yv.y, wv.y); add(xv.z, yv.z, wv.z); add(xv.w, yv.w, wv.w);
+            }
+            if (fsum && (it + 1) % 16 == 0) flush();      // bounded float32 partial sums
         }
-        if ((it + 1) % 64 == 0) flush();      // bounded float32 partial sums
+        for (long long i = (n4 << 2) + t0; i < n; i += stride) add(__ldg(x + i), __ldg(y + i), w ? __ldg(w + i) : 1.f);
+    } else {
+        const long long iters = (n + stride - 1) / stride;
+        for (long long it = 0; it < iters; ++it) {
+            const long long i = t0 + it * stride;
+            if (i < n) add(__ldg(x + i), __ldg(y + i), w ? __ldg(w + i) : 1.f);
+            if (fsum && (it + 1) % 64 == 0) flush();
+        }
     }
     flush();
 }
@@ -238,11 +278,13 @@ extern "C" int32_t hepk_fill_histogram_2d(const float* x, const float* y, const 
     }
     cudaStream_t st = (cudaStream_t)stream;
     const size_t smem = ((size_t)(nx + 1) + (size_t)(ny + 1) + 2 * (size_t)slots) * 4;
-    HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::fill_hist2d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const bool vec = aligned16(x) && aligned16(y) && (!weights || aligned16(weights));
+    auto kern = vec ? dev::fill_hist2d_kernel<true> : dev::fill_hist2d_kernel<false>;
+    HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (sumw) HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)slots * sizeof(double), st));
     unsigned grid = grid_for((n + 3) / 4);
-    dev::fill_hist2d_kernel<<<grid, 256, smem, st>>>(x, y, weights, n, edges_x, nx, edges_y, ny, sumw ? (double*)workspace : nullptr,
-                                                     (unsigned long long*)counts); count_launch();
+    kern<<<grid, 256, smem, st>>>(x, y, weights, n, edges_x, nx, edges_y, ny, sumw ? (double*)workspace : nullptr,
+                                  (unsigned long long*)counts); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     if (sumw) {
         dev::hist2d_finalize<<<(unsigned)((slots + 255) / 256), 256, 0, st>>>(sumw, (const double*)workspace, (int)slots); count_launch();
