@@ -227,6 +227,17 @@ __device__ __forceinline__ int find_bin_guess(float v, const float* edges, int n
     return (v != v) ? n - 1 : g;
 }
 
+// Slot of an axis (0 underflow, 1 + b, n + 1 overflow / NaN) through the arithmetic bin guess (linear or log2 axis,
+// exact after one +-1 step; binary search otherwise).
+__device__ __forceinline__ int axis_slot(float v, const float* s_e, int n, const AxisGuess& ax)
+{
+    const int b = find_bin_guess(v, s_e, n, ax);
+    int s = 1 + b;
+    s = (v < s_e[0]) ? 0 : s;
+    s = !(v < s_e[n]) ? n + 1 : s;
+    return s;
+}
+
 // Histogram slot: 0 underflow, 1+b, nbins+1 overflow/NaN.  Arithmetic guess for (near-)uniform axes,
 // verified against the edges; anything the guess gets wrong falls back to the binary search, so the
 // result is exact for any ascending edges.

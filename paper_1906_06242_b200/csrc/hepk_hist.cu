@@ -88,13 +88,16 @@ __global__ void __launch_bounds__(256) hist_fill_kernel(const __grid_constant__ 
     __syncthreads();
     const float sc = s_sc[0], sc2 = s_sc[1];
     const bool fixed = sc != 0.0f;
-    const float lox = s_ex[0], invx = (float)P.nx / (s_ex[P.nx] - lox);
-    const float loy = P.ny > 0 ? s_ey[0] : 0.0f, invy = P.ny > 0 ? (float)P.ny / (s_ey[P.ny] - loy) : 0.0f;
+    // arithmetic bin guess on linear or log2 axes (exact after one +-1 step), binary search otherwise
+    const AxisGuess ax = classify_axis(s_ex, P.nx);
+    AxisGuess ay;
+    ay.mode = 0; ay.lo = 0.f; ay.inv = 0.f;
+    if (P.ny > 0) ay = classify_axis(s_ey, P.ny);
     const uint32_t bins_a = smem_u32(s_bins);
 
     auto add = [&](float xv, float yv, float wv) {
-        int s = hist_slot(xv, s_ex, P.nx, lox, invx);
-        if (P.ny > 0) s = s * (P.ny + 2) + hist_slot(yv, s_ey, P.ny, loy, invy);
+        int s = axis_slot(xv, s_ex, P.nx, ax);
+        if (P.ny > 0) s = s * (P.ny + 2) + axis_slot(yv, s_ey, P.ny, ay);
         int* row = s_bins + s * P.WS;
         if (fixed) {
             if (P.want_sumw) red_shared_add_u32(row, (unsigned int)__float2int_rn(wv * sc));

@@ -142,17 +142,6 @@ __global__ void __launch_bounds__(256) lookup_interp_kernel(const float* __restr
     }
 }
 
-// Slot of an axis (0 underflow, 1 + b, n + 1 overflow / NaN) through the arithmetic bin guess (linear or log2 axis,
-// exact after one +-1 step; binary search otherwise).
-__device__ __forceinline__ int axis_slot(float v, const float* s_e, int n, const AxisGuess& ax)
-{
-    const int b = find_bin_guess(v, s_e, n, ax);
-    int s = 1 + b;
-    s = (v < s_e[0]) ? 0 : s;
-    s = !(v < s_e[n]) ? n + 1 : s;
-    return s;
-}
-
 // Four entries per thread and step (16-byte loads when the pointers allow).  Without weights only the integer counts are
 // accumulated (native shared-memory atomics) and the weighted sums are taken from them when the bins are flushed;
 // with weights the float32 partial sums (compare-and-swap atomics) are flushed into float64 at bounded intervals.
