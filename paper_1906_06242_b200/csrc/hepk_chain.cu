@@ -1394,7 +1394,7 @@ static int chain_region_layout(ChainParams& P, const hepk_chain_desc* d, bool ca
 }
 
 // plan_warps != nullptr: only work out the CTA shape (warps per SM; 0 = does not fit) and return.
-static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStream_t st, int* plan_warps)
+static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStream_t st, int* plan_warps, bool keep_weight_range = false)
 {
     if (plan_warps) *plan_warps = 0;
     ChainParams P;
@@ -1603,7 +1603,11 @@ static int32_t chain_launch(const hepk_chain_desc* d, void* workspace, cudaStrea
     if (grid > need) grid = need;
     if (grid < 1) grid = 1;
 
-    if (want_hist) {
+    if (want_hist && keep_weight_range) {
+        // a later group of variants of the same call: the weights (and their range in the header) are the same
+        HEPK_CUDA_TRY(cudaMemsetAsync(P.hist_hdr + HDR_TILE, 0, 4, st));
+        HEPK_CUDA_TRY(cudaMemsetAsync(P.hist_acc, 0, (size_t)n_words * 8, st));
+    } else if (want_hist) {
         HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, HDR_WORDS * 4 + (size_t)n_words * 8, st));
         const long long nw = (long long)P.W * P.n_events;
         long long blocks = (nw + 256 * 8 - 1) / (256 * 8);
@@ -1679,7 +1683,7 @@ extern "C" int32_t hepk_analysis_chain(const hepk_chain_desc* d, void* workspace
         if (t.hist_sumw) t.hist_sumw += v0 * spv * W;
         if (t.hist_sumw2) t.hist_sumw2 += v0 * spv * W;
         if (t.hist_counts) t.hist_counts += v0 * spv;
-        const int32_t r = chain_launch(&t, workspace, (cudaStream_t)stream, nullptr);
+        const int32_t r = chain_launch(&t, workspace, (cudaStream_t)stream, nullptr, v0 > 0);
         if (r != HEPK_OK) return r;
     }
     return HEPK_OK;
