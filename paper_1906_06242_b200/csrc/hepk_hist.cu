@@ -10,6 +10,7 @@
 // to its 64-bit global accumulator before it can leave the int32 range.  Everything else takes float32 bins
 // (compare-and-swap atomics) flushed into float64 accumulators at bounded intervals.
 #include "hepk_common.cuh"
+#include "hepk_hist_lanes.cuh"
 
 namespace hepk {
 namespace dev {
@@ -282,13 +283,39 @@ static int32_t hist_fill_launch(const char* who, const float* x, const float* y,
     P.sumw = sumw; P.sumw2 = sumw2; P.counts = counts;
     P.fixed_allowed = h.slots * h.WS <= dev::HIST_FIXED_WORDS ? 1 : 0;
     HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, need, st));
+    const bool vec = aligned16(x) && (!y || aligned16(y)) && (!weights || aligned16(weights));
+    if (ny == 0) {
+        // One dimension, few bins: a private copy of the bins per lane (hepk_hist_lanes.cuh) — float32 partial sums of
+        // n / (threads of the grid) <= 32768 entries each, merged in float64; no pass over the weights, no atomics.
+        const int mode = !weights ? 0 : (sumw2 ? 3 : (counts ? (sumw ? 2 : 0) : 1));
+        const size_t head = dev::lane_hist_head_bytes(nx), per_warp = dev::lane_hist_warp_bytes(nx, mode);
+        int warps = (size_t)max_smem_optin() > head ? (int)(((size_t)max_smem_optin() - head) / per_warp) : 0;
+        if (warps > 8) warps = 8;
+        if (warps >= 4 && n >= (1 << 16) && n <= 32768ll * sm_count() * warps * 32) {
+            void (*k)(const float*, const float*, long long, const float*, int, dev::LaneHistOut);
+            if (mode == 0) k = vec ? dev::fill_hist_lanes_kernel<0, true, true> : dev::fill_hist_lanes_kernel<0, false, true>;
+            else if (mode == 1) k = vec ? dev::fill_hist_lanes_kernel<1, true, true> : dev::fill_hist_lanes_kernel<1, false, true>;
+            else if (mode == 2) k = vec ? dev::fill_hist_lanes_kernel<2, true, true> : dev::fill_hist_lanes_kernel<2, false, true>;
+            else k = vec ? dev::fill_hist_lanes_kernel<3, true, true> : dev::fill_hist_lanes_kernel<3, false, true>;
+            P.fixed_allowed = 0;                  // the accumulators hold float64 sums
+            dev::LaneHistOut o;
+            o.sumw = nullptr; o.counts = nullptr; o.acc = P.acc;
+            o.WS = h.WS; o.want_sumw = h.want_sumw; o.col_w2 = h.col_w2; o.col_cnt = h.col_cnt;
+            const size_t sm = head + (size_t)warps * per_warp;
+            HEPK_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+            k<<<sm_count(), warps * 32, sm, st>>>(x, weights, n, edges_x, nx, o); count_launch();
+            HEPK_CUDA_TRY(cudaGetLastError());
+            dev::hist_finalize_kernel<<<(unsigned)((h.slots + 255) / 256), 256, 0, st>>>(P); count_launch();
+            HEPK_CUDA_TRY(cudaGetLastError());
+            return HEPK_OK;
+        }
+    }
     if (weights && P.fixed_allowed) {
         static const unsigned int inf_bits = 0x7f800000u;
         HEPK_CUDA_TRY(cudaMemcpyAsync((unsigned int*)workspace + dev::HH_WMIN, &inf_bits, 4, cudaMemcpyHostToDevice, st));
         dev::hist_weight_range_kernel<<<grid_for_items((n + 7) / 8), 256, 0, st>>>(weights, n, (unsigned int*)workspace); count_launch();
         HEPK_CUDA_TRY(cudaGetLastError());
     }
-    const bool vec = aligned16(x) && (!y || aligned16(y)) && (!weights || aligned16(weights));
     auto kern = vec ? dev::hist_fill_kernel<true> : dev::hist_fill_kernel<false>;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
