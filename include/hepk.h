@@ -148,10 +148,11 @@ int32_t hepk_lookup_binned(const float* x, const float* y, int64_t n,
  *   slot(x) = 0 if x < edges[0]; nbins+1 if x >= edges[nbins] or x is NaN; else 1+b with
  *   edges[b] <= x < edges[b+1].   sumw[slot] += w (w = 1 if weights == NULL); counts[slot] += 1.
  * data, weights: float32[n]; edges: float32[nbins+1] ascending; sumw: float32[nbins+2] or NULL;
- * counts: int64[nbins+2] or NULL.  Both outputs accumulate.  Bins are privatised per CTA in shared
- * memory (float32 partial sums) and merged into the caller's float32 array with float atomics, so sumw
- * depends on the merge order in its last bits; hepk_fill_histogram_w2 (below) takes a workspace and merges
- * in 64 bits.  nbins+2 <= 16384, else HEPK_ERR_UNSUPPORTED. */
+ * counts: int64[nbins+2] or NULL.  Both outputs accumulate.  Bins are privatised in shared memory — for
+ * small histograms (up to ~200 bins with both outputs) one copy per LANE, updated without atomics and summed
+ * in float64 per CTA; one copy per CTA with float32 atomics otherwise — and merged into the caller's float32
+ * array with float atomics, so sumw depends on the merge order in its last bits; hepk_fill_histogram_w2
+ * (below) takes a workspace and merges in 64 bits.  nbins+2 <= 16384, else HEPK_ERR_UNSUPPORTED. */
 int32_t hepk_fill_histogram(const float* data, const float* weights, int64_t n,
                             const float* edges, int32_t nbins,
                             float* sumw, int64_t* counts, void* stream);
@@ -321,9 +322,10 @@ int32_t hepk_fill_histogram_2d(const float* x, const float* y, const float* weig
  * hepk_fill_histogram_2d; additionally sumw2[slot] += w*w (w = 1 if weights == NULL, so sumw2 == counts).
  * sumw, sumw2: float32, counts: int64, each nullable, all accumulate.  `workspace`: device buffer of at least
  * hepk_hist_workspace_bytes(nx, ny) bytes (ny = 0 for one dimension; 64-bit accumulators), private to the call
- * until the stream reaches its end.  Tolerance class, same guarantee as the chain's weighted bins: fixed-point
- * bins (exact integer sums) for small histograms whose weights are finite and within a factor 8 of each other,
- * float32 partial sums of at most 32768 entries merged in float64 otherwise.  nbins+2 (resp. (nx+2)*(ny+2))
+ * until the stream reaches its end.  Tolerance class, same guarantee as the chain's weighted bins: float32
+ * partial sums of at most 32768 entries merged in float64 (one dimension with few bins: a private copy of the
+ * bins per lane, hepk_hist_lanes.cuh), or fixed-point bins (exact integer sums) for small histograms whose
+ * weights are finite and within a factor 8 of each other.  nbins+2 (resp. (nx+2)*(ny+2))
  * <= 16384 and rows x columns must fit 200 KB of shared memory, else HEPK_ERR_UNSUPPORTED. */
 size_t  hepk_hist_workspace_bytes(int32_t nx, int32_t ny);
 int32_t hepk_fill_histogram_w2(const float* data, const float* weights, int64_t n, const float* edges, int32_t nbins,

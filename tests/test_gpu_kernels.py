@@ -378,6 +378,41 @@ def test_fill_histogram_concentrated_and_nonuniform(hk):
     assert_exact(to_np(gc), wc)
 
 
+def test_fill_histogram_output_subsets_axes_and_sizes(hk):
+    """The lane-private kernel's cell layouts (counts only, sums only, both), its three axis modes (uniform, log-spaced,
+    irregular), pointers that are not 16-byte aligned, and a histogram too large for lane-private copies (per-CTA
+    bins), all against the oracle; +-inf, NaN and exact edges included."""
+    rng = np.random.default_rng(77)
+    n = 300_007
+    w = rng.normal(1, 0.1, n).astype(np.float32)
+    axes = {
+        "uniform": np.linspace(0, 500, 61).astype(np.float32),
+        "log": np.geomspace(20, 3000, 51).astype(np.float32),
+        "irregular": np.sort(np.concatenate([[0.0], rng.uniform(0, 500, 40), [500.0]])).astype(np.float32),
+        "large": np.linspace(0, 500, 2001).astype(np.float32),
+    }
+    for name, edges in axes.items():
+        x = (rng.exponential(120, n) - 5).astype(np.float32)
+        x[:4] = [np.nan, np.inf, -np.inf, 0.0]
+        x[4:4 + edges.size] = edges
+        ws, wc = hepo.fill_histogram(x, w, edges)
+        us, uc = hepo.fill_histogram(x, None, edges)
+        for shift in (0, 1):
+            xd, wd = (misaligned(x, 1), misaligned(w, 3)) if shift else (dev(x), dev(w))
+            gs, gc = hk.fill_histogram(xd, wd, dev(edges))
+            assert_exact(to_np(gc), wc, name + " counts")
+            assert_tol(to_np(gs), ws, name + " sumw")
+            gs, gc = hk.fill_histogram(xd, wd, dev(edges), want_counts=False)
+            assert gc is None
+            assert_tol(to_np(gs), ws, name + " sumw alone")
+            gs, gc = hk.fill_histogram(xd, wd, dev(edges), want_sumw=False)
+            assert gs is None
+            assert_exact(to_np(gc), wc, name + " counts alone")
+            gs, gc = hk.fill_histogram(xd, None, dev(edges))
+            assert_exact(to_np(gc), uc, name + " unweighted counts")
+            assert_exact(to_np(gs), uc.astype(np.float32), name + " unweighted sumw")
+
+
 # --------------------------------------------------------------------------- dense collections (fewer lanes per tile)
 @pytest.mark.parametrize("mean1,mean2", [(30, 6), (90, 20), (400, 3), (7, 70)])
 def test_jagged_kernels_on_dense_collections(hk, mean1, mean2):
