@@ -65,6 +65,8 @@ def parse_args():
     ap.add_argument("--c4-batches", type=int, default=10, help="batches of the streamed config-4 run (BASELINE.json: 10)")
     ap.add_argument("--single-kernels", action="store_true",
                     help="time each single kernel (SURVEY.md 8(a) rows a1-a6 and the f rows) only; one JSON line")
+    ap.add_argument("--sk-eager", action="store_true",
+                    help="--single-kernels without the CUDA-graph replay (the launch-list pass of the profiler)")
     ap.add_argument("--variants", type=int, default=None,
                     help="configs 3/4: number of calibration variants (scales 1 +- k*0.0025); the paper's full-systematics scenario is 40")
     ap.add_argument("--tune", default="", help="chain tuning knobs, e.g. warps_per_sm=20 (testing only)")
@@ -599,6 +601,8 @@ def single_kernels(args, hk, torch, hepgen, steps=None):
         ms = ms_eager
         timer = "eager"
         try:
+            if getattr(args, "sk_eager", False):
+                raise KeyError("--sk-eager")
             g = torch.cuda.CUDAGraph()
             with torch.cuda.stream(side):
                 fn()
@@ -614,6 +618,8 @@ def single_kernels(args, hk, torch, hepgen, steps=None):
             torch.cuda.synchronize()
             ms, timer = e0.elapsed_time(e1) / reps, "graph replay of %d calls" % reps
             del g
+        except KeyError:
+            timer = "eager (--sk-eager)"
         except RuntimeError as exc:                       # a call that cannot be captured keeps the eager figure
             timer = "eager (capture failed: %s)" % str(exc).splitlines()[0][:80]
             torch.cuda.synchronize()
