@@ -331,6 +331,19 @@ size_t  hepk_hist_workspace_bytes(int32_t nx, int32_t ny);
 int32_t hepk_fill_histogram_w2(const float* data, const float* weights, int64_t n, const float* edges, int32_t nbins,
                                float* sumw, float* sumw2, int64_t* counts, void* workspace, size_t workspace_bytes,
                                void* stream);
+/* hepk_fill_histogram_w2 without a workspace and without any allocation, for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  Same arguments, same results
+ * (same kernels) as hepk_fill_histogram_w2; the 64-bit accumulators live in a device array inside the library,
+ * hepk_static_hist_scratch_bytes() = 164,096 bytes that every GPU loading the library holds until exit.
+ * Limits: nbins <= HEPK_STATIC_HIST_MAX_BINS (4094), else HEPK_ERR_UNSUPPORTED with the reason in
+ * hepk_last_error().  The call makes no cudaMalloc / cudaFree and calls no allocating library routine; it clears the
+ * part of the array it uses, on `stream`, before the fill.  ALL calls on a device share the one array: two calls
+ * that can overlap on the GPU (different streams without an ordering between them, or two host threads) race on it
+ * and corrupt each other's sums — order them, or use hepk_fill_histogram_w2 with a workspace per call. */
+#define HEPK_STATIC_HIST_MAX_BINS 4094
+size_t  hepk_static_hist_scratch_bytes(void);
+int32_t hepk_fill_histogram_w2_static(const float* data, const float* weights, int64_t n, const float* edges, int32_t nbins,
+                                      float* sumw, float* sumw2, int64_t* counts, void* stream);
 int32_t hepk_fill_histogram_2d_w2(const float* x, const float* y, const float* weights, int64_t n,
                                   const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
                                   float* sumw, float* sumw2, int64_t* counts, void* workspace, size_t workspace_bytes,

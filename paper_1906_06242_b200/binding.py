@@ -304,6 +304,22 @@ def fill_histogram_w2(data, weights, edges, sumw=None, sumw2=None, counts=None, 
     return sumw, sumw2, counts
 
 
+def static_hist_scratch_bytes():
+    L = lib()
+    L.hepk_static_hist_scratch_bytes.restype = C.c_size_t
+    return int(L.hepk_static_hist_scratch_bytes())
+
+
+def fill_histogram_w2_static(data, weights, edges, sumw, sumw2, counts, stream=None):
+    """hepk_fill_histogram_w2_static: the caller passes every array (each may be None); nothing is allocated, here
+    or in the library.  Calls on one device share the library's scratch array: do not let two overlap on the GPU."""
+    _check(lib().hepk_fill_histogram_w2_static(_ptr(data, torch.float32), _ptr(weights, torch.float32), C.c_int64(data.numel()),
+                                               _ptr(edges, torch.float32), C.c_int32(edges.numel() - 1),
+                                               _ptr(sumw, torch.float32), _ptr(sumw2, torch.float32), _ptr(counts, torch.int64),
+                                               _stream(stream)), "fill_histogram_w2_static")
+    return sumw, sumw2, counts
+
+
 def fill_histogram_2d_w2(x, y, weights, edges_x, edges_y, sumw=None, sumw2=None, counts=None,
                          want=("sumw", "sumw2", "counts"), stream=None):
     nx, ny = edges_x.numel() - 1, edges_y.numel() - 1

@@ -9,6 +9,8 @@
 // within a factor 8 of each other; every CTA checks all its bins after each step of 1024 entries and moves a bin
 // to its 64-bit global accumulator before it can leave the int32 range.  Everything else takes float32 bins
 // (compare-and-swap atomics) flushed into float64 accumulators at bounded intervals.
+#include <mutex>
+
 #include "hepk_common.cuh"
 #include "hepk_hist_lanes.cuh"
 
@@ -355,6 +357,60 @@ extern "C" int32_t hepk_fill_histogram_w2(const float* data, const float* weight
     HEPK_REQUIRE(n == 0 || data, "data is NULL");
     return hist_fill_launch("hepk_fill_histogram_w2", data, nullptr, weights, n, edges, nbins, nullptr, 0, sumw, sumw2,
                             (long long*)counts, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+// ---- the same fill with its scratch in the library (include/hepk.h: hepk_fill_histogram_w2_static) -------------------
+// For callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+// the 64-bit accumulators live in a file-scope device array instead of a caller's workspace.  Every GPU that loads
+// the library holds the array until exit.  In host code its NAME is a host-side stand-in, not a device address: the
+// address comes from cudaGetSymbolAddress, once per device, with that device current.
+namespace hepk {
+constexpr int STATIC_MAX_SLOTS = HEPK_STATIC_HIST_MAX_BINS + 2;
+constexpr size_t STATIC_SCRATCH_BYTES = ((size_t)dev::HH_WORDS * 4 + (size_t)STATIC_MAX_SLOTS * 5 * 8 + 255) / 256 * 256;
+static __device__ __align__(256) unsigned char g_static_hist_scratch[STATIC_SCRATCH_BYTES];
+
+static std::mutex g_static_mutex;
+static void* g_static_ptr[64];          // per device: the array's device address (nullptr: not asked for yet)
+
+static int32_t static_hist_scratch(void** out)
+{
+    int dev = -1;
+    HEPK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) {
+        set_error("hepk_fill_histogram_w2_static: device %d is beyond the 64 the library keeps track of", dev);
+        return HEPK_ERR_UNSUPPORTED;
+    }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        HEPK_CUDA_TRY(cudaGetSymbolAddress(&p, g_static_hist_scratch));
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return HEPK_OK;
+}
+}  // namespace hepk
+
+extern "C" size_t hepk_static_hist_scratch_bytes(void) { return hepk::STATIC_SCRATCH_BYTES; }
+
+extern "C" int32_t hepk_fill_histogram_w2_static(const float* data, const float* weights, int64_t n, const float* edges,
+                                                 int32_t nbins, float* sumw, float* sumw2, int64_t* counts, void* stream)
+{
+    HEPK_REQUIRE(n >= 0, "n < 0");
+    HEPK_REQUIRE(edges && nbins >= 1, "edges is NULL or nbins < 1");
+    if (nbins > HEPK_STATIC_HIST_MAX_BINS) {
+        set_error("hepk_fill_histogram_w2_static: nbins = %d exceeds the %d bins the library's own scratch holds "
+                  "(use hepk_fill_histogram_w2 with a workspace)", nbins, (int)HEPK_STATIC_HIST_MAX_BINS);
+        return HEPK_ERR_UNSUPPORTED;
+    }
+    HEPK_REQUIRE(n == 0 || data, "data is NULL");
+    void* scratch = nullptr;
+    const int32_t rc = static_hist_scratch(&scratch);
+    if (rc != HEPK_OK) return rc;
+    // (hist_fill_launch clears the part of the scratch it uses on the stream before the fill: the array keeps the
+    // last call's contents)
+    return hist_fill_launch("hepk_fill_histogram_w2_static", data, nullptr, weights, n, edges, nbins, nullptr, 0, sumw, sumw2,
+                            (long long*)counts, scratch, STATIC_SCRATCH_BYTES, (cudaStream_t)stream);
 }
 
 extern "C" int32_t hepk_fill_histogram_2d_w2(const float* x, const float* y, const float* weights, int64_t n,
