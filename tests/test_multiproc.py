@@ -49,9 +49,9 @@ def test_sharded_histograms_equal_whole():
     procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
     for p in procs:
         p.start()
-    counts, sumw, n, (e0, e1) = q.get(timeout=120)
+    counts, sumw, n, (e0, e1) = q.get(timeout=600)      # (a cold `import torch` in two fresh processes can take minutes)
     for p in procs:
-        p.join(timeout=60)
+        p.join(timeout=120)
         assert p.exitcode == 0
     wl = hepgen.generate(3, n_events=4001)
     ref = hepo.analysis_chain(wl, want_mask=False)
