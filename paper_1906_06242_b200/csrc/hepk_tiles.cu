@@ -378,14 +378,29 @@ struct ReduceOp {
         // count over a mask: a flat pass turns the tile's mask bytes into a bit string (one ballot per 32 elements), and
         // an event's count is the population count of its bit range
         constexpr bool BITS = OP == OP_COUNT && HAS_MASK;
+        unsigned bit0 = 0;                    // bit of the tile's first element in the string
         if (BITS) {
-            int j0 = 0;
-            for (; j0 < cnt[0]; j0 += 32) {
-                const int j = j0 + lane;
-                const unsigned w = __ballot_sync(0xffffffffu, j < cnt[0] && lds_b(ca[0] + (unsigned)j) != 0u);
-                if (lane == 0) sts_w(extra_a + 4u * (unsigned)(j0 >> 5), w);
+            // Four mask bytes per lane (one 32-bit load from the 4-byte-aligned address at or below the first element),
+            // folded into a nibble; the nibbles of eight neighbouring lanes make a word of the string.  Bits of bytes
+            // in front of the first element or behind the last one are whatever the buffer holds: no range covers them.
+            bit0 = ca[0] & 3u;
+            const uint32_t a4 = ca[0] - bit0;
+            const int nb = cnt[0] + (int)bit0;
+            const unsigned shl = 4u * ((unsigned)lane & 7u);
+            uint32_t wa = extra_a + 4u * ((unsigned)lane >> 3);
+            int i0 = 0;
+            for (; i0 < nb; i0 += 128, wa += 16u) {
+                const int i = i0 + 4 * lane;
+                unsigned w = 0u;
+                if (i < nb) w = lds_w(a4 + (unsigned)i);
+                const unsigned t = (w | ((w & 0x7f7f7f7fu) + 0x7f7f7f7fu)) & 0x80808080u;      // high bit of every non-zero byte
+                unsigned v = (((t >> 7) * 0x01020408u) >> 24) << shl;                            // ... gathered: bit b = byte b
+                v |= __shfl_xor_sync(0xffffffffu, v, 1);
+                v |= __shfl_xor_sync(0xffffffffu, v, 2);
+                v |= __shfl_xor_sync(0xffffffffu, v, 4);
+                if (((unsigned)lane & 7u) == 0u) sts_w(wa, v);
             }
-            if (lane == 0) sts_w(extra_a + 4u * (unsigned)(j0 >> 5), 0u);        // (a range may end exactly at a word boundary)
+            if (lane == 0) sts_w(extra_a + 4u * (unsigned)(i0 >> 5), 0u);        // (a range may end exactly at a word boundary)
             __syncwarp();
         }
         constexpr int TAIL = 16;          // elements of an event beyond this many are reduced by the whole warp
@@ -414,7 +429,7 @@ struct ReduceOp {
             if (!DATA && !HAS_MASK) {
                 acc.i = n;
             } else if (BITS) {
-                int pos = o[0][h] - lo[0], rem = n, c = 0;
+                int pos = o[0][h] - lo[0] + (int)bit0, rem = n, c = 0;
                 while (rem > 0) {
                     const int take = rem < 32 ? rem : 32;
                     const uint32_t wa = extra_a + 4u * (unsigned)(pos >> 5);
@@ -464,10 +479,11 @@ struct ReduceOp {
         }
         // a lane's H results are neighbours in memory: one vector store when the whole group is live
         typename RedOut<OP>::type* dst = out + e0 + lane * H;
-        typedef typename std::conditional<H == 4, int4, int2>::type V;
-        static_assert(H == 2 || H == 4, "the vector store covers 2 or 4 results");
+        typedef typename std::conditional<H >= 4, int4, int2>::type V;
+        static_assert(H == 2 || H == 4 || H == 8, "the vector stores cover 2, 4 or 8 results");
         if (lane * H + H <= ne && (reinterpret_cast<uintptr_t>(dst) & (sizeof(V) - 1)) == 0) {
-            *reinterpret_cast<V*>(dst) = *reinterpret_cast<const V*>(res);
+#pragma unroll
+            for (int q = 0; q < (int)(H * 4 / sizeof(V)); ++q) reinterpret_cast<V*>(dst)[q] = reinterpret_cast<const V*>(res)[q];
         } else {
 #pragma unroll
             for (int h = 0; h < H; ++h)
