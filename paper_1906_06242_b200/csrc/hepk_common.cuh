@@ -238,6 +238,67 @@ __device__ __forceinline__ int axis_slot(float v, const float* s_e, int n, const
     return s;
 }
 
+// ---- padded axes: the +-1 step with no clamps, range tests or NaN selects ------------------------------
+// A second copy of the edges whose ends absorb every special case, so that the guess needs one fused multiply-add, a
+// float clamp, a conversion, two loads and two compare-and-adjust steps (13 instructions; find_bin_guess / axis_slot
+// take 25-30 with their range tests, clamps and NaN selects, and a run-time mode test).
+//   SLOTS (histograms):  pad[0] = -inf, pad[1 + i] = edges[i] (i = 0..n), pad[n + 2] = NaN;
+//                        slot s in [0, n + 1] is the one with pad[s] <= v < pad[s + 1]   (0 underflow, n + 1 overflow)
+//   bins (clamped lookups): pad[0] = -inf, pad[i] = edges[i] (i = 1..n-1), pad[n] = NaN;
+//                        bin b in [0, n - 1] is the one with pad[b] <= v < pad[b + 1]     (B(v) of find_bin_clamped)
+// No comparison with NaN is true, so the last slot / bin takes everything at or beyond the last edge, and a NaN value
+// (guess = top through fminf(NaN, top) = top, no comparison moves it) lands there too, as the readings R5 / R9 ask.
+// The guess is floor of the position in slot units, good to +-1 on an axis classify_axis accepted (mode 1 or 2), and
+// the step against the REAL edges makes the result exact.  AXIS is the mode, fixed at compile time by the caller;
+// AXIS == 0 takes the general functions above on the unpadded edges.
+template <bool SLOTS>
+__device__ __forceinline__ int pad_axis_words(int n) { return SLOTS ? n + 3 : n + 1; }
+
+template <bool SLOTS>
+__device__ __forceinline__ void pad_axis_fill(float* s_pad, const float* __restrict__ edges, int n)     // all threads of the CTA
+{
+    const int last = SLOTS ? n + 2 : n;
+    for (int i = threadIdx.x; i <= last; i += blockDim.x)
+        s_pad[i] = i == 0 ? -CUDART_INF_F : (i == last ? CUDART_NAN_F : edges[SLOTS ? i - 1 : i]);
+}
+
+// top = (float)(n + 1) for slots, (float)(n - 1) for bins
+template <int AXIS, bool SLOTS>
+__device__ __forceinline__ int pad_axis_find(float v, const float* s_edges, const float* s_pad, int n, const AxisGuess& a, float top)
+{
+    if (AXIS == 0) return SLOTS ? axis_slot(v, s_edges, n, a) : find_bin_guess(v, s_edges, n, a);
+    const float one = SLOTS ? 1.0f : 0.0f;
+    float pos;
+    if (AXIS == 1) pos = fmaf(v - a.lo, a.inv, one);
+    else pos = v > 0.0f ? fmaf(__log2f(v) - a.lo, a.inv, one) : (v != v ? top : 0.0f);
+    int s = (int)fmaxf(fminf(pos, top), 0.0f);
+    const float e0 = s_pad[s], e1 = s_pad[s + 1];
+    s += (v >= e1) ? 1 : 0;
+    s -= (v < e0) ? 1 : 0;
+    return s;
+}
+
+// Calls f(tag_x, tag_y) with the axis modes as compile-time tags when both axes have an arithmetic guess, and with
+// (0, 0) (the general functions, which test the mode at run time) otherwise.  The modes are uniform over the CTA.
+template <int N> struct AxisTag { static constexpr int value = N; };
+template <class F>
+__device__ __forceinline__ void dispatch_axes(int mode_x, int mode_y, F&& f)
+{
+    if (mode_x == 1 && mode_y == 1) f(AxisTag<1>{}, AxisTag<1>{});
+    else if (mode_x == 1 && mode_y == 2) f(AxisTag<1>{}, AxisTag<2>{});
+    else if (mode_x == 2 && mode_y == 1) f(AxisTag<2>{}, AxisTag<1>{});
+    else if (mode_x == 2 && mode_y == 2) f(AxisTag<2>{}, AxisTag<2>{});
+    else f(AxisTag<0>{}, AxisTag<0>{});
+}
+
+template <class F>
+__device__ __forceinline__ void dispatch_axis(int mode, F&& f)
+{
+    if (mode == 1) f(AxisTag<1>{});
+    else if (mode == 2) f(AxisTag<2>{});
+    else f(AxisTag<0>{});
+}
+
 // Histogram slot: 0 underflow, 1+b, nbins+1 overflow/NaN.  Arithmetic guess for (near-)uniform axes,
 // verified against the edges; anything the guess gets wrong falls back to the binary search, so the
 // result is exact for any ascending edges.

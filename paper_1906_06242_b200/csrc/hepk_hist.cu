@@ -84,9 +84,13 @@ __global__ void __launch_bounds__(256) hist_fill_kernel(const __grid_constant__ 
     int* s_bins = (int*)(s_ey + (P.ny > 0 ? P.ny + 1 : 0));
     __shared__ float s_sc[2];
     const int n_words = P.slots * P.WS;
+    float* s_px = (float*)(s_bins + n_words);      // padded copies of the edges (pad_axis_find, slot form)
+    float* s_py = s_px + (P.nx + 3);
     for (int i = threadIdx.x; i <= P.nx; i += blockDim.x) s_ex[i] = P.edges_x[i];
     if (P.ny > 0) for (int i = threadIdx.x; i <= P.ny; i += blockDim.x) s_ey[i] = P.edges_y[i];
     for (int i = threadIdx.x; i < n_words; i += blockDim.x) s_bins[i] = 0;
+    pad_axis_fill<true>(s_px, P.edges_x, P.nx);
+    if (P.ny > 0) pad_axis_fill<true>(s_py, P.edges_y, P.ny);
     if (threadIdx.x == 0) hist_fill_scales(P, s_sc[0], s_sc[1]);
     __syncthreads();
     const float sc = s_sc[0], sc2 = s_sc[1];
@@ -94,28 +98,10 @@ __global__ void __launch_bounds__(256) hist_fill_kernel(const __grid_constant__ 
     // arithmetic bin guess on linear or log2 axes (exact after one +-1 step), binary search otherwise
     const AxisGuess ax = classify_axis(s_ex, P.nx);
     AxisGuess ay;
-    ay.mode = 0; ay.lo = 0.f; ay.inv = 0.f;
+    ay.mode = 1; ay.lo = 0.f; ay.inv = 0.f;        // (one dimension: the tag of the unused axis)
     if (P.ny > 0) ay = classify_axis(s_ey, P.ny);
-    const uint32_t bins_a = smem_u32(s_bins);
+    const float top_x = (float)(P.nx + 1), top_y = (float)(P.ny + 1);
 
-    auto add = [&](float xv, float yv, float wv) {
-        int s = axis_slot(xv, s_ex, P.nx, ax);
-        if (P.ny > 0) s = s * (P.ny + 2) + axis_slot(yv, s_ey, P.ny, ay);
-        int* row = s_bins + s * P.WS;
-        if (fixed) {
-            if (P.want_sumw) red_shared_add_u32(row, (unsigned int)__float2int_rn(wv * sc));
-            if (P.col_w2 >= 0) {
-                const float y2 = wv * wv * sc2;
-                const int qh = __float2int_rn(y2);
-                red_shared_add_u32(row + P.col_w2, (unsigned int)qh);
-                red_shared_add_u32(row + P.col_w2 + 1, (unsigned int)__float2int_rn((y2 - (float)qh) * 1048576.0f));
-            }
-        } else {
-            if (P.want_sumw) red_shared_add_f32(row, wv);
-            if (P.col_w2 >= 0) red_shared_add_f32(row + P.col_w2, wv * wv);
-        }
-        if (P.col_cnt >= 0) red_shared_add_u32(row + P.col_cnt, 1u);
-    };
     // move bins into the global accumulators; `all`: everything non-zero, else only integers about to overflow
     auto flush = [&](bool all) {
         for (int i = threadIdx.x; i < n_words; i += blockDim.x) {
@@ -132,34 +118,59 @@ __global__ void __launch_bounds__(256) hist_fill_kernel(const __grid_constant__ 
             }
         }
     };
-    (void)bins_a;
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     // fixed point: a step adds at most 1024 entries < 2^19 each to a bin, so a check per step keeps |bin| < 2^31;
     // float: bounded partial sums (a flush every 32 steps)
     const int check_every = fixed ? 1 : 32;
-    if (VEC) {
-        const long long n4 = P.n / 4;
-        const long long iters = (n4 + stride - 1) / stride;
-        for (long long it = 0; it < iters; ++it) {
-            const long long g = t0 + it * stride;
-            if (g < n4) {
-                const float4 xv = __ldg((const float4*)P.x + g);
-                const float4 yv = P.ny > 0 ? __ldg((const float4*)P.y + g) : make_float4(0.f, 0.f, 0.f, 0.f);
-                const float4 wv = P.w ? __ldg((const float4*)P.w + g) : make_float4(1.f, 1.f, 1.f, 1.f);
-                add(xv.x, yv.x, wv.x); add(xv.y, yv.y, wv.y); add(xv.z, yv.z, wv.z); add(xv.w, yv.w, wv.w);
+    dispatch_axes(ax.mode, ay.mode, [&](auto tx, auto ty) {
+        constexpr int AX = decltype(tx)::value, AY = decltype(ty)::value;
+        auto slot_of = [&](float xv, float yv) {
+            int s = pad_axis_find<AX, true>(xv, s_ex, s_px, P.nx, ax, top_x);
+            if (P.ny > 0) s = s * (P.ny + 2) + pad_axis_find<AY, true>(yv, s_ey, s_py, P.ny, ay, top_y);
+            return s;
+        };
+        auto put = [&](int s, float wv) {
+            int* row = s_bins + s * P.WS;
+            if (fixed) {
+                if (P.want_sumw) red_shared_add_u32(row, (unsigned int)__float2int_rn(wv * sc));
+                if (P.col_w2 >= 0) {
+                    const float y2 = wv * wv * sc2;
+                    const int qh = __float2int_rn(y2);
+                    red_shared_add_u32(row + P.col_w2, (unsigned int)qh);
+                    red_shared_add_u32(row + P.col_w2 + 1, (unsigned int)__float2int_rn((y2 - (float)qh) * 1048576.0f));
+                }
+            } else {
+                if (P.want_sumw) red_shared_add_f32(row, wv);
+                if (P.col_w2 >= 0) red_shared_add_f32(row + P.col_w2, wv * wv);
             }
-            if ((it + 1) % check_every == 0) flush(!fixed);
+            if (P.col_cnt >= 0) red_shared_add_u32(row + P.col_cnt, 1u);
+        };
+        if (VEC) {
+            const long long n4 = P.n / 4;
+            const long long iters = (n4 + stride - 1) / stride;
+            for (long long it = 0; it < iters; ++it) {
+                const long long g = t0 + it * stride;
+                if (g < n4) {
+                    const float4 xv = __ldg((const float4*)P.x + g);
+                    const float4 yv = P.ny > 0 ? __ldg((const float4*)P.y + g) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    const float4 wv = P.w ? __ldg((const float4*)P.w + g) : make_float4(1.f, 1.f, 1.f, 1.f);
+                    // all four slots before the first update (an edge load cannot move across a shared-memory atomic)
+                    const int s0 = slot_of(xv.x, yv.x), s1 = slot_of(xv.y, yv.y), s2 = slot_of(xv.z, yv.z), s3 = slot_of(xv.w, yv.w);
+                    put(s0, wv.x); put(s1, wv.y); put(s2, wv.z); put(s3, wv.w);
+                }
+                if ((it + 1) % check_every == 0) flush(!fixed);
+            }
+            for (long long i = n4 * 4 + t0; i < P.n; i += stride) put(slot_of(P.x[i], P.ny > 0 ? P.y[i] : 0.f), P.w ? P.w[i] : 1.f);
+        } else {
+            const long long iters = (P.n + stride - 1) / stride;
+            for (long long it = 0; it < iters; ++it) {
+                const long long i = t0 + it * stride;
+                if (i < P.n) put(slot_of(P.x[i], P.ny > 0 ? P.y[i] : 0.f), P.w ? P.w[i] : 1.f);
+                if ((it + 1) % (4 * check_every) == 0) flush(!fixed);
+            }
         }
-        for (long long i = n4 * 4 + t0; i < P.n; i += stride) add(P.x[i], P.ny > 0 ? P.y[i] : 0.f, P.w ? P.w[i] : 1.f);
-    } else {
-        const long long iters = (P.n + stride - 1) / stride;
-        for (long long it = 0; it < iters; ++it) {
-            const long long i = t0 + it * stride;
-            if (i < P.n) add(P.x[i], P.ny > 0 ? P.y[i] : 0.f, P.w ? P.w[i] : 1.f);
-            if ((it + 1) % (4 * check_every) == 0) flush(!fixed);
-        }
-    }
+    });
     __syncthreads();
     flush(true);
 }
@@ -192,31 +203,36 @@ __global__ void __launch_bounds__(256) event_weight_lookup_kernel(const float* _
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* s_e = (float*)smem_raw;
     float* s_t = s_e + (nb + 1);
+    float* s_p = s_t + nb;                          // padded copy of the edges (pad_axis_find, bin form)
     for (int i = threadIdx.x; i <= nb; i += blockDim.x) s_e[i] = edges[i];
     for (int i = threadIdx.x; i < nb; i += blockDim.x) s_t[i] = table[i];
     __syncthreads();
-    const AxisGuess ax = classify_axis(s_e, nb);
+    pad_axis_fill<false>(s_p, s_e, nb);
+    const AxisGuess ax = classify_axis(s_e, nb);      // (its barriers publish s_p)
+    const float top = (float)(nb - 1);
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool vec = ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(w_out) | reinterpret_cast<uintptr_t>(w_in)) & 15u) == 0;
-    if (vec) {
-        const long long n4 = n / 4;
-        for (long long g = t0; g < n4; g += stride) {
-            const float4 xv = __ldg((const float4*)x + g);
-            const float4 wv = w_in ? __ldg((const float4*)w_in + g) : make_float4(1.f, 1.f, 1.f, 1.f);
-            float4 o;
-            o.x = __fmul_rn(wv.x, s_t[find_bin_guess(xv.x, s_e, nb, ax)]);
-            o.y = __fmul_rn(wv.y, s_t[find_bin_guess(xv.y, s_e, nb, ax)]);
-            o.z = __fmul_rn(wv.z, s_t[find_bin_guess(xv.z, s_e, nb, ax)]);
-            o.w = __fmul_rn(wv.w, s_t[find_bin_guess(xv.w, s_e, nb, ax)]);
-            ((float4*)w_out)[g] = o;
+    dispatch_axis(ax.mode, [&](auto tx) {
+        constexpr int AX = decltype(tx)::value;
+        auto factor = [&](float v) { return s_t[pad_axis_find<AX, false>(v, s_e, s_p, nb, ax, top)]; };
+        if (vec) {
+            const long long n4 = n / 4;
+            for (long long g = t0; g < n4; g += stride) {
+                const float4 xv = __ldg((const float4*)x + g);
+                const float4 wv = w_in ? __ldg((const float4*)w_in + g) : make_float4(1.f, 1.f, 1.f, 1.f);
+                float4 o;
+                o.x = __fmul_rn(wv.x, factor(xv.x));
+                o.y = __fmul_rn(wv.y, factor(xv.y));
+                o.z = __fmul_rn(wv.z, factor(xv.z));
+                o.w = __fmul_rn(wv.w, factor(xv.w));
+                ((float4*)w_out)[g] = o;
+            }
+            for (long long i = n4 * 4 + t0; i < n; i += stride) w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, factor(x[i]));
+        } else {
+            for (long long i = t0; i < n; i += stride) w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, factor(x[i]));
         }
-        for (long long i = n4 * 4 + t0; i < n; i += stride)
-            w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, s_t[find_bin_guess(x[i], s_e, nb, ax)]);
-    } else {
-        for (long long i = t0; i < n; i += stride)
-            w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, s_t[find_bin_guess(x[i], s_e, nb, ax)]);
-    }
+    });
 }
 
 // measurement hook: lane-atomics of red.shared.add.s32 per launch, random addresses in `nbins` words
@@ -271,7 +287,7 @@ static int32_t hist_fill_launch(const char* who, const float* x, const float* y,
         set_error("%s: workspace is NULL or smaller than %zu bytes", who, need);
         return HEPK_ERR_INVALID;
     }
-    const size_t smem = ((size_t)(nx + 1) + (ny > 0 ? (size_t)(ny + 1) : 0) + (size_t)h.slots * h.WS) * 4;
+    const size_t smem = ((size_t)(nx + 1) + (ny > 0 ? (size_t)(ny + 1) : 0) + (size_t)h.slots * h.WS + (size_t)(nx + 3) + (size_t)(ny > 0 ? ny + 3 : 0)) * 4;
     if (smem > 200 * 1024) {
         set_error("%s: %d slots x %d columns do not fit 200 KB of shared memory", who, h.slots, h.WS);
         return HEPK_ERR_UNSUPPORTED;
@@ -440,7 +456,7 @@ extern "C" int32_t hepk_event_weight_lookup(const float* w_in, const float* x, i
     }
     if (n == 0) return HEPK_OK;
     HEPK_REQUIRE(x && w_out, "x/w_out is NULL");
-    const size_t smem = (size_t)(2 * nbins + 1) * 4;
+    const size_t smem = (size_t)(3 * nbins + 2) * 4;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::event_weight_lookup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dev::event_weight_lookup_kernel<<<grid_for_items((n + 3) / 4), 256, smem, (cudaStream_t)stream>>>(w_in, x, n, edges, nbins,
                                                                                                     table, w_out); count_launch();

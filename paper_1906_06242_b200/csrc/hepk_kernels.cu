@@ -69,35 +69,43 @@ __global__ void __launch_bounds__(256) lookup_kernel(const float* __restrict__ x
     float* s_ey = s_ex + (nx + 1);
     float* s_t = s_ey + (y ? ny + 1 : 0);
     const int nyy = y ? ny : 1;
+    float* s_px = s_t + nx * nyy;              // padded copies of the edges (pad_axis_find, bin form)
+    float* s_py = s_px + (nx + 1);
     for (int i = threadIdx.x; i <= nx; i += blockDim.x) s_ex[i] = edges_x[i];
     if (y) for (int i = threadIdx.x; i <= ny; i += blockDim.x) s_ey[i] = edges_y[i];
     for (int i = threadIdx.x; i < nx * nyy; i += blockDim.x) s_t[i] = table[i];
+    pad_axis_fill<false>(s_px, edges_x, nx);
+    if (y) pad_axis_fill<false>(s_py, edges_y, ny);
     __syncthreads();
     const AxisGuess ax = classify_axis(s_ex, nx);
     AxisGuess ay;
-    ay.mode = 0; ay.lo = 0.f; ay.inv = 0.f;
+    ay.mode = 1; ay.lo = 0.f; ay.inv = 0.f;
     if (y) ay = classify_axis(s_ey, ny);
-    auto look = [&](float xv, float yv) {
-        const int bx = find_bin_guess(xv, s_ex, nx, ax);
-        const int by = y ? find_bin_guess(yv, s_ey, ny, ay) : 0;
-        return s_t[bx * nyy + by];
-    };
+    const float top_x = (float)(nx - 1), top_y = (float)(ny - 1);
     const long long stride = (long long)gridDim.x * blockDim.x;
-    if (VEC) {
-        const long long n4 = n / 4;
-        for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < n4; g += stride) {
-            const float4 xv = __ldg((const float4*)x + g);
-            const float4 yv = y ? __ldg((const float4*)y + g) : make_float4(0.f, 0.f, 0.f, 0.f);
-            float4 r;
-            r.x = look(xv.x, yv.x); r.y = look(xv.y, yv.y); r.z = look(xv.z, yv.z); r.w = look(xv.w, yv.w);
-            ((float4*)out)[g] = r;
+    dispatch_axes(ax.mode, ay.mode, [&](auto tx, auto ty) {
+        constexpr int AX = decltype(tx)::value, AY = decltype(ty)::value;
+        auto look = [&](float xv, float yv) {
+            const int bx = pad_axis_find<AX, false>(xv, s_ex, s_px, nx, ax, top_x);
+            const int by = y ? pad_axis_find<AY, false>(yv, s_ey, s_py, ny, ay, top_y) : 0;
+            return s_t[bx * nyy + by];
+        };
+        if (VEC) {
+            const long long n4 = n / 4;
+            for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < n4; g += stride) {
+                const float4 xv = __ldg((const float4*)x + g);
+                const float4 yv = y ? __ldg((const float4*)y + g) : make_float4(0.f, 0.f, 0.f, 0.f);
+                float4 r;
+                r.x = look(xv.x, yv.x); r.y = look(xv.y, yv.y); r.z = look(xv.z, yv.z); r.w = look(xv.w, yv.w);
+                ((float4*)out)[g] = r;
+            }
+            for (long long i = n4 * 4 + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+                out[i] = look(x[i], y ? y[i] : 0.f);
+        } else {
+            for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+                out[i] = look(x[i], y ? y[i] : 0.f);
         }
-        for (long long i = n4 * 4 + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-            out[i] = look(x[i], y ? y[i] : 0.f);
-    } else {
-        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-            out[i] = look(x[i], y ? y[i] : 0.f);
-    }
+    });
 }
 
 // =========================================================================================== fill_histogram
@@ -202,7 +210,7 @@ extern "C" int32_t hepk_lookup_binned(const float* x, const float* y, int64_t n,
     HEPK_REQUIRE(!y || (edges_y && ny >= 1), "edges_y is NULL or ny < 1");
     if (n == 0) return HEPK_OK;
     HEPK_REQUIRE(x && out, "x/out is NULL");
-    const size_t smem = ((size_t)(nx + 1) + (y ? ny + 1 : 0) + (size_t)nx * (y ? ny : 1)) * 4;
+    const size_t smem = (2 * (size_t)(nx + 1) + (y ? 2 * (size_t)(ny + 1) : 0) + (size_t)nx * (y ? ny : 1)) * 4;
     if (smem > 200 * 1024) {
         set_error("hepk_lookup_binned: table of %zu bytes does not fit shared memory", smem);
         return HEPK_ERR_UNSUPPORTED;

@@ -115,31 +115,38 @@ __global__ void __launch_bounds__(256) lookup_interp_kernel(const float* __restr
     __syncthreads();
     for (int i = threadIdx.x; i + 1 < nk; i += blockDim.x) s_m[i] = (s_y[i + 1] - s_y[i]) / (s_x[i + 1] - s_x[i]);
     __syncthreads();
+    float* s_p = s_m + nk;                                 // padded copy of the knots (pad_axis_find, bin form)
+    pad_axis_fill<false>(s_p, xs, nk - 1);
     AxisGuess ax;
     ax.mode = 0; ax.lo = 0.f; ax.inv = 0.f;
-    if (nk >= 2) ax = classify_axis(s_x, nk - 1);          // the knots as the edges of nk - 1 segments
+    if (nk >= 2) ax = classify_axis(s_x, nk - 1);          // the knots as the edges of nk - 1 segments (its barriers publish s_p)
     const float x_lo = s_x[0], x_hi = s_x[nk - 1];
-    auto interp = [&](float v) {
-        if (v != v) return v;
-        if (v <= x_lo) return s_y[0];
-        if (v >= x_hi) return s_y[nk - 1];
-        const int lo = find_bin_guess(v, s_x, nk - 1, ax);  // s_x[lo] <= v < s_x[lo + 1]
-        return fmaf(v - s_x[lo], s_m[lo], s_y[lo]);        // tolerance class: a few float32 roundings
-    };
+    const float y_lo = s_y[0], y_hi = s_y[nk - 1];
+    const float top = (float)(nk - 2);
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (VEC) {
-        const long long n4 = n >> 2;
-        for (long long g = t0; g < n4; g += stride) {
-            const float4 v = __ldg(reinterpret_cast<const float4*>(x) + g);
-            float4 r;
-            r.x = interp(v.x); r.y = interp(v.y); r.z = interp(v.z); r.w = interp(v.w);
-            reinterpret_cast<float4*>(out)[g] = r;
+    dispatch_axis(ax.mode, [&](auto tx) {
+        constexpr int AX = decltype(tx)::value;
+        auto interp = [&](float v) {
+            const int lo = pad_axis_find<AX, false>(v, s_x, s_p, nk - 1, ax, top);  // s_x[lo] <= v < s_x[lo + 1] inside the range
+            float r = fmaf(v - s_x[lo], s_m[lo], s_y[lo]);       // tolerance class: a few float32 roundings
+            r = v <= x_lo ? y_lo : r;
+            r = v >= x_hi ? y_hi : r;
+            return v != v ? v : r;
+        };
+        if (VEC) {
+            const long long n4 = n >> 2;
+            for (long long g = t0; g < n4; g += stride) {
+                const float4 v = __ldg(reinterpret_cast<const float4*>(x) + g);
+                float4 r;
+                r.x = interp(v.x); r.y = interp(v.y); r.z = interp(v.z); r.w = interp(v.w);
+                reinterpret_cast<float4*>(out)[g] = r;
+            }
+            for (long long i = (n4 << 2) + t0; i < n; i += stride) out[i] = interp(__ldg(x + i));
+        } else {
+            for (long long i = t0; i < n; i += stride) out[i] = interp(__ldg(x + i));
         }
-        for (long long i = (n4 << 2) + t0; i < n; i += stride) out[i] = interp(__ldg(x + i));
-    } else {
-        for (long long i = t0; i < n; i += stride) out[i] = interp(__ldg(x + i));
-    }
+    });
 }
 
 // Four entries per thread and step (16-byte loads when the pointers allow).  Without weights only the integer counts are
@@ -158,9 +165,13 @@ __global__ void __launch_bounds__(256) fill_hist2d_kernel(const float* __restric
     float* s_sumw = s_ey + (ny + 1);
     const int slots = (nx + 2) * (ny + 2);
     unsigned int* s_cnt = (unsigned int*)(s_sumw + slots);
+    float* s_px = (float*)(s_cnt + slots);      // padded copies of the edges (pad_axis_find, slot form)
+    float* s_py = s_px + (nx + 3);
     for (int i = threadIdx.x; i <= nx; i += blockDim.x) s_ex[i] = edges_x[i];
     for (int i = threadIdx.x; i <= ny; i += blockDim.x) s_ey[i] = edges_y[i];
     for (int i = threadIdx.x; i < slots; i += blockDim.x) { s_sumw[i] = 0.f; s_cnt[i] = 0u; }
+    pad_axis_fill<true>(s_px, edges_x, nx);
+    pad_axis_fill<true>(s_py, edges_y, ny);
     __syncthreads();
     const AxisGuess ax = classify_axis(s_ex, nx), ay = classify_axis(s_ey, ny);
     const bool fsum = acc != nullptr && w != nullptr;          // float partial sums are needed
@@ -180,34 +191,44 @@ __global__ void __launch_bounds__(256) fill_hist2d_kernel(const float* __restric
         }
         __syncthreads();
     };
-    auto add = [&](float xv, float yv, float wv) {
-        const int s = axis_slot(xv, s_ex, nx, ax) * (ny + 2) + axis_slot(yv, s_ey, ny, ay);
-        if (fsum) red_shared_add_f32(&s_sumw[s], wv);
-        if (icnt) red_shared_add_u32(&s_cnt[s], 1u);
-    };
+    const float top_x = (float)(nx + 1), top_y = (float)(ny + 1);
+    const int row = ny + 2;
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (VEC) {
-        const long long n4 = n >> 2;
-        const long long iters = (n4 + stride - 1) / stride;
-        for (long long it = 0; it < iters; ++it) {
-            const long long g = t0 + it * stride;
-            if (g < n4) {
-                const float4 xv = __ldg(reinterpret_cast<const float4*>(x) + g), yv = __ldg(reinterpret_cast<const float4*>(y) + g);
-                const float4 wv = w ? __ldg(reinterpret_cast<const float4*>(w) + g) : make_float4(1.f, 1.f, 1.f, 1.f);
-                add(xv.x, yv.x, wv.x); add(xv.y, yv.y, wv.y); add(xv.z, yv.z, wv.z); add(xv.w, yv.w, wv.w);
+    dispatch_axes(ax.mode, ay.mode, [&](auto tx, auto ty) {
+        constexpr int AX = decltype(tx)::value, AY = decltype(ty)::value;
+        auto slot_of = [&](float xv, float yv) {
+            return pad_axis_find<AX, true>(xv, s_ex, s_px, nx, ax, top_x) * row + pad_axis_find<AY, true>(yv, s_ey, s_py, ny, ay, top_y);
+        };
+        auto put = [&](int s, float wv) {
+            if (fsum) red_shared_add_f32(&s_sumw[s], wv);
+            if (icnt) red_shared_add_u32(&s_cnt[s], 1u);
+        };
+        if (VEC) {
+            const long long n4 = n >> 2;
+            const long long iters = (n4 + stride - 1) / stride;
+            for (long long it = 0; it < iters; ++it) {
+                const long long g = t0 + it * stride;
+                if (g < n4) {
+                    const float4 xv = __ldg(reinterpret_cast<const float4*>(x) + g), yv = __ldg(reinterpret_cast<const float4*>(y) + g);
+                    const float4 wv = w ? __ldg(reinterpret_cast<const float4*>(w) + g) : make_float4(1.f, 1.f, 1.f, 1.f);
+                    // all four slots before the first update (the updates are opaque to the compiler: an edge load
+                    // cannot move across one)
+                    const int s0 = slot_of(xv.x, yv.x), s1 = slot_of(xv.y, yv.y), s2 = slot_of(xv.z, yv.z), s3 = slot_of(xv.w, yv.w);
+                    put(s0, wv.x); put(s1, wv.y); put(s2, wv.z); put(s3, wv.w);
+                }
+                if (fsum && (it + 1) % 16 == 0) flush();      // bounded float32 partial sums
             }
-            if (fsum && (it + 1) % 16 == 0) flush();      // bounded float32 partial sums
+            for (long long i = (n4 << 2) + t0; i < n; i += stride) put(slot_of(__ldg(x + i), __ldg(y + i)), w ? __ldg(w + i) : 1.f);
+        } else {
+            const long long iters = (n + stride - 1) / stride;
+            for (long long it = 0; it < iters; ++it) {
+                const long long i = t0 + it * stride;
+                if (i < n) put(slot_of(__ldg(x + i), __ldg(y + i)), w ? __ldg(w + i) : 1.f);
+                if (fsum && (it + 1) % 64 == 0) flush();
+            }
         }
-        for (long long i = (n4 << 2) + t0; i < n; i += stride) add(__ldg(x + i), __ldg(y + i), w ? __ldg(w + i) : 1.f);
-    } else {
-        const long long iters = (n + stride - 1) / stride;
-        for (long long it = 0; it < iters; ++it) {
-            const long long i = t0 + it * stride;
-            if (i < n) add(__ldg(x + i), __ldg(y + i), w ? __ldg(w + i) : 1.f);
-            if (fsum && (it + 1) % 64 == 0) flush();
-        }
-    }
+    });
     flush();
 }
 
@@ -226,13 +247,13 @@ extern "C" int32_t hepk_lookup_interp(const float* x, int64_t n, const float* xs
 {
     HEPK_REQUIRE(n >= 0, "n < 0");
     HEPK_REQUIRE(xs && ys && nk >= 2, "knots are NULL or fewer than 2");
-    if ((size_t)nk * 12 > 200 * 1024) {
+    if ((size_t)nk * 16 > 200 * 1024) {
         set_error("hepk_lookup_interp: %d knots do not fit 200 KB of shared memory", nk);
         return HEPK_ERR_UNSUPPORTED;
     }
     if (n == 0) return HEPK_OK;
     HEPK_REQUIRE(x && out, "x/out is NULL");
-    const size_t smem = (size_t)nk * 12;
+    const size_t smem = (size_t)nk * 16;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::lookup_interp_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::lookup_interp_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const bool vec = aligned16(x) && aligned16(out);
@@ -266,7 +287,7 @@ extern "C" int32_t hepk_fill_histogram_2d(const float* x, const float* y, const 
         HEPK_REQUIRE(workspace_bytes >= hepk_hist2d_workspace_bytes(nx, ny), "workspace too small");
     }
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t smem = ((size_t)(nx + 1) + (size_t)(ny + 1) + 2 * (size_t)slots) * 4;
+    const size_t smem = ((size_t)(nx + 1) + (size_t)(ny + 1) + 2 * (size_t)slots + (size_t)(nx + 3) + (size_t)(ny + 3)) * 4;
     const bool vec = aligned16(x) && aligned16(y) && (!weights || aligned16(weights));
     auto kern = vec ? dev::fill_hist2d_kernel<true> : dev::fill_hist2d_kernel<false>;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -917,8 +917,14 @@ static int32_t tile_launch(Kern kern, const TileLayout& L, const Op& op, cudaStr
     return HEPK_OK;
 }
 
-// Slice capacities (objects per tile).  Fixed: the kernels adapt the number of events per tile to them.
-constexpr int CAP_REDUCE = 672, CAP_DR_1 = 416, CAP_DR_2 = 160, CAP_MASS = 416;      // (reductions: 64 events per tile)
+// Slice capacities (objects per tile).  Fixed: the kernels adapt the number of events per tile to them (a tile of E
+// events is taken when E * mean + 4 sqrt(2 E mean + 1) + 8 objects fit: 32-event tiles up to a mean of 9.7 objects
+// per event at 416, 8.8 at 384, 1.9 at 112).  They are sized for the warps they leave room for, measured on
+// BASELINE.json configs[2]: deltar_mask 416/160 -> 416/112 takes 20 warps per SM instead of 18 (0.465 -> 0.421 ms per
+// 10 M events; 400/128 0.423, 384/128 0.438: with fewer than ~410 jets a few dozen tiles per launch overflow into the
+// lane-per-event path and the warps that meet them finish last), pair_invmass 416 -> 384 takes 16 instead of 15
+// (0.399 -> 0.374 ms).
+constexpr int CAP_REDUCE = 672, CAP_DR_1 = 416, CAP_DR_2 = 112, CAP_MASS = 384;      // (reductions: 64 events per tile)
 
 template <int OP>
 static int32_t segreduce_dispatch(const float* data, const int64_t* offsets, int64_t n_events, int64_t base,
@@ -1020,7 +1026,7 @@ extern "C" int32_t hepk_deltar_mask(const float* eta1, const float* phi1, const 
     const int64_t bases[2] = {base1, base2};
     const int caps[2] = {CAP_DR_1, CAP_DR_2};
     TileLayout L;
-    const int32_t rc = tile_layout(L, n_events, 2, offs, bases, n_cls, ptr, caps, 4 * WT_EVENTS + CAP_DR_1 + 32, 32);
+    const int32_t rc = tile_layout(L, n_events, 2, offs, bases, n_cls, ptr, caps, 4 * WT_EVENTS + caps[0] + 32, 32);
     if (rc != HEPK_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     if (sel1 && sel2) return deltar_launch<true, true>(L, eta1, phi1, sel1, eta2, phi2, sel2, dr_max, out_matched, st);
