@@ -76,7 +76,7 @@ __device__ __forceinline__ void hist_fill_scales(const HistParams& P, float& sc,
 }
 
 template <bool VEC>
-__global__ void __launch_bounds__(256) hist_fill_kernel(const __grid_constant__ HistParams P)
+__global__ void __launch_bounds__(256, 6) hist_fill_kernel(const __grid_constant__ HistParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* s_ex = (float*)smem_raw;
@@ -203,36 +203,33 @@ __global__ void __launch_bounds__(256) event_weight_lookup_kernel(const float* _
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* s_e = (float*)smem_raw;
     float* s_t = s_e + (nb + 1);
-    float* s_p = s_t + nb;                          // padded copy of the edges (pad_axis_find, bin form)
     for (int i = threadIdx.x; i <= nb; i += blockDim.x) s_e[i] = edges[i];
     for (int i = threadIdx.x; i < nb; i += blockDim.x) s_t[i] = table[i];
     __syncthreads();
-    pad_axis_fill<false>(s_p, s_e, nb);
-    const AxisGuess ax = classify_axis(s_e, nb);      // (its barriers publish s_p)
-    const float top = (float)(nb - 1);
+    // (HBM bound as it is: the padded-axis form of the guess saves a third of the instructions and no time here, and
+    // its longer set-up showed in back-to-back calls of this 21 us kernel)
+    const AxisGuess ax = classify_axis(s_e, nb);
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool vec = ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(w_out) | reinterpret_cast<uintptr_t>(w_in)) & 15u) == 0;
-    dispatch_axis(ax.mode, [&](auto tx) {
-        constexpr int AX = decltype(tx)::value;
-        auto factor = [&](float v) { return s_t[pad_axis_find<AX, false>(v, s_e, s_p, nb, ax, top)]; };
-        if (vec) {
-            const long long n4 = n / 4;
-            for (long long g = t0; g < n4; g += stride) {
-                const float4 xv = __ldg((const float4*)x + g);
-                const float4 wv = w_in ? __ldg((const float4*)w_in + g) : make_float4(1.f, 1.f, 1.f, 1.f);
-                float4 o;
-                o.x = __fmul_rn(wv.x, factor(xv.x));
-                o.y = __fmul_rn(wv.y, factor(xv.y));
-                o.z = __fmul_rn(wv.z, factor(xv.z));
-                o.w = __fmul_rn(wv.w, factor(xv.w));
-                ((float4*)w_out)[g] = o;
-            }
-            for (long long i = n4 * 4 + t0; i < n; i += stride) w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, factor(x[i]));
-        } else {
-            for (long long i = t0; i < n; i += stride) w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, factor(x[i]));
+    if (vec) {
+        const long long n4 = n / 4;
+        for (long long g = t0; g < n4; g += stride) {
+            const float4 xv = __ldg((const float4*)x + g);
+            const float4 wv = w_in ? __ldg((const float4*)w_in + g) : make_float4(1.f, 1.f, 1.f, 1.f);
+            float4 o;
+            o.x = __fmul_rn(wv.x, s_t[find_bin_guess(xv.x, s_e, nb, ax)]);
+            o.y = __fmul_rn(wv.y, s_t[find_bin_guess(xv.y, s_e, nb, ax)]);
+            o.z = __fmul_rn(wv.z, s_t[find_bin_guess(xv.z, s_e, nb, ax)]);
+            o.w = __fmul_rn(wv.w, s_t[find_bin_guess(xv.w, s_e, nb, ax)]);
+            ((float4*)w_out)[g] = o;
         }
-    });
+        for (long long i = n4 * 4 + t0; i < n; i += stride)
+            w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, s_t[find_bin_guess(x[i], s_e, nb, ax)]);
+    } else {
+        for (long long i = t0; i < n; i += stride)
+            w_out[i] = __fmul_rn(w_in ? w_in[i] : 1.0f, s_t[find_bin_guess(x[i], s_e, nb, ax)]);
+    }
 }
 
 // measurement hook: lane-atomics of red.shared.add.s32 per launch, random addresses in `nbins` words
@@ -456,7 +453,7 @@ extern "C" int32_t hepk_event_weight_lookup(const float* w_in, const float* x, i
     }
     if (n == 0) return HEPK_OK;
     HEPK_REQUIRE(x && w_out, "x/w_out is NULL");
-    const size_t smem = (size_t)(3 * nbins + 2) * 4;
+    const size_t smem = (size_t)(2 * nbins + 1) * 4;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::event_weight_lookup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dev::event_weight_lookup_kernel<<<grid_for_items((n + 3) / 4), 256, smem, (cudaStream_t)stream>>>(w_in, x, n, edges, nbins,
                                                                                                     table, w_out); count_launch();

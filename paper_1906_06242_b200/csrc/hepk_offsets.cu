@@ -54,6 +54,17 @@ __global__ void set_in_offsets_kernel(float* __restrict__ data, const long long*
 
 }  // namespace dev
 
+// one wave of resident CTAs (kernels that stage tables once per CTA and merge privatised bins at its end)
+static unsigned grid_resident(const void* kern, size_t smem, long long items)
+{
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem) != cudaSuccess || occ < 1) occ = 1;
+    long long blocks = (items + 255) / 256;
+    const long long maxb = (long long)sm_count() * occ;
+    if (blocks > maxb) blocks = maxb;
+    return (unsigned)(blocks < 1 ? 1 : blocks);
+}
+
 static unsigned grid_for(long long n)
 {
     long long blocks = (n + 255) / 256;
@@ -153,7 +164,7 @@ __global__ void __launch_bounds__(256) lookup_interp_kernel(const float* __restr
 // accumulated (native shared-memory atomics) and the weighted sums are taken from them when the bins are flushed;
 // with weights the float32 partial sums (compare-and-swap atomics) are flushed into float64 at bounded intervals.
 template <bool VEC>
-__global__ void __launch_bounds__(256) fill_hist2d_kernel(const float* __restrict__ x, const float* __restrict__ y,
+__global__ void __launch_bounds__(256, 6) fill_hist2d_kernel(const float* __restrict__ x, const float* __restrict__ y,
                                                           const float* __restrict__ w, long long n,
                                                           const float* __restrict__ edges_x, int nx,
                                                           const float* __restrict__ edges_y, int ny,
@@ -258,7 +269,7 @@ extern "C" int32_t hepk_lookup_interp(const float* x, int64_t n, const float* xs
     HEPK_CUDA_TRY(cudaFuncSetAttribute(dev::lookup_interp_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const bool vec = aligned16(x) && aligned16(out);
     auto kern = vec ? dev::lookup_interp_kernel<true> : dev::lookup_interp_kernel<false>;
-    kern<<<grid_for(vec ? (n + 3) / 4 : n), 256, smem, (cudaStream_t)stream>>>(x, n, xs, ys, nk, out); count_launch();
+    kern<<<grid_resident((const void*)kern, smem, vec ? (n + 3) / 4 : n), 256, smem, (cudaStream_t)stream>>>(x, n, xs, ys, nk, out); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
     return HEPK_OK;
 }
@@ -292,7 +303,7 @@ extern "C" int32_t hepk_fill_histogram_2d(const float* x, const float* y, const 
     auto kern = vec ? dev::fill_hist2d_kernel<true> : dev::fill_hist2d_kernel<false>;
     HEPK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (sumw) HEPK_CUDA_TRY(cudaMemsetAsync(workspace, 0, (size_t)slots * sizeof(double), st));
-    unsigned grid = grid_for((n + 3) / 4);
+    unsigned grid = grid_resident((const void*)kern, smem, (n + 3) / 4);
     kern<<<grid, 256, smem, st>>>(x, y, weights, n, edges_x, nx, edges_y, ny, sumw ? (double*)workspace : nullptr,
                                   (unsigned long long*)counts); count_launch();
     HEPK_CUDA_TRY(cudaGetLastError());
