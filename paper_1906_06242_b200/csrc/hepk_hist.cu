@@ -17,7 +17,7 @@
 namespace hepk {
 namespace dev {
 
-enum { HH_WMAX = 0, HH_WMIN = 1, HH_BAD = 2, HH_WORDS = 4 };
+enum { HH_WMAX = 0, HH_WMIN = 1, HH_BAD = 2, HH_DONE = 3 /* CTAs of the lane-private fill that have finished */, HH_WORDS = 4 };
 constexpr int HIST_FIXED_WORDS = 1024;      // privatised words a CTA can afford to check after every step
 constexpr int HIST_FLUSH_AT = 1 << 29;
 
@@ -316,11 +316,12 @@ static int32_t hist_fill_launch(const char* who, const float* x, const float* y,
             dev::LaneHistOut o;
             o.sumw = nullptr; o.counts = nullptr; o.acc = P.acc;
             o.WS = h.WS; o.want_sumw = h.want_sumw; o.col_w2 = h.col_w2; o.col_cnt = h.col_cnt;
+            // the last CTA to finish adds the rows to the caller's arrays (what hist_finalize_kernel does for float64 rows)
+            o.done = (unsigned int*)workspace + dev::HH_DONE;
+            o.fin_sumw = sumw; o.fin_sumw2 = sumw2; o.fin_counts = counts;
             const size_t sm = head + (size_t)warps * per_warp;
             HEPK_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
             k<<<sm_count(), warps * 32, sm, st>>>(x, weights, n, edges_x, nx, o); count_launch();
-            HEPK_CUDA_TRY(cudaGetLastError());
-            dev::hist_finalize_kernel<<<(unsigned)((h.slots + 255) / 256), 256, 0, st>>>(P); count_launch();
             HEPK_CUDA_TRY(cudaGetLastError());
             return HEPK_OK;
         }

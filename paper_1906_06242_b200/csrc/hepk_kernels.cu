@@ -253,6 +253,7 @@ extern "C" int32_t hepk_fill_histogram(const float* data, const float* weights, 
             dev::LaneHistOut o;
             o.sumw = sumw; o.counts = (unsigned long long*)counts; o.acc = nullptr;
             o.WS = 0; o.want_sumw = 0; o.col_w2 = -1; o.col_cnt = -1;
+            o.done = nullptr; o.fin_sumw = nullptr; o.fin_sumw2 = nullptr; o.fin_counts = nullptr;
             HEPK_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
             k<<<sm_count(), warps * 32, sm, st>>>(data, weights, n, edges, nbins, o); count_launch();
             HEPK_CUDA_TRY(cudaGetLastError());
