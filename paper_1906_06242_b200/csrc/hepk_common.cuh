@@ -111,6 +111,16 @@ __device__ __forceinline__ void red_shared_add_f32(void* p, float v)
     asm volatile("red.shared.add.f32 [%0], %1;" ::"r"(smem_u32(p)), "f"(v) : "memory");
 }
 
+// the same on a shared-memory byte address (smem_u32 taken once outside the loop: the conversion is three instructions)
+__device__ __forceinline__ void red_shared_add_u32_at(uint32_t a, unsigned int v)
+{
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_shared_add_f32_at(uint32_t a, float v)
+{
+    asm volatile("red.shared.add.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory");
+}
+
 // ---- staging a slice [l0, l1) of a column into shared memory -----------------------------------
 // Element l of `col` lands at dst[l - a0], a0 <= l0 chosen so that the 16-byte aligned body of the slice
 // can be moved by ONE bulk copy; the ragged head (col not 16-byte aligned near element 0) and the tail
@@ -200,7 +210,9 @@ __device__ __forceinline__ AxisGuess classify_axis(const float* s_edges, int n)
     const float inv1 = (float)n / (hi - lo);
     const float l0 = __log2f(lo), inv2 = (float)n / (__log2f(hi) - l0);
     bool ok1 = (hi > lo) && (inv1 > 0.0f) && (inv1 < CUDART_INF_F);
-    bool ok2 = (lo > 0.0f) && (hi > lo) && (inv2 > 0.0f) && (inv2 < CUDART_INF_F);
+    // (mode 2 wants a NORMAL first edge: pad_axis_find's log2 flushes denormal values to zero, which is only right when
+    // every denormal value lies below the axis)
+    bool ok2 = (lo >= 1.17549435e-38f) && (hi > lo) && (inv2 > 0.0f) && (inv2 < CUDART_INF_F);
     for (int i = threadIdx.x; i <= n; i += blockDim.x) {
         ok1 = ok1 && (fabsf((s_edges[i] - lo) * inv1 - (float)i) <= 0.45f);
         ok2 = ok2 && (fabsf((__log2f(s_edges[i]) - l0) * inv2 - (float)i) <= 0.45f);
@@ -269,8 +281,18 @@ __device__ __forceinline__ int pad_axis_find(float v, const float* s_edges, cons
     if (AXIS == 0) return SLOTS ? axis_slot(v, s_edges, n, a) : find_bin_guess(v, s_edges, n, a);
     const float one = SLOTS ? 1.0f : 0.0f;
     float pos;
-    if (AXIS == 1) pos = fmaf(v - a.lo, a.inv, one);
-    else pos = v > 0.0f ? fmaf(__log2f(v) - a.lo, a.inv, one) : (v != v ? top : 0.0f);
+    if (AXIS == 1) {
+        pos = fmaf(v - a.lo, a.inv, one);
+    } else {
+        // One MUFU and no branch: lg2.approx.ftz gives -inf for zeros and denormals (clamped to the first slot below, where
+        // they belong: the first edge is a normal float), NaN for NaN (-> top, as for any NaN) and NaN for negative values,
+        // which belong in the first slot instead: one select.  (__log2f without -ftz is five instructions, and the
+        // three-way test on v a branch.)
+        float lg;
+        asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(v));
+        pos = fmaf(lg - a.lo, a.inv, one);
+        pos = v < 0.0f ? 0.0f : pos;
+    }
     int s = (int)fmaxf(fminf(pos, top), 0.0f);
     const float e0 = s_pad[s], e1 = s_pad[s + 1];
     s += (v >= e1) ? 1 : 0;

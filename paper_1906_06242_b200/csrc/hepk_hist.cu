@@ -101,6 +101,8 @@ __global__ void __launch_bounds__(256, 6) hist_fill_kernel(const __grid_constant
     ay.mode = 1; ay.lo = 0.f; ay.inv = 0.f;        // (one dimension: the tag of the unused axis)
     if (P.ny > 0) ay = classify_axis(s_ey, P.ny);
     const float top_x = (float)(P.nx + 1), top_y = (float)(P.ny + 1);
+    const uint32_t bins_a = smem_u32(s_bins);
+    const uint32_t w2_off = 4u * (unsigned)(P.col_w2 >= 0 ? P.col_w2 : 0), cnt_off = 4u * (unsigned)(P.col_cnt >= 0 ? P.col_cnt : 0);
 
     // move bins into the global accumulators; `all`: everything non-zero, else only integers about to overflow
     auto flush = [&](bool all) {
@@ -131,20 +133,20 @@ __global__ void __launch_bounds__(256, 6) hist_fill_kernel(const __grid_constant
             return s;
         };
         auto put = [&](int s, float wv) {
-            int* row = s_bins + s * P.WS;
+            const uint32_t row = bins_a + 4u * (unsigned)(s * P.WS);
             if (fixed) {
-                if (P.want_sumw) red_shared_add_u32(row, (unsigned int)__float2int_rn(wv * sc));
+                if (P.want_sumw) red_shared_add_u32_at(row, (unsigned int)__float2int_rn(wv * sc));
                 if (P.col_w2 >= 0) {
                     const float y2 = wv * wv * sc2;
                     const int qh = __float2int_rn(y2);
-                    red_shared_add_u32(row + P.col_w2, (unsigned int)qh);
-                    red_shared_add_u32(row + P.col_w2 + 1, (unsigned int)__float2int_rn((y2 - (float)qh) * 1048576.0f));
+                    red_shared_add_u32_at(row + w2_off, (unsigned int)qh);
+                    red_shared_add_u32_at(row + w2_off + 4u, (unsigned int)__float2int_rn((y2 - (float)qh) * 1048576.0f));
                 }
             } else {
-                if (P.want_sumw) red_shared_add_f32(row, wv);
-                if (P.col_w2 >= 0) red_shared_add_f32(row + P.col_w2, wv * wv);
+                if (P.want_sumw) red_shared_add_f32_at(row, wv);
+                if (P.col_w2 >= 0) red_shared_add_f32_at(row + w2_off, wv * wv);
             }
-            if (P.col_cnt >= 0) red_shared_add_u32(row + P.col_cnt, 1u);
+            if (P.col_cnt >= 0) red_shared_add_u32_at(row + cnt_off, 1u);
         };
         if (VEC) {
             const long long n4 = P.n / 4;

@@ -204,6 +204,7 @@ __global__ void __launch_bounds__(256, 6) fill_hist2d_kernel(const float* __rest
     };
     const float top_x = (float)(nx + 1), top_y = (float)(ny + 1);
     const int row = ny + 2;
+    const uint32_t sumw_a = smem_u32(s_sumw), cnt_a = smem_u32(s_cnt);
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     dispatch_axes(ax.mode, ay.mode, [&](auto tx, auto ty) {
@@ -212,8 +213,8 @@ __global__ void __launch_bounds__(256, 6) fill_hist2d_kernel(const float* __rest
             return pad_axis_find<AX, true>(xv, s_ex, s_px, nx, ax, top_x) * row + pad_axis_find<AY, true>(yv, s_ey, s_py, ny, ay, top_y);
         };
         auto put = [&](int s, float wv) {
-            if (fsum) red_shared_add_f32(&s_sumw[s], wv);
-            if (icnt) red_shared_add_u32(&s_cnt[s], 1u);
+            if (fsum) red_shared_add_f32_at(sumw_a + 4u * (unsigned)s, wv);
+            if (icnt) red_shared_add_u32_at(cnt_a + 4u * (unsigned)s, 1u);
         };
         if (VEC) {
             const long long n4 = n >> 2;
