@@ -136,8 +136,8 @@ int32_t hepk_pair_invmass(const float* pt, const float* eta, const float* phi, c
  *   out[i] = table[B(x[i], edges_x, nx) * ny + B(y[i], edges_y, ny)]     (y == NULL: table[B(x[i])])
  *   B(v) = the b with edges[b] <= v < edges[b+1], clamped: v < edges[0] -> 0; v >= edges[n] or NaN -> n-1.
  * x, y: float32[n]; edges_x: float32[nx+1] ascending; edges_y: float32[ny+1]; table: float32[nx*ny]
- * row-major, no flow bins; out: float32[n].  Limit: (nx+1)+(ny+1)+nx*ny floats must fit 200 KB of
- * shared memory, else HEPK_ERR_UNSUPPORTED. */
+ * row-major, no flow bins; out: float32[n].  Limit: 2*(nx+1)+2*(ny+1)+nx*ny floats (the edges, a padded copy of
+ * them for the bin search, the table) must fit 200 KB of shared memory, else HEPK_ERR_UNSUPPORTED. */
 int32_t hepk_lookup_binned(const float* x, const float* y, int64_t n,
                            const float* edges_x, int32_t nx, const float* edges_y, int32_t ny,
                            const float* table, float* out, void* stream);
@@ -302,8 +302,8 @@ int32_t hepk_select_opposite_sign(const float* pt, const int32_t* charge, const 
  *   knots xs[0..nk) ascending with values ys[0..nk), nk >= 2;
  *   out[i] = ys[b] + (x[i] - xs[b]) * (ys[b+1] - ys[b]) / (xs[b+1] - xs[b])  for xs[b] <= x[i] < xs[b+1];
  *   x <= xs[0] -> ys[0], x >= xs[nk-1] -> ys[nk-1] (constant extrapolation), NaN -> NaN.
- * Tolerance class (float32 evaluation with one slope per segment).  12*nk bytes of shared memory, more than 200 KB ->
- * HEPK_ERR_UNSUPPORTED. */
+ * Tolerance class (float32 evaluation with one slope per segment).  16*nk bytes of shared memory (knots, values,
+ * slopes, a padded copy of the knots for the segment search), more than 200 KB (nk > 12,800) -> HEPK_ERR_UNSUPPORTED. */
 int32_t hepk_lookup_interp(const float* x, int64_t n, const float* xs, const float* ys, int32_t nk, float* out, void* stream);
 
 /* Two-dimensional weighted histogram ("Extension to multidimensional histograms is straightforward"):
@@ -326,7 +326,8 @@ int32_t hepk_fill_histogram_2d(const float* x, const float* y, const float* weig
  * partial sums of at most 32768 entries merged in float64 (one dimension with few bins: a private copy of the
  * bins per lane, hepk_hist_lanes.cuh), or fixed-point bins (exact integer sums) for small histograms whose
  * weights are finite and within a factor 8 of each other.  nbins+2 (resp. (nx+2)*(ny+2))
- * <= 16384 and rows x columns must fit 200 KB of shared memory, else HEPK_ERR_UNSUPPORTED. */
+ * <= 16384 and rows x columns (plus two copies of the edges) must fit 200 KB of shared memory, else
+ * HEPK_ERR_UNSUPPORTED. */
 size_t  hepk_hist_workspace_bytes(int32_t nx, int32_t ny);
 int32_t hepk_fill_histogram_w2(const float* data, const float* weights, int64_t n, const float* edges, int32_t nbins,
                                float* sumw, float* sumw2, int64_t* counts, void* workspace, size_t workspace_bytes,

@@ -151,3 +151,37 @@ def test_large_one_axis_histogram_takes_the_general_kernel(hk):
         assert_exact(to_np(gc), rc, "counts")
         assert_tol(to_np(gs), rs, "sumw")
         assert_tol(to_np(g2), r2, "sumw2")
+
+
+def test_tables_at_the_shared_memory_limits(hk):
+    """The largest tables each entry accepts (include/hepk.h states the limits; the padded copies of the edges count),
+    and one step beyond: refused with HEPK_ERR_UNSUPPORTED, never a launch with too little shared memory."""
+    rng = np.random.default_rng(5)
+    # lookup_interp: 16 bytes of shared memory per knot, 200 KB
+    for nk, log in ((12_800, False), (12_800, True)):
+        xs = (np.geomspace(1.0, 1e5, nk) if log else np.linspace(0.0, 1000.0, nk)).astype(np.float32)
+        ys = rng.uniform(0.9, 1.1, nk).astype(np.float32)
+        x = values(xs[::37], rng, 200_001)
+        assert_tol(to_np(hk.lookup_interp(cu(x), cu(xs), cu(ys))), hepo.lookup_interp(x, xs, ys), "lookup_interp, 12,800 knots")
+    xs = np.linspace(0.0, 1000.0, 12_801).astype(np.float32)
+    with pytest.raises(hk.HepkError):
+        hk.lookup_interp(cu(xs), cu(xs), cu(xs))
+    # lookup_binned: 2 (nx + 1) + 2 (ny + 1) + nx ny floats, 200 KB
+    ex, ey = np.linspace(-5.0, 5.0, 201).astype(np.float32), np.geomspace(10.0, 5000.0, 241).astype(np.float32)
+    table = rng.uniform(0.5, 1.5, (200, 240)).astype(np.float32)
+    x, y = values(ex, rng, 200_001), values(ey, rng, 200_001)
+    assert_exact(to_np(hk.lookup_binned(cu(x), cu(y), cu(ex), cu(ey), cu(table))), hepo.lookup_binned(x, y, ex, ey, table),
+                 "lookup_binned, 200 x 240 table")
+    ex2 = np.linspace(-5.0, 5.0, 221).astype(np.float32)
+    with pytest.raises(hk.HepkError):
+        hk.lookup_binned(cu(x), cu(y), cu(ex2), cu(ey), cu(np.zeros((220, 240), np.float32)))
+    # fill_histogram_2d: (nx + 2) (ny + 2) = 16384 slots
+    ex, ey = np.linspace(-3.0, 3.0, 127).astype(np.float32), np.geomspace(20.0, 2000.0, 127).astype(np.float32)
+    x, y = values(ex, rng, 300_001), values(ey, rng, 300_001)
+    w = rng.normal(1.0, 0.1, x.size).astype(np.float32)
+    sw_ref, ct_ref = hepo.fill_histogram_2d(x, y, w, ex, ey)
+    sw, ct = hk.fill_histogram_2d(cu(x), cu(y), cu(w), cu(ex), cu(ey))
+    assert_exact(to_np(ct), ct_ref, "fill_histogram_2d counts, 16384 slots")
+    assert_tol(to_np(sw), sw_ref, "fill_histogram_2d sumw, 16384 slots")
+    with pytest.raises(hk.HepkError):
+        hk.fill_histogram_2d(cu(x), cu(y), None, cu(np.linspace(-3.0, 3.0, 128).astype(np.float32)), cu(ey))
